@@ -1,0 +1,175 @@
+"""ctypes binding of oracle/neb_oracle.c — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package; it imports nothing from paper_2606_24154_b200 and the CUDA path imports nothing
+from here.  Two builds of the same C source: `f64` (real = double, the timed CPU baseline) and
+`ld` (real = long double, the truth for parity tests).  See the header of neb_oracle.c for the
+passages each function follows and the list of pins.
+"""
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "neb_oracle.c")
+_LIBS = {"f64": os.path.join(_HERE, "liborc_f64.so"), "ld": os.path.join(_HERE, "liborc_ld.so")}
+_FLAGS = {"f64": [], "ld": ["-DORC_LONG_DOUBLE"]}
+_cache = {}
+
+EPS0 = 8.8541878128e-12          # reading S3 (the same CODATA value is restated in the C source)
+K_COULOMB = 1.0 / (4.0 * np.pi * EPS0)
+
+
+def build(force: bool = False) -> None:
+    """gcc -O2 -fopenmp (no -ffast-math), both precisions."""
+    for mode, lib in _LIBS.items():
+        if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-ffp-contract=off",
+                   *_FLAGS[mode], _SRC, "-o", lib, "-lm"]
+            subprocess.check_call(cmd)
+
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_lp = C.POINTER(C.c_int64)
+
+
+def _lib(mode: str):
+    if mode not in _cache:
+        build()
+        L = C.CDLL(_LIBS[mode])
+        L.orc_real_bytes.restype = C.c_int
+        L.orc_threads.restype = C.c_int
+        L.orc_lu_factor.restype = C.c_void_p
+        L.orc_lu_factor.argtypes = [C.c_int64, _dp, _ip]
+        L.orc_lu_solve.argtypes = [C.c_void_p, _dp, _dp]
+        L.orc_lu_free.argtypes = [C.c_void_p]
+        L.orc_solve.restype = C.c_int32
+        _cache[mode] = L
+    return _cache[mode]
+
+
+def _d(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a, t=_dp):
+    return None if a is None else a.ctypes.data_as(t)
+
+
+def threads(mode="f64") -> int:
+    return int(_lib(mode).orc_threads())
+
+
+def influence(kind, v0, e1, e2, P, radius=0.0, mode="ld"):
+    """(Phi', E'x, E'y, E'z) of one element at one point, primed (no 1/4 pi eps0, no sigma)."""
+    v0, e1, e2, P = (_d(x) for x in (v0, e1, e2, P))
+    out = np.zeros(4)
+    _lib(mode).orc_influence(C.c_int32(int(kind)), _p(v0), _p(e1), _p(e2), C.c_double(float(radius)), _p(P), _p(out))
+    return out
+
+
+class Geometry:
+    """Holds contiguous SoA copies of a workloads.configs.Problem's arrays for the C calls."""
+
+    def __init__(self, pr, colloc=None):
+        self.n = int(pr.kind.shape[0])
+        self.kind = np.ascontiguousarray(pr.kind, dtype=np.int32)
+        self.v0, self.e1, self.e2 = _d(pr.v0), _d(pr.e1), _d(pr.e2)
+        self.radius = _d(pr.radius)
+        self.colloc = _d(pr.centroids() if colloc is None else colloc)
+        self.bc_kind = np.ascontiguousarray(pr.bc_kind, dtype=np.int32)
+        self.bc_value = _d(pr.bc_value)
+        self.eps_plus, self.eps_minus = _d(pr.eps_plus), _d(pr.eps_minus)
+        self.img = _d(pr.img_shift)
+        self.n_img = 0 if self.img is None else int(self.img.shape[1])
+
+    def _geo(self):
+        return (C.c_int64(self.n), _p(self.kind, _ip), _p(self.v0), _p(self.e1), _p(self.e2), _p(self.radius))
+
+
+def assemble(g: Geometry, mode="ld") -> np.ndarray:
+    """K[i, j], row i = collocation point i, column j = source element j (LHMatrix)."""
+    K = np.zeros((g.n, g.n))
+    _lib(mode).orc_assemble(*g._geo(), _p(g.colloc), _p(g.bc_kind, _ip), _p(g.eps_plus), _p(g.eps_minus),
+                            C.c_int32(g.n_img), _p(g.img), _p(K))
+    return K
+
+
+def matrix_entries(g: Geometry, rows, cols, mode="ld") -> np.ndarray:
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    cols = np.ascontiguousarray(cols, dtype=np.int64)
+    vals = np.zeros(rows.shape[0])
+    _lib(mode).orc_matrix_entries(*g._geo(), _p(g.colloc), _p(g.bc_kind, _ip), _p(g.eps_plus), _p(g.eps_minus),
+                                  C.c_int32(g.n_img), _p(g.img), C.c_int64(rows.shape[0]), _p(rows, _lp),
+                                  _p(cols, _lp), _p(vals))
+    return vals
+
+
+def rhs(g: Geometry, charge_pos=None, charge_q=None, mode="ld") -> np.ndarray:
+    b = np.zeros(g.n)
+    pos, ch = _d(charge_pos), _d(charge_q)
+    q = 0 if ch is None else int(ch.shape[0])
+    _lib(mode).orc_rhs(C.c_int64(g.n), _p(g.e1), _p(g.e2), _p(g.colloc), _p(g.bc_kind, _ip), _p(g.bc_value),
+                       C.c_int64(q), _p(pos), _p(ch), _p(b))
+    return b
+
+
+def solve(K: np.ndarray, b: np.ndarray, mode="ld") -> np.ndarray:
+    K, b = _d(K), _d(b)
+    x = np.zeros_like(b)
+    st = _lib(mode).orc_solve(C.c_int64(K.shape[0]), _p(K), _p(b), _p(x))
+    if st != 0:
+        raise np.linalg.LinAlgError(f"oracle LU: status {st}")
+    return x
+
+
+class LU:
+    """Factor once, re-solve many times (reading S13)."""
+
+    def __init__(self, K, mode="ld"):
+        self._L = _lib(mode)
+        K = _d(K)
+        self.n = K.shape[0]
+        st = C.c_int32(0)
+        self._h = self._L.orc_lu_factor(C.c_int64(self.n), _p(K), C.byref(st))
+        if st.value != 0:
+            raise np.linalg.LinAlgError(f"oracle LU: status {st.value}")
+
+    def solve(self, b):
+        b = _d(b)
+        x = np.zeros_like(b)
+        self._L.orc_lu_solve(C.c_void_p(self._h), _p(b), _p(x))
+        return x
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._L.orc_lu_free(C.c_void_p(self._h))
+            self._h = None
+
+
+def point_charges(pts, charge_pos, charge_q, mode="ld"):
+    pts, pos, ch = _d(pts), _d(charge_pos), _d(charge_q)
+    m = pts.shape[1]
+    phi, E = np.zeros(m), np.zeros((3, m))
+    _lib(mode).orc_point_charges(C.c_int64(m), _p(pts), C.c_int64(ch.shape[0]), _p(pos), _p(ch), _p(phi), _p(E))
+    return phi, E
+
+
+def evaluate(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="ld"):
+    """Phi (m), E (3, m) at pts (3, m) from elements with densities sigma, plus space charges."""
+    sigma, pts, pos, ch = _d(sigma), _d(pts), _d(charge_pos), _d(charge_q)
+    m = pts.shape[1]
+    q = 0 if ch is None else int(ch.shape[0])
+    phi, E = np.zeros(m), np.zeros((3, m))
+    _lib(mode).orc_eval(*g._geo(), _p(sigma), C.c_int32(g.n_img), _p(g.img), C.c_int64(q), _p(pos), _p(ch),
+                        C.c_int64(m), _p(pts), _p(phi), _p(E))
+    return phi, E
+
+
+def push(pos, E, mu, dt, mode="ld"):
+    pos = np.array(pos, dtype=np.float64, order="C")
+    E = _d(E)
+    _lib(mode).orc_push(C.c_int64(pos.shape[1]), _p(pos), _p(E), C.c_double(mu), C.c_double(dt))
+    return pos

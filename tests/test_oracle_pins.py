@@ -1,0 +1,475 @@
+"""Pins of the CPU oracle to things other than itself (SURVEY.md §8(c) "What pins the oracle").
+
+Every expected value here comes from brute-force quadrature of the paper's defining integrals
+(P:121), from a closed form / invariant the mathematics fixes, from a physical
+constant, or from a library routine (numpy.linalg) — never from oracle/ or the CUDA path.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from workloads import configs as W
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+RECT, TRI, WIRE = 0, 1, 2
+PI = np.pi
+
+
+def local_elem(kind, a, b):
+    """Element in the local frame of P:119: XZ plane from the origin, normal +Y (wires on X)."""
+    return dict(kind=kind, v0=[0, 0, 0], e1=[a, 0, 0], e2=[0, 0, b if kind != WIRE else 0.0])
+
+
+def infl(orc, kind, a, b, P, mode="ld", radius=0.0):
+    e = local_elem(kind, a, b)
+    return orc.influence(e["kind"], e["v0"], e["e1"], e["e2"], P, radius=radius, mode=mode)
+
+
+# ---------------------------------------------------------------------------------------------
+# 1. brute-force quadrature of the defining integrals (stored pins, mpmath 30 digits)
+# ---------------------------------------------------------------------------------------------
+def _gold_cases():
+    out = []
+    with open(os.path.join(GOLD, "quadrature_pins.txt")) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            t = line.split()
+            out.append((t[0], float(t[1]), float(t[2]), [float(x) for x in t[3:6]], np.array([float(x) for x in t[6:10]])))
+    return out
+
+
+@pytest.mark.parametrize("mode,tol", [("ld", 2e-14), ("f64", 5e-12)])
+def test_quadrature_pins(orc, mode, tol):
+    cases = _gold_cases()
+    assert len(cases) >= 15
+    for kind, a, b, P, want in cases:
+        k = {"rect": RECT, "tri": TRI, "wire": WIRE}[kind]
+        if k == WIRE:
+            r = 1e-3
+            got = infl(orc, k, a, b, P, mode, radius=r) / (2 * PI * r)      # S24: lambda = 2 pi r_w sigma
+        else:
+            got = infl(orc, k, a, b, P, mode)
+        scale = max(abs(want[0]), np.linalg.norm(want[1:]))
+        assert np.max(np.abs(got - want)) <= tol * scale, (kind, a, b, P, got, want)
+
+
+# ---------------------------------------------------------------------------------------------
+# 2. independent tensor Gauss-Legendre quadrature (numpy) at random non-singular points, random
+#    orientation in space: pins the local-frame convention and the rotation of E' to global
+# ---------------------------------------------------------------------------------------------
+def _gl_quadrature(kind, v0, e1, e2, P, n=96):
+    x, w = np.polynomial.legendre.leggauss(n)
+    s = 0.5 * (x + 1.0)
+    ws = 0.5 * w
+    if kind == WIRE:
+        src = v0[:, None] + e1[:, None] * s[None, :]
+        wt = ws * np.linalg.norm(e1)
+    else:
+        S, T = np.meshgrid(s, s, indexing="ij")
+        WS, WT = np.meshgrid(ws, ws, indexing="ij")
+        if kind == TRI:                     # collapsed map: z runs to (1 - s) of the second leg
+            T = T * (1.0 - S)
+            WT = WT * (1.0 - S)
+        src = v0[:, None] + e1[:, None] * S.ravel()[None, :] + e2[:, None] * T.ravel()[None, :]
+        wt = (WS * WT).ravel() * np.linalg.norm(np.cross(e1, e2))
+    d = P[:, None] - src
+    r = np.linalg.norm(d, axis=0)
+    return np.concatenate([[np.sum(wt / r)], (d / r ** 3) @ wt])
+
+
+@pytest.mark.parametrize("kind", [RECT, TRI, WIRE])
+def test_random_orientation_vs_gauss_legendre(orc, kind):
+    pr = W.random_elements(24, seed=11 + kind, kinds=(kind,), size_mm=(0.3, 1.0))
+    rs = np.random.RandomState(5 + kind)
+    worst = 0.0
+    for j in range(pr.n):
+        v0, e1, e2 = pr.v0[:, j], pr.e1[:, j], pr.e2[:, j]
+        L = max(np.linalg.norm(e1), np.linalg.norm(e2))
+        c = v0 + 0.5 * e1 + (0.5 * e2 if kind != WIRE else 0)
+        u = rs.normal(size=3)
+        u /= np.linalg.norm(u)
+        P = c + u * L * rs.uniform(1.2, 4.0)                # distance >= 0.2 L from the element
+        want = _gl_quadrature(kind, v0, e1, e2, P)
+        rad = 1e-6
+        got = orc.influence(kind, v0, e1, e2, P, radius=rad, mode="ld")
+        if kind == WIRE:
+            got = got / (2 * PI * rad)
+        scale = max(abs(want[0]), np.linalg.norm(want[1:]))
+        worst = max(worst, np.max(np.abs(got - want)) / scale)
+    assert worst < 1e-12, worst
+
+
+# ---------------------------------------------------------------------------------------------
+# 3. closed forms the mathematics fixes
+# ---------------------------------------------------------------------------------------------
+def test_rectangle_centre_closed_form(orc):
+    # Phi' at the centre of an a x b rectangle = 2[a asinh(b/a) + b asinh(a/b)]; field vanishes (symmetry, S5)
+    for a, b in [(2.0, 3.0), (1.0, 1.0), (0.01, 7.0)]:
+        got = infl(orc, RECT, a, b, [a / 2, 0.0, b / 2])
+        want = 2 * (a * np.arcsinh(b / a) + b * np.arcsinh(a / b))
+        assert abs(got[0] - want) < 1e-14 * want
+        assert np.max(np.abs(got[1:])) < 1e-14
+    assert abs(infl(orc, RECT, 2.0, 3.0, [1.0, 0.0, 1.5])[0] - 8.5299235726509373) < 1e-13   # SURVEY value, a=2,b=3
+    a = 1.7
+    assert abs(infl(orc, RECT, a, a, [a / 2, 0, a / 2])[0] - 4 * a * np.log(1 + np.sqrt(2))) < 1e-14
+
+
+def test_square_on_axis_closed_form(orc):
+    # Phi' = 2a ln[(r+a/2)/(r-a/2)] - 4h atan(a^2/(4hr)),  E'_y = 4 atan(a^2/(4hr)),  r = sqrt(a^2/2+h^2)
+    for a, h in [(1.0, 0.3), (2.5, 0.01), (1.0, 40.0)]:
+        r = np.sqrt(a * a / 2 + h * h)
+        phi = 2 * a * np.log((r + a / 2) / (r - a / 2)) - 4 * h * np.arctan(a * a / (4 * h * r))
+        ey = 4 * np.arctan(a * a / (4 * h * r))
+        for sgn in (+1, -1):
+            got = infl(orc, RECT, a, a, [a / 2, sgn * h, a / 2])
+            assert abs(got[0] - phi) < 2e-13 * phi
+            assert abs(got[2] - sgn * ey) < 2e-13 * ey
+            assert abs(got[1]) < 1e-13 and abs(got[3]) < 1e-13
+
+
+def test_triangle_centroid_solid_angle_limit(orc):
+    # just above the interior the element fills half of space: Omega -> 2 pi, E'_y -> +-2 pi
+    for sgn in (+1, -1):
+        got = infl(orc, TRI, 1.0, 1.0, [1 / 3, sgn * 1e-9, 1 / 3])
+        assert abs(got[2] - sgn * 2 * PI) < 1e-7
+    got = infl(orc, TRI, 1.0, 1.0, [1 / 3, 0.0, 1 / 3])
+    assert got[2] == 0.0                                   # reading S5: principal value on the surface
+    assert abs(got[1] - got[3]) < 1e-14                    # mirror symmetry of the isosceles right triangle
+
+
+def test_wire_closed_form_midplane(orc):
+    # mid-plane of a wire of length 2h: Phi' = 2 asinh(h/rho); E' radial = 2h/(rho sqrt(rho^2+h^2))
+    h, rho, rw = 0.5, 0.2, 1e-3
+    got = orc.influence(WIRE, [0, 0, -h], [0, 0, 2 * h], [0, 0, 0], [rho, 0, 0], radius=rw) / (2 * PI * rw)
+    assert abs(got[0] - 2 * np.arcsinh(h / rho)) < 1e-14
+    assert abs(got[1] - 2 * h / (rho * np.hypot(rho, h))) < 1e-13
+    assert abs(got[2]) < 1e-15 and abs(got[3]) < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# 4. far-field limit Eq.(2) P:68 and E = -grad Phi P:75
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", [RECT, TRI, WIRE])
+def test_far_field_monopole(orc, kind):
+    a, b = 1.0, 0.6
+    area = {RECT: a * b, TRI: 0.5 * a * b, WIRE: a}[kind]
+    cen = {RECT: np.array([a / 2, 0, b / 2]), TRI: np.array([a / 3, 0, b / 3]), WIRE: np.array([a / 2, 0, 0])}[kind]
+    u = np.array([0.3, -0.5, 0.81]); u /= np.linalg.norm(u)
+    prev = None
+    for R in (50.0, 100.0, 200.0):
+        rw = 1e-3
+        got = infl(orc, kind, a, b, cen + R * u, radius=rw)
+        if kind == WIRE:
+            got = got / (2 * PI * rw)
+        err = abs(got[0] * R / area - 1.0)
+        assert err < 0.6 * (a / R) ** 2                      # O((L/r)^2): no dipole about the centroid
+        assert np.linalg.norm(got[1:] * R * R / area - u) < 2 * (a / R) ** 2
+        if prev is not None:
+            assert err < 0.3 * prev                          # and it really falls off quadratically
+        prev = err
+
+
+@pytest.mark.parametrize("kind", [RECT, TRI, WIRE])
+def test_field_is_minus_gradient(orc, kind):
+    pr = W.random_elements(16, seed=40 + kind, kinds=(kind,), size_mm=(0.3, 1.0))
+    rs = np.random.RandomState(17)
+    for j in range(pr.n):
+        v0, e1, e2 = pr.v0[:, j], pr.e1[:, j], pr.e2[:, j]
+        L = max(np.linalg.norm(e1), np.linalg.norm(e2))
+        P = v0 + 0.4 * e1 + 0.3 * e2 + rs.normal(size=3) * L * 0.7
+        rad = pr.radius[j]
+        if kind == WIRE:                                     # stay outside the wire surface
+            P = P + 5 * rad * np.cross(e1 / np.linalg.norm(e1), [0.3, 0.5, 0.8])
+        f = lambda Q: orc.influence(kind, v0, e1, e2, Q, radius=rad, mode="ld")
+        E = f(P)[1:]
+        h = 1e-5 * L
+        G = np.array([(f(P + h * np.eye(3)[c])[0] - f(P - h * np.eye(3)[c])[0]) / (2 * h) for c in range(3)])
+        assert np.linalg.norm(E + G) < 1e-7 * np.linalg.norm(E), (j, E, G)
+
+
+# ---------------------------------------------------------------------------------------------
+# 5. additivity and invariances
+# ---------------------------------------------------------------------------------------------
+def test_rectangle_is_two_right_triangles(orc):
+    a, b = 1.0, 0.7
+    for P in ([0.3, 0.25, 0.4], [0.9, -0.1, 0.1], [2.0, 0.0, -1.0], [0.5, 1e-4, 0.35]):
+        r = orc.influence(RECT, [0, 0, 0], [a, 0, 0], [0, 0, b], P)
+        t1 = orc.influence(TRI, [0, 0, 0], [a, 0, 0], [0, 0, b], P)
+        # complementary triangle: right angle at (a,0,b), legs -e1 and -e2 (same normal: (-e2)x(-e1) = e2 x e1)
+        t2 = orc.influence(TRI, [a, 0, b], [-a, 0, 0], [0, 0, -b], P)
+        assert np.max(np.abs(r - t1 - t2)) < 2e-14 * max(1.0, np.max(np.abs(r)))
+    assert abs(orc.influence(RECT, [0, 0, 0], [a, 0, 0], [0, 0, b], [0.3, 0.25, 0.4])[0] - 1.67956850898329) < 1e-13
+
+
+def test_rectangle_is_four_subrectangles(orc):
+    a, b, sx, sz = 1.3, 0.9, 0.45, 0.7
+    for P in ([0.37, 0.21, -0.45], [0.45, 0.0, 0.7], [0.1, -0.02, 0.2]):
+        whole = orc.influence(RECT, [0, 0, 0], [a, 0, 0], [0, 0, b], P)
+        parts = sum(orc.influence(RECT, [x0, 0, z0], [dx, 0, 0], [0, 0, dz], P)
+                    for x0, dx in ((0, sx), (sx, a - sx)) for z0, dz in ((0, sz), (sz, b - sz)))
+        # at the shared corner (second point) the sub-rectangles' in-plane fields are log-singular (S6): Phi' only
+        idx = [0, 2] if P[1] == 0.0 else [0, 1, 2, 3]
+        assert np.max(np.abs(whole - parts)[idx]) < 3e-14 * max(1.0, np.max(np.abs(whole)))
+
+
+def test_rotation_translation_invariance(orc):
+    rs = np.random.RandomState(3)
+    for kind in (RECT, TRI, WIRE):
+        A, _ = np.linalg.qr(rs.normal(size=(3, 3)))
+        if np.linalg.det(A) < 0:
+            A[:, 0] = -A[:, 0]
+        t = rs.normal(size=3)
+        v0, e1, e2, P = np.array([0.1, 0.2, -0.3]), np.array([0.8, 0, 0]), np.array([0, 0, 0.5]), np.array([0.5, 0.3, 0.9])
+        ref = orc.influence(kind, v0, e1, e2, P, radius=0.01)
+        got = orc.influence(kind, A @ v0 + t, A @ e1, A @ e2, A @ P + t, radius=0.01)
+        assert abs(got[0] - ref[0]) < 1e-14 * abs(ref[0])
+        assert np.linalg.norm(got[1:] - A @ ref[1:]) < 1e-14 * np.linalg.norm(ref[1:])
+
+
+def test_normal_convention_and_side(orc):
+    # n = e2 x e1 / |..| (include/neb.h); E' points away from the element on both sides
+    v0, e1, e2 = np.array([0, 0, 0.0]), np.array([0, 1.0, 0]), np.array([1.0, 0, 0])      # n = x cross y = +z
+    up = orc.influence(RECT, v0, e1, e2, [0.5, 0.5, 0.2])
+    dn = orc.influence(RECT, v0, e1, e2, [0.5, 0.5, -0.2])
+    assert up[3] > 0 and dn[3] < 0 and abs(up[3] + dn[3]) < 1e-15 and abs(up[0] - dn[0]) < 1e-15
+
+
+def test_gauss_law_closed_cube(orc):
+    # sum over the faces of a closed cube of n_j.E'_j(P) = sum sgn(d_j) Omega_j = -4 pi inside, 0 outside
+    pr = W.cube(n_side=2, m_points=1)
+    nrm = pr.normals()
+    for P, want in (([1e-3, -2e-3, 1.5e-3], -4 * PI), ([0.0, 0.0, 0.0], -4 * PI), ([9e-3, 1e-3, -2e-3], 0.0),
+                    ([-6e-3, 7e-3, 8e-3], 0.0)):
+        tot = 0.0
+        for j in range(pr.n):
+            o = orc.influence(RECT, pr.v0[:, j], pr.e1[:, j], pr.e2[:, j], P)
+            tot += float(np.dot(nrm[:, j], o[1:]))
+        assert abs(tot - want) < 1e-12, (P, tot)
+
+
+def test_edge_and_corner_limits_are_finite(orc):
+    # reading S6: on an edge / corner / edge extension nothing is inf or NaN and Phi' stays exact
+    a, b = 1.0, 0.6
+    on_edge = infl(orc, RECT, a, b, [0.4, 0.0, 0.0])
+    corner = infl(orc, RECT, a, b, [0.0, 0.0, 0.0])
+    ext = infl(orc, RECT, a, b, [1.7, 0.0, 0.0])
+    for v in (on_edge, corner, ext):
+        assert np.all(np.isfinite(v))
+    # Phi' at a corner of an a x b rectangle: a asinh(b/a) + b asinh(a/b) (quarter of the centre value of 2a x 2b)
+    assert abs(corner[0] - (a * np.arcsinh(b / a) + b * np.arcsinh(a / b))) < 1e-14
+    # Phi' on an edge at abscissa s: two corner values
+    s = 0.4
+    want = sum(x * np.arcsinh(b / x) + b * np.arcsinh(x / b) for x in (s, a - s))
+    assert abs(on_edge[0] - want) < 1e-14
+    for v in (infl(orc, TRI, a, b, [0.5, 0.0, 0.3]), infl(orc, TRI, a, b, [0, 0, 0]), infl(orc, TRI, a, b, [0.3, 0, 0])):
+        assert np.all(np.isfinite(v))
+
+
+# ---------------------------------------------------------------------------------------------
+# 6. point charges (Eq. 2, Alg. 2)
+# ---------------------------------------------------------------------------------------------
+def test_point_charge_coulomb_constant_and_skip(orc):
+    # 1 C at 1 m: Phi = k_e = 8.9875517923e9 V (CODATA), |E| = k_e V/m, pointing away
+    pts = np.array([[1.0, 0.0], [0.0, 0.0], [0.0, 0.0]])
+    phi, E = orc.point_charges(pts, np.zeros((3, 1)), np.array([1.0]))
+    assert abs(phi[0] / 8.9875517923e9 - 1) < 1e-10
+    assert abs(E[0, 0] / 8.9875517923e9 - 1) < 1e-10 and E[1, 0] == 0 and E[2, 0] == 0
+    assert phi[1] == 0 and np.all(E[:, 1] == 0)            # r = 0 contributes nothing (S11)
+
+
+def test_point_charge_superposition_and_gradient(orc):
+    rs = np.random.RandomState(0)
+    pos, q = rs.normal(size=(3, 50)), rs.normal(size=50)
+    P = np.array([[3.0], [-2.0], [1.5]])
+    phi, E = orc.point_charges(P, pos, q)
+    one = sum(orc.point_charges(P, pos[:, k:k + 1], q[k:k + 1])[0][0] for k in range(50))
+    assert abs(phi[0] - one) < 1e-12 * abs(phi[0])
+    h = 1e-5
+    G = [(orc.point_charges(P + h * np.eye(3)[:, c:c + 1], pos, q)[0][0]
+          - orc.point_charges(P - h * np.eye(3)[:, c:c + 1], pos, q)[0][0]) / (2 * h) for c in range(3)]
+    assert np.linalg.norm(E[:, 0] + G) < 1e-8 * np.linalg.norm(E[:, 0])
+    # far away the cloud is a monopole
+    far = np.array([[4e3], [3e3], [0.0]])
+    phi_f, _ = orc.point_charges(far, pos, q)
+    assert abs(phi_f[0] - 8.9875517923e9 * q.sum() / 5e3) < 2e-3 * abs(phi_f[0])
+
+
+# ---------------------------------------------------------------------------------------------
+# 7. dense solve (Alg. 1; S13, S15, S16) against numpy.linalg
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["ld", "f64"])
+def test_lu_against_numpy(orc, mode):
+    rs = np.random.RandomState(1)
+    n = 200
+    K = rs.normal(size=(n, n))
+    K[np.arange(n), np.arange(n)] = 0.0                      # forces row exchanges
+    K *= 10.0 ** rs.uniform(-6, 6, size=(n, 1))              # rows spanning 12 decades (S15)
+    b = rs.normal(size=n) * np.abs(K).max(axis=1)
+    x = orc.solve(K, b, mode=mode)
+    want = np.linalg.solve(K / np.abs(K).max(axis=1, keepdims=True), b / np.abs(K).max(axis=1))
+    assert np.max(np.abs(x - want)) < 1e-9 * np.max(np.abs(want))
+    lu = orc.LU(K, mode=mode)
+    b2 = rs.normal(size=n)
+    x2 = lu.solve(b2)
+    rowmax = np.abs(K).max(axis=1)
+    assert np.max(np.abs(K @ x2 - b2) / rowmax) < 1e-12 * n * np.max(np.abs(x2))     # S16 residual, row-scaled
+    with pytest.raises(np.linalg.LinAlgError):
+        orc.solve(np.zeros((4, 4)), np.ones(4), mode=mode)
+
+
+# ---------------------------------------------------------------------------------------------
+# 8. whole pipeline on problems with known answers
+# ---------------------------------------------------------------------------------------------
+def _solve_dirichlet(orc, pr, mode="f64"):
+    g = orc.Geometry(pr)
+    K = orc.assemble(g, mode=mode)
+    b = orc.rhs(g, mode=mode)
+    return g, K, orc.solve(K, b, mode=mode)
+
+
+def _areas(pr):
+    a = np.linalg.norm(np.cross(pr.e1.T, pr.e2.T), axis=1)
+    return np.where(pr.kind == TRI, 0.5 * a, a)
+
+
+def test_c0_plate_charge_density_and_capacitance(orc):
+    pr = W.plate()
+    g, K, sig = _solve_dirichlet(orc, pr)
+    n = 16
+    S = sig.reshape(n, n)
+    # the 8 symmetries of the square
+    for T in (S.T, S[::-1], S[:, ::-1], S[::-1, ::-1].T):
+        assert np.max(np.abs(T - S)) < 1e-12 * S.max()
+    # edge peaking: monotone from centre to edge along a row, largest at the corners, smallest at the centre
+    assert np.all(np.diff(S[n // 2, n // 2:]) > 0)
+    assert S.max() == pytest.approx(S[0, 0]) and S.min() == pytest.approx(S[n // 2, n // 2])
+    # capacitance of a square plate of side a: C/(4 pi eps0 a) = 0.3667896 (literature value, 7 digits);
+    # uniform panels converge to it from below (16x16 gives 0.3593, 2 % low)
+    a = pr.meta["side"]
+    cap = np.sum(sig * _areas(pr)) / (4 * PI * orc.EPS0 * a)
+    assert 0.355 < cap < 0.3668
+    cap8 = np.sum(_solve_dirichlet(orc, W.plate(n_side=8))[2] * _areas(W.plate(n_side=8))) / (4 * PI * orc.EPS0 * a)
+    assert cap8 < cap
+    # boundary condition reproduced at the collocation points by the evaluation path (assembly/eval consistent)
+    phi, _ = orc.evaluate(g, sig, g.colloc, mode="f64")
+    assert np.max(np.abs(phi - 1.0)) < 1e-12
+    # on-axis field: odd in z, no transverse component; potential even in z
+    pts = np.array([[0, 0, 0, 0], [0, 0, 0, 0], [1e-3, -1e-3, 5e-3, -5e-3]], dtype=float)
+    phi, E = orc.evaluate(g, sig, pts, mode="f64")
+    assert abs(phi[0] - phi[1]) < 1e-13 and abs(E[2, 0] + E[2, 1]) < 1e-10 * abs(E[2, 0])
+    assert np.max(np.abs(E[:2])) < 1e-9 * abs(E[2, 0])
+    assert 0.5 < phi[2] < phi[0] < 1.0 and E[2, 0] > 0 and E[2, 1] < 0
+
+
+def test_c1_cube_capacitance_sequence(orc):
+    # unit-cube capacitance C/(4 pi eps0 a) = 0.66078 (literature, 5 digits); uniform-panel BEM converges from below
+    caps = []
+    for ns in (4, 6, 8, 12):
+        pr = W.cube(n_side=ns, m_points=1)
+        _, _, sig = _solve_dirichlet(orc, pr)
+        caps.append(np.sum(sig * _areas(pr)) / (4 * PI * orc.EPS0 * pr.meta["side"]))
+    assert np.all(np.diff(caps) > 0) and caps[-1] < 0.6608
+    assert abs(caps[-1] - 0.6608) < 0.004
+    # Richardson with error ~ 1/ns
+    rich = (12 * caps[3] - 8 * caps[2]) / 4
+    assert abs(rich - 0.6608) < 1.5e-3
+    # inside a closed conductor Phi = V and E = 0 up to discretisation error
+    pr = W.cube(n_side=8, m_points=1)
+    g, _, sig = _solve_dirichlet(orc, pr)
+    phi, E = orc.evaluate(g, sig, np.array([[1e-3], [-2e-3], [0.5e-3]]), mode="f64")
+    assert abs(phi[0] - 1.0) < 2e-3
+    e_surface = sig.mean() / orc.EPS0
+    assert np.linalg.norm(E[:, 0]) < 2e-2 * e_surface
+
+
+def test_two_plate_capacitor_uniform_field(orc):
+    # stand-in for the paper's Case 1: between large plates the field tends to V/gap
+    side, gap, ns = 10.0, 0.5, 20
+    top, bot = W.plate(n_side=ns, side_mm=side, volt=+0.5, m_points=1), W.plate(n_side=ns, side_mm=side, volt=-0.5, m_points=1)
+    top.v0[2] += gap / 2 * W.MM
+    bot.v0[2] -= gap / 2 * W.MM
+    pr = _concat(top, bot)
+    g, _, sig = _solve_dirichlet(orc, pr)
+    phi, E = orc.evaluate(g, sig, np.zeros((3, 1)), mode="f64")
+    assert abs(phi[0]) < 1e-9
+    assert abs(E[2, 0] / (-1.0 / (gap * W.MM)) - 1) < 5e-3
+
+
+def _concat(*prs):
+    cat = lambda k: np.concatenate([getattr(p, k) for p in prs], axis=-1)
+    return W.Problem(name="+".join(p.name for p in prs), kind=cat("kind"), v0=cat("v0"), e1=cat("e1"), e2=cat("e2"),
+                     radius=cat("radius"), bc_kind=cat("bc_kind"), bc_value=cat("bc_value"), eps_plus=cat("eps_plus"),
+                     eps_minus=cat("eps_minus"))
+
+
+def _sheet(ns, side_mm, z_mm, normal_sign, **bc):
+    b = W._Builder()
+    p = side_mm / ns
+    ia, ib = W._grid_cells(ns, ns)
+    b.rect_cells((-side_mm / 2, -side_mm / 2, z_mm), (p, 0, 0), (0, p, 0), ia, ib, (0, 0, normal_sign), **bc)
+    return b.finish("sheet")
+
+
+def test_point_charge_over_dielectric_half_space(orc):
+    # dielectric rows only (reading S8 sign and lambda, S10 RHS): coplanar panels exert no normal field on each
+    # other, so K is diagonal and sigma_i equals the textbook image-solution bound charge at every centroid:
+    #   sigma_b(rho) = -(q / 2 pi) (eps_r - 1)/(eps_r + 1) d / (rho^2 + d^2)^(3/2)
+    eps_r, d, q = 4.4, 0.7e-3, 3e-15
+    pr = _sheet(10, 4.0, 0.0, +1, bc_kind=W.DIELECTRIC, bc_value=0.0, eps_plus=1.0, eps_minus=eps_r)
+    g = orc.Geometry(pr)
+    K = orc.assemble(g, mode="ld")
+    off = K - np.diag(np.diag(K))
+    assert np.max(np.abs(off)) == 0.0
+    b = orc.rhs(g, np.array([[0.0], [0.0], [d]]), np.array([q]), mode="ld")
+    sig = orc.solve(K, b, mode="ld")
+    rho2 = g.colloc[0] ** 2 + g.colloc[1] ** 2
+    want = -(q / (2 * PI)) * (eps_r - 1) / (eps_r + 1) * d / (rho2 + d * d) ** 1.5
+    assert np.max(np.abs(sig - want)) < 1e-13 * np.max(np.abs(want))
+
+
+def test_dielectric_slab_in_capacitor(orc):
+    # plates +-0.5 V at z=+-0.5 mm, slab faces at z=+-0.2 mm, eps_r=4.4, all W x W with W=8 mm, 20x20 panels each.
+    # central |E_z|: gas 1/(0.6+0.4/4.4) V/mm = 1.447368, slab 0.328947 (series capacitor), finite-size error ~1e-4
+    ns, Wd = 20, 8.0
+    pr = _concat(_sheet(ns, Wd, +0.5, -1, bc_kind=W.DIRICHLET, bc_value=+0.5),
+                 _sheet(ns, Wd, -0.5, +1, bc_kind=W.DIRICHLET, bc_value=-0.5),
+                 _sheet(ns, Wd, +0.2, +1, bc_kind=W.DIELECTRIC, bc_value=0.0, eps_plus=1.0, eps_minus=4.4),
+                 _sheet(ns, Wd, -0.2, -1, bc_kind=W.DIELECTRIC, bc_value=0.0, eps_plus=1.0, eps_minus=4.4))
+    g, _, sig = _solve_dirichlet(orc, pr)
+    # keep off the panel centroids' singular normal-field jump: evaluate mid-gas and mid-slab on the axis
+    _, E = orc.evaluate(g, sig, np.array([[0.0, 0.0], [0.0, 0.0], [0.35e-3, 0.0]]), mode="f64")
+    assert abs(abs(E[2, 0]) * 1e-3 / 1.447368 - 1) < 5e-4
+    assert abs(abs(E[2, 1]) * 1e-3 / 0.328947 - 1) < 5e-4
+    assert E[2, 0] < 0 and E[2, 1] < 0                      # from the +0.5 V plate down to the -0.5 V plate
+
+
+def test_image_copies_equal_explicit_replication(orc):
+    # reading S12: summing shifted copies inside each coefficient == meshing the copies explicitly with shared sigma
+    pr = W.random_elements(6, seed=9, kinds=(RECT, TRI), size_mm=(0.2, 0.5), box_mm=0.4, m_points=5)
+    shifts = W.image_shifts(1, pitch_mm=1.0)
+    pr.img_shift = shifts
+    g = orc.Geometry(pr)
+    sig = np.linspace(1.0, 2.0, pr.n) * 1e-6
+    phi, E = orc.evaluate(g, sig, pr.points)
+    reps = []
+    for s in range(shifts.shape[1]):
+        c = W.random_elements(6, seed=9, kinds=(RECT, TRI), size_mm=(0.2, 0.5), box_mm=0.4)
+        c.v0 = c.v0 + shifts[:, s:s + 1]
+        reps.append(c)
+    big = _concat(*reps)
+    phi2, E2 = orc.evaluate(orc.Geometry(big), np.tile(sig, shifts.shape[1]), pr.points)
+    assert np.max(np.abs(phi - phi2)) < 1e-13 * np.max(np.abs(phi))
+    assert np.max(np.abs(E - E2)) < 1e-13 * np.max(np.abs(E))
+    K = orc.assemble(g)
+    Kbig = orc.assemble(orc.Geometry(big))
+    fold = sum(Kbig[:pr.n, s * pr.n:(s + 1) * pr.n] for s in range(shifts.shape[1]))
+    assert np.max(np.abs(K - fold)) < 1e-13 * np.max(np.abs(K))
+
+
+def test_push_is_axpy(orc):
+    pos = np.array([[1.0, 2.0], [3.0, 4.0], [5.0, 6.0]])
+    E = np.array([[1e3, 0.0], [0.0, -2e3], [4e3, 0.0]])
+    out = orc.push(pos, E, mu=1.5e-4, dt=1e-9)
+    assert out[0, 0] == 1.0 + 1.5e-4 * 1e3 * 1e-9 and out[1, 1] == 4.0 - 1.5e-4 * 2e3 * 1e-9 and out[2, 1] == 6.0
