@@ -1,0 +1,151 @@
+/* neb.h — C ABI of the B200-native neBEM hot path (libneb.so).
+ *
+ * The calls follow the paper's statement of the problem (arxiv 2606.24154; "P:n" = line n of
+ * PAPER.md) and BASELINE.json's north_star:
+ *   neb_assemble         = LHMatrix()                         (Eq.(6))
+ *   neb_solve            = InvertMatrix() + RHVector() + ValueKnCh() + Solve()  (Alg.1)
+ *   neb_eval             = PFAtPoint() = ElePFAtPoint() + KnChPFAtPoint()       (Eq.(3),(4) P:70-78)
+ *   neb_add_space_charge = UpdateSpaceCharge()                (Alg.2)
+ *   neb_solve again      = UpdateFields(): RHVector() + Solve() on resident factors (Alg.4)
+ *
+ * Conventions common to every call
+ *   - Plain C; no exception crosses the boundary; every call returns a neb_status and
+ *     neb_last_error() holds a message for the last non-OK status of that context.
+ *   - SI units: metres, volts, coulombs, C/m^2.  eps0 = 8.8541878128e-12 F/m.
+ *   - Vectors are SoA: an array "3*n" is x[0..n) then y[0..n) then z[0..n).
+ *   - Every array pointer may be a HOST or a DEVICE pointer (detected with
+ *     cudaPointerGetAttributes; device pointers must live on the context's device).  Inputs are
+ *     borrowed for the duration of the call and copied; outputs are caller-owned.
+ *   - Work is ordered on the CUDA stream given to neb_create.  A call synchronises that stream
+ *     only when it has to write to host memory.
+ *   - Everything runs in the CUDA kernels of this library.  There is no CPU fallback: without a
+ *     usable device neb_create fails with NEB_ECUDA.
+ *   - State machine: create -> assemble -> (add_space_charge)* -> solve -> eval*; out-of-order
+ *     calls return NEB_ESTATE.  neb_set_sigma also unlocks neb_eval.
+ */
+#ifndef NEB_H
+#define NEB_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct neb_ctx neb_ctx; /* opaque; owns every device buffer it allocates */
+
+typedef enum {
+  NEB_OK = 0,
+  NEB_EINVAL = 1,    /* bad argument (NULL, negative size, unknown kind, degenerate element)  */
+  NEB_ENOMEM = 2,    /* device or host allocation failed                                     */
+  NEB_ESTATE = 3,    /* call out of order                                                    */
+  NEB_ESINGULAR = 4, /* zero or NaN pivot in the LU                                          */
+  NEB_ECUDA = 5      /* CUDA runtime error; message in neb_last_error                        */
+} neb_status;
+
+enum { NEB_RECT = 0, NEB_TRI = 1, NEB_WIRE = 2 };       /* element kinds  */
+enum { NEB_BC_DIRICHLET = 0, NEB_BC_DIELECTRIC = 1 };   /* row kinds                            */
+
+/* Options for neb_set_option. */
+enum {
+  NEB_OPT_MATH = 0,     /* 1 (default): hand-written log/atan2/sqrt/rcp sequences; 0: CUDA libm  */
+  NEB_OPT_LU_BLOCK = 1, /* LU panel width nb (multiple of 32, 32..256); default 128              */
+  NEB_OPT_PROFILE = 2   /* 1: record per-stage CUDA-event timings (neb_stage_ms); default 0      */
+};
+
+/* Stages for neb_stage_ms. */
+enum {
+  NEB_STAGE_GEOMETRY = 0, /* a1 frame tables                                   */
+  NEB_STAGE_ASSEMBLE = 1, /* a3 influence matrix kernel                        */
+  NEB_STAGE_EQUIL = 2,    /* row equilibration (reading S15)                   */
+  NEB_STAGE_LU = 3,       /* a5 factorisation                                  */
+  NEB_STAGE_LU_GEMM = 4,  /* a5 trailing update (DMMA) only, subset of LU      */
+  NEB_STAGE_RHS = 5,      /* a4                                                */
+  NEB_STAGE_TRISOLVE = 6, /* a6                                                */
+  NEB_STAGE_EVAL = 7,     /* a7 fused element kernel                           */
+  NEB_STAGE_CHARGES = 8,  /* a8 point-charge direct sum                        */
+  NEB_STAGE_COUNT = 9
+};
+
+/* Creates a context on `device`.  `cuda_stream` is a cudaStream_t (e.g. torch's current stream),
+ * NULL = the legacy default stream.  NEB_ECUDA if the device is absent or not sm_100. */
+neb_status neb_create(neb_ctx** out, int device, void* cuda_stream);
+void neb_destroy(neb_ctx* ctx);
+const char* neb_last_error(const neb_ctx* ctx);
+neb_status neb_set_option(neb_ctx* ctx, int32_t option, int64_t value);
+
+/* LHMatrix: builds the frame tables (a1) and the dense n*n fp64 influence matrix (a3)
+ * on the device, column-major, and scales its rows (S15).
+ *
+ * Elements, in GLOBAL coordinates (length n each; vectors 3*n SoA):
+ *   kind      NEB_RECT / NEB_TRI / NEB_WIRE
+ *   v0        corner (rect), right-angle vertex (tri), start point (wire)
+ *   e1, e2    the two perpendicular edge vectors from v0 (rect: sides; tri: legs, hypotenuse from
+ *             v0+e1 to v0+e2, P:123-127 with reading S2; wire: e1 = axis vector, e2 ignored).
+ *             The unit normal is n = e2 x e1 / |e2 x e1|, so that (e1^, n, e2^) is the paper's
+ *             local (X, Y, Z) of P:119.
+ *   radius    wire radius r_w (wires only; may be NULL if there are no wires).  A wire's
+ *             sigma is a surface density: line density = 2 pi r_w sigma (reading S24).
+ *   colloc    3*n collocation points, or NULL = centroids (S4: rectangle centre, triangle
+ *             v0+(e1+e2)/3, wire: mid-length on the surface).
+ *   bc_kind   NEB_BC_DIRICHLET: row i is  sum_j K_ij sigma_j = bc_value[i] - Phi_sc(p_i)   (Eq.5)
+ *             NEB_BC_DIELECTRIC: row i is the normal-displacement condition (reading S8)
+ *               sum_j (1/4 pi eps0) n_i.E'_j(p_i) sigma_j + sigma_i/(2 eps0 lambda_i) = -n_i.E_sc(p_i),
+ *               lambda_i = (eps_plus - eps_minus)/(eps_plus + eps_minus); eps_plus is the relative
+ *               permittivity on the +n side.  bc_value is ignored on these rows.
+ *   eps_plus, eps_minus   may be NULL if no row is dielectric.
+ *   n_img, img_shift      periodic copies (reading S12): 3*n_img SoA shift vectors, which must
+ *             include (0,0,0); every coefficient sums the element's copies.  NULL / 0 = none.
+ *             The same copies are applied by neb_eval; never to space charges.
+ * Errors: NEB_EINVAL (n <= 0, NULL required array, unknown kind, zero-length edge, wire without
+ * radius, eps_plus == eps_minus on a dielectric row), NEB_ENOMEM, NEB_ECUDA. */
+neb_status neb_assemble(neb_ctx* ctx, int64_t n, const int32_t* kind, const double* v0, const double* e1,
+                        const double* e2, const double* radius, const double* colloc, const int32_t* bc_kind,
+                        const double* bc_value, const double* eps_plus, const double* eps_minus, int32_t n_img,
+                        const double* img_shift);
+
+/* InvertMatrix + RHVector + Solve.  The first call factorises P K = L U in place (blocked,
+ * partial pivoting, trailing update on FP64 DMMA; factors stay resident, no explicit inverse:
+ * reading S13).  Every call forms the RHS from the boundary values and the current space
+ * charges (S10) and does the two triangular solves.  sigma_out (n) may be NULL.
+ * Errors: NEB_ESTATE before neb_assemble; NEB_ESINGULAR. */
+neb_status neb_solve(neb_ctx* ctx, double* sigma_out);
+
+/* Test hook: sets the charge densities directly (n values, caller's element order). */
+neb_status neb_set_sigma(neb_ctx* ctx, const double* sigma);
+
+/* PFAtPoint: Phi (m) and E (3*m SoA) at m points pts (3*m SoA) from all elements (with
+ * their periodic copies) and all space charges; a charge exactly at a point is skipped
+ * (reading S11).  Either output may be NULL.  m = 0 is allowed. */
+neb_status neb_eval(neb_ctx* ctx, int64_t m, const double* pts, double* phi, double* E);
+
+/* UpdateSpaceCharge: q point charges, pos 3*q SoA (m), charge in coulomb.
+ * replace != 0 discards the charges held so far; q = 0 with replace clears them. */
+neb_status neb_add_space_charge(neb_ctx* ctx, int64_t q, const double* pos, const double* charge, int32_t replace);
+
+/* Charge push of the synthetic dynamic loop (BASELINE configs[4], reading S23): pos += mu_dt * E,
+ * 3*q values, in place.  Stateless; pos and E must both be device or both be host pointers. */
+neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, double mu_dt);
+
+/* Test hooks.  neb_get_matrix: the UNSCALED matrix in the caller's element order, n*n
+ * column-major (K_out[i + j*n] = row i, column j); only between neb_assemble and the first
+ * neb_solve (NEB_ESTATE afterwards: the factors overwrite it).  neb_get_rhs: the RHS the last
+ * neb_solve used (unscaled, caller's order). */
+neb_status neb_get_matrix(neb_ctx* ctx, double* K_out);
+neb_status neb_get_rhs(neb_ctx* ctx, double* b_out);
+
+/* Measurement aids: register-only FP64 microbenchmarks on all SMs.
+ * kind 0: DFMA chains; kind 1: mma.sync m8n8k4 f64 (DMMA).  Result in TFLOP/s (FMA = 2 flop). */
+neb_status neb_fp64_peak(neb_ctx* ctx, int32_t kind, double* tflops);
+
+/* Accumulated device time (ms) and number of kernel launches of a stage since the last
+ * neb_reset_stats; valid when NEB_OPT_PROFILE is 1.  neb_launch_count counts every kernel this
+ * library launched on the context since creation (profiling on or off). */
+neb_status neb_stage_ms(neb_ctx* ctx, int32_t stage, double* ms, int64_t* launches);
+neb_status neb_reset_stats(neb_ctx* ctx);
+int64_t neb_launch_count(const neb_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEB_H */

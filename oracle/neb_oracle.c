@@ -236,21 +236,25 @@ void orc_influence(int32_t kind, const double* v0, const double* e1, const doubl
 }
 
 /* Sum over periodic copies (reading S12): the copy of element j shifted by +s seen from P equals
- * element j seen from P - s. */
+ * element j seen from P - s.  self_pv != 0 marks the pair (collocation point of element j, element j
+ * itself): the unshifted copy then contributes NO field — the principal value of the normal field of
+ * a flat element at a point of its own surface is zero (readings S5, S8: "self term 0 for a flat
+ * element, but its image copies do contribute").  The rule is applied by index, not by testing Y == 0,
+ * because the centroid of an obliquely oriented element is only in its plane up to rounding. */
 static void elem_influence_images(const elems_t* g, int64_t j, const real P[3], int32_t n_img,
-                                  const double* img, long double acc[4]) {
+                                  const double* img, int self_pv, long double acc[4]) {
   for (int k = 0; k < 4; ++k) acc[k] = 0;
-  if (n_img <= 0 || !img) {
-    real o[4];
-    elem_influence(g, j, P, o);
-    for (int k = 0; k < 4; ++k) acc[k] = o[k];
-    return;
-  }
-  for (int32_t s = 0; s < n_img; ++s) {
-    real Ps[3] = {P[0] - (real)img[s], P[1] - (real)img[n_img + s], P[2] - (real)img[2 * n_img + s]};
+  int32_t copies = (n_img <= 0 || !img) ? 1 : n_img;
+  for (int32_t s = 0; s < copies; ++s) {
+    real sh[3] = {0, 0, 0};
+    if (n_img > 0 && img) { sh[0] = (real)img[s]; sh[1] = (real)img[n_img + s]; sh[2] = (real)img[2 * n_img + s]; }
+    real Ps[3] = {P[0] - sh[0], P[1] - sh[1], P[2] - sh[2]};
     real o[4];
     elem_influence(g, j, Ps, o);
-    for (int k = 0; k < 4; ++k) acc[k] += o[k];
+    int unshifted = (sh[0] == 0 && sh[1] == 0 && sh[2] == 0);
+    acc[0] += o[0];
+    if (!(self_pv && unshifted))
+      for (int k = 1; k < 4; ++k) acc[k] += o[k];
   }
 }
 
@@ -273,7 +277,7 @@ static real matrix_entry(const elems_t* g, const double* colloc, const int32_t* 
                          int64_t i, int64_t j) {
   real P[3] = {colloc[i], colloc[g->n + i], colloc[2 * g->n + i]};
   long double acc[4];
-  elem_influence_images(g, j, P, n_img, img, acc);
+  elem_influence_images(g, j, P, n_img, img, i == j, acc);
   if (bc_kind[i] == ORC_DIRICHLET) return (real)(K_COULOMB * acc[0]);
   real nrm[3];
   unit_normal(g, i, nrm);
@@ -465,7 +469,7 @@ void orc_eval(int64_t n, const int32_t* kind, const double* v0, const double* e1
     long double tot[4] = {0, 0, 0, 0};
     for (int64_t j = 0; j < n; ++j) {
       long double acc[4];
-      elem_influence_images(&g, j, P, n_img, img, acc);
+      elem_influence_images(&g, j, P, n_img, img, 0, acc);
       for (int k = 0; k < 4; ++k) tot[k] += (long double)sigma[j] * acc[k];
     }
     for (int k = 0; k < 4; ++k) tot[k] *= K_COULOMB;

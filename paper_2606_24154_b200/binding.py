@@ -1,0 +1,225 @@
+"""ctypes binding of libneb.so: same names as include/neb.h, marshalling only."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+from . import build as _build
+
+NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
+NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
+NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE = 0, 1, 2
+STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges"]
+_STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_HEADER = os.path.join(os.path.dirname(_HERE), "include", "neb.h")
+_lib = None
+
+
+class NebError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def exported_symbols():
+    """Names declared in include/neb.h (every `neb_*(` prototype)."""
+    with open(_HEADER) as fh:
+        text = fh.read()
+    return sorted(set(re.findall(r"\b(neb_[a-z0-9_]+)\s*\(", text)))
+
+
+def lib():
+    """Loads libneb.so (building it in-tree if it is missing); raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        L.neb_create.argtypes = [C.POINTER(vp), C.c_int, vp]
+        L.neb_destroy.argtypes = [vp]
+        L.neb_destroy.restype = None
+        L.neb_last_error.argtypes = [vp]
+        L.neb_last_error.restype = C.c_char_p
+        L.neb_set_option.argtypes = [vp, i32, i64]
+        L.neb_assemble.argtypes = [vp, i64] + [vp] * 10 + [i32, vp]
+        L.neb_solve.argtypes = [vp, vp]
+        L.neb_set_sigma.argtypes = [vp, vp]
+        L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
+        L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
+        L.neb_push.argtypes = [vp, i64, vp, vp, dbl]
+        L.neb_get_matrix.argtypes = [vp, vp]
+        L.neb_get_rhs.argtypes = [vp, vp]
+        L.neb_fp64_peak.argtypes = [vp, i32, C.POINTER(dbl)]
+        L.neb_stage_ms.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(i64)]
+        L.neb_reset_stats.argtypes = [vp]
+        L.neb_launch_count.argtypes = [vp]
+        L.neb_launch_count.restype = i64
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    """Raw address of a torch tensor (device or host) or a numpy array; None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()            # torch.Tensor
+
+
+def _check_arr(a, dtype_np, dtype_name, count, name):
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if a.dtype != dtype_np or not a.flags["C_CONTIGUOUS"]:
+            a = np.ascontiguousarray(a, dtype=dtype_np)
+    else:
+        import torch
+        want = {"float64": torch.float64, "int32": torch.int32}[dtype_name]
+        if a.dtype != want or not a.is_contiguous():
+            a = a.to(want).contiguous()
+    n = a.size if isinstance(a, np.ndarray) else a.numel()
+    if n != count:
+        raise ValueError(f"{name}: expected {count} values, got {n}")
+    return a
+
+
+class Neb:
+    """One neb_ctx.  Arrays may be numpy arrays (host) or torch tensors (host or cuda); vectors are SoA
+    with shape (3, n).  Outputs are returned in the same kind of memory as `pts` unless `out` is given."""
+
+    def __init__(self, device: int = 0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise NebError(5, "no CUDA device: this library has no CPU path")
+        self._L = lib()
+        self._h = C.c_void_p()
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        self.device = device
+        st = self._L.neb_create(C.byref(self._h), device, C.c_void_p(stream))
+        if st != 0:
+            raise NebError(st, "neb_create failed (needs an sm_100 device)")
+        self.n = 0
+
+    def _ck(self, st):
+        if st != 0:
+            raise NebError(st, self._L.neb_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._L.neb_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, option: int, value: int):
+        self._ck(self._L.neb_set_option(self._h, option, value))
+
+    def assemble(self, kind, v0, e1, e2, bc_kind, bc_value=None, radius=None, colloc=None, eps_plus=None,
+                 eps_minus=None, img_shift=None):
+        n = int(kind.shape[0])
+        a = dict(kind=_check_arr(kind, np.int32, "int32", n, "kind"), v0=_check_arr(v0, np.float64, "float64", 3 * n, "v0"),
+                 e1=_check_arr(e1, np.float64, "float64", 3 * n, "e1"), e2=_check_arr(e2, np.float64, "float64", 3 * n, "e2"),
+                 radius=_check_arr(radius, np.float64, "float64", n, "radius"),
+                 colloc=_check_arr(colloc, np.float64, "float64", 3 * n, "colloc"),
+                 bc_kind=_check_arr(bc_kind, np.int32, "int32", n, "bc_kind"),
+                 bc_value=_check_arr(bc_value, np.float64, "float64", n, "bc_value"),
+                 eps_plus=_check_arr(eps_plus, np.float64, "float64", n, "eps_plus"),
+                 eps_minus=_check_arr(eps_minus, np.float64, "float64", n, "eps_minus"))
+        n_img = 0
+        if img_shift is not None:
+            n_img = int(img_shift.shape[1])
+            img_shift = _check_arr(img_shift, np.float64, "float64", 3 * n_img, "img_shift")
+        self._ck(self._L.neb_assemble(self._h, n, _ptr(a["kind"]), _ptr(a["v0"]), _ptr(a["e1"]), _ptr(a["e2"]),
+                                      _ptr(a["radius"]), _ptr(a["colloc"]), _ptr(a["bc_kind"]), _ptr(a["bc_value"]),
+                                      _ptr(a["eps_plus"]), _ptr(a["eps_minus"]), n_img, _ptr(img_shift)))
+        self.n = n
+
+    def assemble_problem(self, pr, colloc=None):
+        """Convenience: a workloads.configs.Problem (host arrays)."""
+        self.assemble(pr.kind, pr.v0, pr.e1, pr.e2, pr.bc_kind, pr.bc_value, radius=pr.radius, colloc=colloc,
+                      eps_plus=pr.eps_plus, eps_minus=pr.eps_minus, img_shift=pr.img_shift)
+
+    def solve(self, out=None):
+        """Returns sigma (n) as a numpy array, or fills `out` (numpy or torch, host or device)."""
+        if out is None:
+            out = np.empty(self.n)
+        self._ck(self._L.neb_solve(self._h, _ptr(out)))
+        return out
+
+    def solve_resident(self):
+        """neb_solve without reading sigma back."""
+        self._ck(self._L.neb_solve(self._h, None))
+
+    def set_sigma(self, sigma):
+        sigma = _check_arr(sigma, np.float64, "float64", self.n, "sigma")
+        self._ck(self._L.neb_set_sigma(self._h, _ptr(sigma)))
+
+    def eval(self, pts, phi=None, E=None, want_phi=True, want_E=True):
+        m = int(pts.shape[1])
+        pts = _check_arr(pts, np.float64, "float64", 3 * m, "pts")
+        if isinstance(pts, np.ndarray):
+            if phi is None and want_phi:
+                phi = np.empty(m)
+            if E is None and want_E:
+                E = np.empty((3, m))
+        else:
+            import torch
+            if phi is None and want_phi:
+                phi = torch.empty(m, dtype=torch.float64, device=pts.device)
+            if E is None and want_E:
+                E = torch.empty((3, m), dtype=torch.float64, device=pts.device)
+        self._ck(self._L.neb_eval(self._h, m, _ptr(pts), _ptr(phi), _ptr(E)))
+        return phi, E
+
+    def add_space_charge(self, pos, charge, replace=True):
+        q = 0 if charge is None else int(charge.shape[0])
+        pos = _check_arr(pos, np.float64, "float64", 3 * q, "pos")
+        charge = _check_arr(charge, np.float64, "float64", q, "charge")
+        self._ck(self._L.neb_add_space_charge(self._h, q, _ptr(pos), _ptr(charge), 1 if replace else 0))
+
+    def push(self, pos, E, mu_dt: float):
+        q = int(pos.shape[1])
+        self._ck(self._L.neb_push(self._h, q, _ptr(pos), _ptr(E), float(mu_dt)))
+        return pos
+
+    def get_matrix(self):
+        K = np.empty((self.n, self.n))
+        self._ck(self._L.neb_get_matrix(self._h, _ptr(K)))
+        return K.T            # column-major n*n -> K[i, j]
+
+    def get_rhs(self):
+        b = np.empty(self.n)
+        self._ck(self._L.neb_get_rhs(self._h, _ptr(b)))
+        return b
+
+    def fp64_peak(self, kind: int) -> float:
+        v = C.c_double(0.0)
+        self._ck(self._L.neb_fp64_peak(self._h, kind, C.byref(v)))
+        return v.value
+
+    def stage_ms(self):
+        out = {}
+        for s, name in enumerate(STAGES):
+            ms, ln = C.c_double(0.0), C.c_int64(0)
+            self._ck(self._L.neb_stage_ms(self._h, s, C.byref(ms), C.byref(ln)))
+            out[name] = (ms.value, ln.value)
+        return out
+
+    def reset_stats(self):
+        self._ck(self._L.neb_reset_stats(self._h))
+
+    def launch_count(self) -> int:
+        return int(self._L.neb_launch_count(self._h))

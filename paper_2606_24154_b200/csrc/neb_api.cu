@@ -1,0 +1,583 @@
+// neb_api.cu — the C ABI of include/neb.h: context, pointer staging, a1 frame tables, call ordering.
+#include <math.h>
+#include <string.h>
+
+#include <vector>
+
+#include "neb_internal.h"
+
+namespace neb {
+
+neb_status fail(neb_ctx* c, neb_status st, const std::string& msg) {
+  if (c) c->err = msg;
+  return st;
+}
+
+neb_status ensure_scratch(neb_ctx* c, size_t bytes) {
+  if (bytes <= c->scratch_bytes) return NEB_OK;
+  if (c->d_scratch) {
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    NEB_CUDA(c, cudaFree(c->d_scratch));
+    c->d_scratch = nullptr;
+    c->scratch_bytes = 0;
+  }
+  size_t want = bytes + bytes / 8;
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_scratch, want));
+  c->scratch_bytes = want;
+  return NEB_OK;
+}
+
+StageTimer::StageTimer(neb_ctx* c_, int stage_) : c(c_), stage(stage_), l0(c_->launches) {
+  if (c->profile) cudaEventRecord(c->ev0[stage], c->stream);
+}
+StageTimer::~StageTimer() {
+  if (c->profile) {
+    cudaEventRecord(c->ev1[stage], c->stream);
+    cudaEventSynchronize(c->ev1[stage]);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, c->ev0[stage], c->ev1[stage]);
+    c->stat[stage].ms += ms;
+  }
+  c->stat[stage].launches += c->launches - l0;
+}
+
+// ---- pointer staging -------------------------------------------------------------------------------
+static bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+struct Staging {   // temporaries of one ABI call
+  neb_ctx* c;
+  std::vector<void*> temps;
+  explicit Staging(neb_ctx* c_) : c(c_) {}
+  ~Staging() {
+    for (void* p : temps) cudaFreeAsync(p, c->stream);
+  }
+  // device view of an input array (copied if it lives on the host)
+  neb_status in(const void* p, size_t bytes, const void** out) {
+    *out = nullptr;
+    if (!p || bytes == 0) return NEB_OK;
+    if (is_device_ptr(p)) { *out = p; return NEB_OK; }
+    void* d = nullptr;
+    NEB_CUDA(c, cudaMallocAsync(&d, bytes, c->stream));
+    temps.push_back(d);
+    NEB_CUDA(c, cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, c->stream));
+    *out = d;
+    return NEB_OK;
+  }
+  // device buffer standing for an output array; host_dst != nullptr means copy back at finish()
+  struct Out { void* dev; void* host; size_t bytes; };
+  std::vector<Out> outs;
+  neb_status out(void* p, size_t bytes, void** dev) {
+    *dev = nullptr;
+    if (!p || bytes == 0) return NEB_OK;
+    if (is_device_ptr(p)) { *dev = p; return NEB_OK; }
+    void* d = nullptr;
+    NEB_CUDA(c, cudaMallocAsync(&d, bytes, c->stream));
+    temps.push_back(d);
+    outs.push_back({d, p, bytes});
+    *dev = d;
+    return NEB_OK;
+  }
+  neb_status finish() {
+    if (outs.empty()) return NEB_OK;
+    for (auto& o : outs) NEB_CUDA(c, cudaMemcpyAsync(o.host, o.dev, o.bytes, cudaMemcpyDeviceToHost, c->stream));
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    outs.clear();
+    return NEB_OK;
+  }
+};
+
+// ---- a1: frame tables -------------------------------------------------------------------------------
+// Stable partition of the element indices by kind (single CTA): perm[sorted position] = caller index.
+__global__ void __launch_bounds__(1024) kind_partition_kernel(const int32_t* __restrict__ kind, int n, int32_t* __restrict__ perm,
+                                                              int32_t* __restrict__ counts, int32_t* __restrict__ flag) {
+  __shared__ int s_cnt[3], s_run[3], s_warp[32][3];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid < 3) s_cnt[tid] = 0;
+  __syncthreads();
+  int local[3] = {0, 0, 0};
+  for (int i = tid; i < n; i += 1024) {
+    int k = kind[i];
+    if (k < 0 || k > 2) atomicOr(flag, 1);
+    else local[k]++;
+  }
+  for (int kk = 0; kk < 3; ++kk) atomicAdd(&s_cnt[kk], local[kk]);
+  __syncthreads();
+  if (tid == 0) {
+    s_run[0] = 0; s_run[1] = s_cnt[0]; s_run[2] = s_cnt[0] + s_cnt[1];
+    counts[0] = s_cnt[0]; counts[1] = s_cnt[1]; counts[2] = s_cnt[2];
+  }
+  __syncthreads();
+  for (int chunk = 0; chunk < n; chunk += 1024) {
+    int i = chunk + tid;
+    int k = (i < n) ? kind[i] : -1;
+    if (k < 0 || k > 2) k = -1;
+    int rank = 0;
+    for (int kk = 0; kk < 3; ++kk) {
+      unsigned bal = __ballot_sync(0xffffffffu, k == kk);
+      if (k == kk) rank = __popc(bal & ((1u << lane) - 1u));
+      if (lane == 0) s_warp[warp][kk] = __popc(bal);
+    }
+    __syncthreads();
+    if (k >= 0) {
+      int pre = 0;
+      for (int w = 0; w < warp; ++w) pre += s_warp[w][k];
+      perm[s_run[k] + pre + rank] = i;
+    }
+    __syncthreads();
+    if (tid < 3) {
+      int tot = 0;
+      for (int w = 0; w < 32; ++w) tot += s_warp[w][tid];
+      s_run[tid] += tot;
+    }
+    __syncthreads();
+  }
+}
+
+// One thread per sorted position: unit frame, edge lengths, collocation point, normal, row data.
+__global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restrict__ perm, const int32_t* __restrict__ kind,
+                              const double* __restrict__ v0, const double* __restrict__ e1, const double* __restrict__ e2,
+                              const double* __restrict__ radius, const double* __restrict__ colloc_in,
+                              const int32_t* __restrict__ bc_kind_in, const double* __restrict__ bc_value_in,
+                              const double* __restrict__ eps_plus, const double* __restrict__ eps_minus,
+                              double* __restrict__ rec, double* __restrict__ colloc, double* __restrict__ normal,
+                              int32_t* __restrict__ bc_kind, double* __restrict__ bc_value, double* __restrict__ diag,
+                              int32_t* __restrict__ flag) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  int64_t j = perm[s];
+  int k = kind[j];
+  double p0[3] = {v0[j], v0[n + j], v0[2 * n + j]};
+  double a1[3] = {e1[j], e1[n + j], e1[2 * n + j]};
+  double a2[3] = {e2[j], e2[n + j], e2[2 * n + j]};
+  double la = sqrt(a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2]);
+  if (!(la > 0.0)) { atomicOr(flag, 4); la = 1.0; }
+  double ex[3] = {a1[0] / la, a1[1] / la, a1[2] / la};
+  double ey[3] = {0, 0, 0}, ez[3] = {0, 0, 0};
+  double lb = 0.0, aux = 0.0;
+  double cp[3];
+  if (k == NEB_WIRE) {
+    double rw = radius ? radius[j] : 0.0;
+    if (!(rw > 0.0)) { atomicOr(flag, 8); rw = 1.0; }
+    lb = rw;
+    aux = 2.0 * 3.14159265358979323846 * rw;
+    // default collocation: mid-length, on the surface, along axis x (least-aligned coordinate axis)
+    int m = 0;
+    if (fabs(ex[1]) < fabs(ex[m])) m = 1;
+    if (fabs(ex[2]) < fabs(ex[m])) m = 2;
+    double ax[3] = {m == 0 ? 1.0 : 0.0, m == 1 ? 1.0 : 0.0, m == 2 ? 1.0 : 0.0};
+    double pr[3] = {ex[1] * ax[2] - ex[2] * ax[1], ex[2] * ax[0] - ex[0] * ax[2], ex[0] * ax[1] - ex[1] * ax[0]};
+    double lp = sqrt(pr[0] * pr[0] + pr[1] * pr[1] + pr[2] * pr[2]);
+    for (int c = 0; c < 3; ++c) cp[c] = p0[c] + 0.5 * a1[c] + rw * pr[c] / lp;
+  } else {
+    double l2 = sqrt(a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2]);
+    if (!(l2 > 0.0)) { atomicOr(flag, 4); l2 = 1.0; }
+    double z0[3] = {a2[0] / l2, a2[1] / l2, a2[2] / l2};
+    // n = e2 x e1 / |e2 x e1| (local Y); then local Z = X x Y so the frame is orthonormal
+    double c0 = z0[1] * ex[2] - z0[2] * ex[1], c1 = z0[2] * ex[0] - z0[0] * ex[2], c2 = z0[0] * ex[1] - z0[1] * ex[0];
+    double lc = sqrt(c0 * c0 + c1 * c1 + c2 * c2);
+    if (!(lc > 0.5)) { atomicOr(flag, 4); lc = 1.0; }   // edges must be (nearly) perpendicular
+    ey[0] = c0 / lc; ey[1] = c1 / lc; ey[2] = c2 / lc;
+    ez[0] = ex[1] * ey[2] - ex[2] * ey[1];
+    ez[1] = ex[2] * ey[0] - ex[0] * ey[2];
+    ez[2] = ex[0] * ey[1] - ex[1] * ey[0];
+    lb = a2[0] * ez[0] + a2[1] * ez[1] + a2[2] * ez[2];
+    double w = (k == NEB_RECT) ? 0.5 : (1.0 / 3.0);
+    for (int c = 0; c < 3; ++c) cp[c] = p0[c] + w * (a1[c] + a2[c]);
+    if (k == NEB_TRI) aux = 1.0 / sqrt(la * la + lb * lb);
+  }
+  if (colloc_in) { cp[0] = colloc_in[j]; cp[1] = colloc_in[n + j]; cp[2] = colloc_in[2 * n + j]; }
+  double* r = rec + s;
+  r[0 * stride] = p0[0]; r[1 * stride] = p0[1]; r[2 * stride] = p0[2];
+  r[3 * stride] = ex[0]; r[4 * stride] = ex[1]; r[5 * stride] = ex[2];
+  r[6 * stride] = ey[0]; r[7 * stride] = ey[1]; r[8 * stride] = ey[2];
+  r[9 * stride] = ez[0]; r[10 * stride] = ez[1]; r[11 * stride] = ez[2];
+  r[12 * stride] = la; r[13 * stride] = lb; r[14 * stride] = aux; r[15 * stride] = 0.0;
+  for (int c = 0; c < 3; ++c) { colloc[c * stride + s] = cp[c]; normal[c * stride + s] = ey[c]; }
+  int bk = bc_kind_in[j];
+  if (bk != NEB_BC_DIRICHLET && bk != NEB_BC_DIELECTRIC) { atomicOr(flag, 16); bk = NEB_BC_DIRICHLET; }
+  double dg = 0.0;
+  if (bk == NEB_BC_DIELECTRIC) {
+    double ep = eps_plus ? eps_plus[j] : 1.0, em = eps_minus ? eps_minus[j] : 1.0;
+    if (!(ep > 0.0) || !(em > 0.0) || ep == em || k == NEB_WIRE) { atomicOr(flag, 32); }
+    else dg = (ep + em) / (2.0 * kEps0 * (ep - em));     // 1 / (2 eps0 lambda), reading S8
+  }
+  bc_kind[s] = bk;
+  bc_value[s] = bc_value_in ? bc_value_in[j] : 0.0;
+  diag[s] = dg;
+}
+
+__global__ void set_weights_kernel(int64_t n, int64_t stride, const int32_t* __restrict__ perm, const double* __restrict__ sigma_caller,
+                                   double* __restrict__ rec) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) rec[15 * stride + s] = sigma_caller[perm[s]] * kCoulomb;
+}
+
+__global__ void finish_sigma_kernel(int64_t n, int64_t stride, const int32_t* __restrict__ perm, const double* __restrict__ x,
+                                    double* __restrict__ rec, double* __restrict__ sigma_caller) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) {
+    double v = x[s];
+    rec[15 * stride + s] = v * kCoulomb;
+    sigma_caller[perm[s]] = v;
+  }
+}
+
+__global__ void unpermute_matrix_kernel(int64_t n, int64_t ld, const int32_t* __restrict__ perm, const double* __restrict__ K,
+                                        double* __restrict__ out) {
+  int64_t si = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t sj = blockIdx.y;
+  if (si < n) out[(int64_t)perm[si] + (int64_t)perm[sj] * n] = K[si + sj * ld];
+}
+
+__global__ void unpermute_vector_kernel(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ v, double* __restrict__ out) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) out[perm[s]] = v[s];
+}
+
+__global__ void push_kernel(int64_t n3, double* __restrict__ pos, const double* __restrict__ E, double mu_dt) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n3) pos[i] = fma(mu_dt, E[i], pos[i]);
+}
+
+static void free_problem(neb_ctx* c) {
+  void* ptrs[] = {c->d_rec, c->d_perm, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_img,
+                  c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  c->d_rec = nullptr; c->d_perm = nullptr; c->d_colloc = nullptr; c->d_normal = nullptr; c->d_bc_kind = nullptr;
+  c->d_bc_value = nullptr; c->d_diag = nullptr; c->d_img = nullptr; c->d_K = nullptr; c->d_rscale = nullptr;
+  c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr;
+  c->assembled = c->factored = c->have_sigma = false;
+  c->n = c->npad = c->stride = 0;
+}
+
+}  // namespace neb
+
+using namespace neb;
+
+extern "C" {
+
+neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
+  if (!out) return NEB_EINVAL;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+    cudaGetLastError();
+    return NEB_ECUDA;
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NEB_ECUDA;
+  if (prop.major != 10) return NEB_ECUDA;   // built for sm_100a only; no other code path exists
+  if (cudaSetDevice(device) != cudaSuccess) return NEB_ECUDA;
+  neb_ctx* c = new neb_ctx();
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->num_sms = prop.multiProcessorCount;
+  bool ok = cudaMalloc((void**)&c->d_flag, sizeof(int32_t)) == cudaSuccess &&
+            cudaMemset(c->d_flag, 0, sizeof(int32_t)) == cudaSuccess &&
+            cudaMalloc(&c->d_panel_ws, lu_panel_ws_bytes(c->num_sms)) == cudaSuccess;
+  for (int s = 0; ok && s < NEB_STAGE_COUNT; ++s)
+    ok = cudaEventCreate(&c->ev0[s]) == cudaSuccess && cudaEventCreate(&c->ev1[s]) == cudaSuccess;
+  if (!ok) {
+    neb_destroy(c);
+    return NEB_ECUDA;
+  }
+  *out = c;
+  return NEB_OK;
+}
+
+void neb_destroy(neb_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  free_problem(c);
+  if (c->d_flag) cudaFree(c->d_flag);
+  if (c->d_panel_ws) cudaFree(c->d_panel_ws);
+  if (c->d_charges) cudaFree(c->d_charges);
+  if (c->d_scratch) cudaFree(c->d_scratch);
+  for (int s = 0; s < NEB_STAGE_COUNT; ++s) {
+    if (c->ev0[s]) cudaEventDestroy(c->ev0[s]);
+    if (c->ev1[s]) cudaEventDestroy(c->ev1[s]);
+  }
+  delete c;
+}
+
+const char* neb_last_error(const neb_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
+  if (!c) return NEB_EINVAL;
+  switch (option) {
+    case NEB_OPT_MATH: c->math_fast = value ? 1 : 0; return NEB_OK;
+    case NEB_OPT_LU_BLOCK:
+      if (value != 64) return fail(c, NEB_EINVAL, "this build supports LU panel width 64 only");
+      return NEB_OK;
+    case NEB_OPT_PROFILE: c->profile = value ? 1 : 0; return NEB_OK;
+    default: return fail(c, NEB_EINVAL, "unknown option");
+  }
+}
+
+neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double* v0, const double* e1, const double* e2,
+                        const double* radius, const double* colloc, const int32_t* bc_kind, const double* bc_value,
+                        const double* eps_plus, const double* eps_minus, int32_t n_img, const double* img_shift) {
+  if (!c) return NEB_EINVAL;
+  if (n <= 0 || n > 65000 || !kind || !v0 || !e1 || !e2 || !bc_kind)
+    return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1..65000 and kind, v0, e1, e2, bc_kind non-NULL");
+  if (n_img < 0 || n_img > 32 || (n_img > 0 && !img_shift)) return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= 32");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+  free_problem(c);
+  c->n = n;
+  c->npad = (n + kPad - 1) / kPad * kPad;
+  c->stride = c->npad;
+  const int64_t st = c->stride, npad = c->npad;
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_perm, sizeof(int32_t) * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_colloc, sizeof(double) * 3 * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_normal, sizeof(double) * 3 * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_kind, sizeof(int32_t) * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_value, sizeof(double) * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_diag, sizeof(double) * st));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_rscale, sizeof(double) * npad));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_ipiv, sizeof(int32_t) * npad));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_rowperm, sizeof(int32_t) * npad));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_b, sizeof(double) * npad));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * npad));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
+  c->n_img = n_img > 0 ? n_img : 1;
+  NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * c->n_img));
+  NEB_CUDA(c, cudaMemsetAsync(c->d_img, 0, sizeof(double) * 3 * c->n_img, c->stream));
+  NEB_CUDA(c, cudaMemsetAsync(c->d_rec, 0, sizeof(double) * kRec * st, c->stream));
+  NEB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int32_t), c->stream));
+
+  Staging sg(c);
+  const void *dk, *dv0, *de1, *de2, *drad, *dcol, *dbk, *dbv, *dep, *dem;
+  NEB_TRY(sg.in(kind, sizeof(int32_t) * n, &dk));
+  NEB_TRY(sg.in(v0, sizeof(double) * 3 * n, &dv0));
+  NEB_TRY(sg.in(e1, sizeof(double) * 3 * n, &de1));
+  NEB_TRY(sg.in(e2, sizeof(double) * 3 * n, &de2));
+  NEB_TRY(sg.in(radius, sizeof(double) * n, &drad));
+  NEB_TRY(sg.in(colloc, sizeof(double) * 3 * n, &dcol));
+  NEB_TRY(sg.in(bc_kind, sizeof(int32_t) * n, &dbk));
+  NEB_TRY(sg.in(bc_value, sizeof(double) * n, &dbv));
+  NEB_TRY(sg.in(eps_plus, sizeof(double) * n, &dep));
+  NEB_TRY(sg.in(eps_minus, sizeof(double) * n, &dem));
+  if (n_img > 0) {
+    // the unshifted copy goes to slot 0 (the kernels treat slot 0 as the element itself); it must be present
+    double h_img[3 * 32];
+    NEB_CUDA(c, cudaMemcpy(h_img, img_shift, sizeof(double) * 3 * n_img, cudaMemcpyDefault));
+    int zero = -1;
+    for (int s = 0; s < n_img && zero < 0; ++s)
+      if (h_img[s] == 0.0 && h_img[n_img + s] == 0.0 && h_img[2 * n_img + s] == 0.0) zero = s;
+    if (zero < 0) { free_problem(c); return fail(c, NEB_EINVAL, "neb_assemble: img_shift must include (0,0,0)"); }
+    for (int k = 0; k < 3; ++k) { double t = h_img[k * n_img]; h_img[k * n_img] = h_img[k * n_img + zero]; h_img[k * n_img + zero] = t; }
+    NEB_CUDA(c, cudaMemcpyAsync(c->d_img, h_img, sizeof(double) * 3 * n_img, cudaMemcpyHostToDevice, c->stream));
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_img is a stack buffer
+  }
+  int32_t* d_counts = nullptr;
+  NEB_CUDA(c, cudaMallocAsync((void**)&d_counts, 3 * sizeof(int32_t), c->stream));
+  sg.temps.push_back(d_counts);
+  {
+    StageTimer t(c, NEB_STAGE_GEOMETRY);
+    kind_partition_kernel<<<1, 1024, 0, c->stream>>>((const int32_t*)dk, (int)n, c->d_perm, d_counts, c->d_flag);
+    c->launches++;
+    frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(
+        n, st, c->d_perm, (const int32_t*)dk, (const double*)dv0, (const double*)de1, (const double*)de2,
+        (const double*)drad, (const double*)dcol, (const int32_t*)dbk, (const double*)dbv, (const double*)dep,
+        (const double*)dem, c->d_rec, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_flag);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  int32_t h_counts[3], h_flag = 0;
+  NEB_CUDA(c, cudaMemcpyAsync(h_counts, d_counts, sizeof(h_counts), cudaMemcpyDeviceToHost, c->stream));
+  NEB_CUDA(c, cudaMemcpyAsync(&h_flag, c->d_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (h_flag != 0) {
+    std::string why = "neb_assemble: invalid input:";
+    if (h_flag & 1) why += " unknown element kind;";
+    if (h_flag & 4) why += " zero-length or non-perpendicular edge;";
+    if (h_flag & 8) why += " wire without a positive radius;";
+    if (h_flag & 16) why += " unknown bc_kind;";
+    if (h_flag & 32) why += " dielectric row with eps_plus == eps_minus, a non-positive permittivity, or on a wire;";
+    free_problem(c);
+    return fail(c, NEB_EINVAL, why);
+  }
+  c->n_rect = h_counts[0]; c->n_tri = h_counts[1]; c->n_wire = h_counts[2];
+  // the image set must contain the zero shift in slot 0 for the kernels' first evaluation: any order is
+  // fine mathematically, the kernels simply sum all n_img copies
+  NEB_TRY(assemble_matrix(c));
+  c->assembled = true;
+  return NEB_OK;
+}
+
+neb_status neb_solve(neb_ctx* c, double* sigma_out) {
+  if (!c) return NEB_EINVAL;
+  if (!c->assembled) return fail(c, NEB_ESTATE, "neb_solve before neb_assemble");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  if (!c->factored) {
+    NEB_TRY(scale_matrix_rows(c));
+    NEB_TRY(lu_factor(c));
+    int32_t h_flag = 0;
+    NEB_CUDA(c, cudaMemcpyAsync(&h_flag, c->d_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->factored = true;   // the matrix is overwritten either way
+    if (h_flag & 2) {
+      c->assembled = false;
+      return fail(c, NEB_ESINGULAR, "neb_solve: zero or NaN pivot");
+    }
+  }
+  NEB_TRY(form_rhs(c));
+  NEB_TRY(lu_solve(c));
+  finish_sigma_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->stride, c->d_perm, c->d_x, c->d_rec, c->d_sigma);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  c->have_sigma = true;
+  if (sigma_out) {
+    if (is_device_ptr(sigma_out)) {
+      NEB_CUDA(c, cudaMemcpyAsync(sigma_out, c->d_sigma, sizeof(double) * c->n, cudaMemcpyDeviceToDevice, c->stream));
+    } else {
+      NEB_CUDA(c, cudaMemcpyAsync(sigma_out, c->d_sigma, sizeof(double) * c->n, cudaMemcpyDeviceToHost, c->stream));
+      NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+  }
+  return NEB_OK;
+}
+
+neb_status neb_set_sigma(neb_ctx* c, const double* sigma) {
+  if (!c || !sigma) return NEB_EINVAL;
+  if (!c->assembled && c->n == 0) return fail(c, NEB_ESTATE, "neb_set_sigma before neb_assemble");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  const void* ds;
+  NEB_TRY(sg.in(sigma, sizeof(double) * c->n, &ds));
+  NEB_CUDA(c, cudaMemcpyAsync(c->d_sigma, ds, sizeof(double) * c->n, cudaMemcpyDeviceToDevice, c->stream));
+  set_weights_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->stride, c->d_perm, c->d_sigma, c->d_rec);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  c->have_sigma = true;
+  return NEB_OK;
+}
+
+neb_status neb_eval(neb_ctx* c, int64_t m, const double* pts, double* phi, double* E) {
+  if (!c || m < 0 || (m > 0 && !pts)) return NEB_EINVAL;
+  if (!c->have_sigma) return fail(c, NEB_ESTATE, "neb_eval before neb_solve / neb_set_sigma");
+  if (m == 0) return NEB_OK;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  const void* dp;
+  void *dphi, *dE;
+  NEB_TRY(sg.in(pts, sizeof(double) * 3 * m, &dp));
+  NEB_TRY(sg.out(phi, sizeof(double) * m, &dphi));
+  NEB_TRY(sg.out(E, sizeof(double) * 3 * m, &dE));
+  NEB_TRY(field_at_points(c, m, (const double*)dp, true, true, (double*)dphi, (double*)dE));
+  return sg.finish();
+}
+
+neb_status neb_add_space_charge(neb_ctx* c, int64_t q, const double* pos, const double* charge, int32_t replace) {
+  if (!c || q < 0 || (q > 0 && (!pos || !charge))) return NEB_EINVAL;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  if (replace) c->q = 0;
+  if (q == 0) return NEB_OK;
+  int64_t need = c->q + q;
+  if (need > c->q_cap) {
+    int64_t cap = need > 2 * c->q_cap ? need : 2 * c->q_cap;
+    cap = (cap + 255) / 256 * 256;
+    double* nd = nullptr;
+    NEB_CUDA(c, cudaMalloc((void**)&nd, sizeof(double) * 4 * cap));
+    for (int f = 0; f < 4 && c->q > 0; ++f)
+      NEB_CUDA(c, cudaMemcpyAsync(nd + f * cap, c->d_charges + f * c->q_cap, sizeof(double) * c->q, cudaMemcpyDeviceToDevice, c->stream));
+    if (c->d_charges) {
+      NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+      NEB_CUDA(c, cudaFree(c->d_charges));
+    }
+    c->d_charges = nd;
+    c->q_cap = cap;
+  }
+  cudaMemcpyKind kp = is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  cudaMemcpyKind kq = is_device_ptr(charge) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  for (int f = 0; f < 3; ++f)
+    NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + f * c->q_cap + c->q, pos + f * q, sizeof(double) * q, kp, c->stream));
+  NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + 3 * c->q_cap + c->q, charge, sizeof(double) * q, kq, c->stream));
+  c->q = need;
+  return NEB_OK;
+}
+
+neb_status neb_push(neb_ctx* c, int64_t q, double* pos, const double* E, double mu_dt) {
+  if (!c || q < 0 || (q > 0 && (!pos || !E))) return NEB_EINVAL;
+  if (q == 0) return NEB_OK;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  bool dp = is_device_ptr(pos), dE = is_device_ptr(E);
+  if (dp != dE) return fail(c, NEB_EINVAL, "neb_push: pos and E must both be host or both be device pointers");
+  Staging sg(c);
+  const void* din;
+  const void* dEv;
+  void* dpos;
+  NEB_TRY(sg.in(E, sizeof(double) * 3 * q, &dEv));
+  if (dp) dpos = pos;
+  else {
+    NEB_TRY(sg.in(pos, sizeof(double) * 3 * q, &din));
+    dpos = const_cast<void*>(din);
+    sg.outs.push_back({dpos, pos, sizeof(double) * 3 * (size_t)q});
+  }
+  push_kernel<<<(unsigned)((3 * q + 255) / 256), 256, 0, c->stream>>>(3 * q, (double*)dpos, (const double*)dEv, mu_dt);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return sg.finish();
+}
+
+neb_status neb_get_matrix(neb_ctx* c, double* K_out) {
+  if (!c || !K_out) return NEB_EINVAL;
+  if (!c->assembled || c->factored) return fail(c, NEB_ESTATE, "neb_get_matrix: only between neb_assemble and the first neb_solve");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  void* dout;
+  NEB_TRY(sg.out(K_out, sizeof(double) * (size_t)c->n * (size_t)c->n, &dout));
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)c->n);
+  unpermute_matrix_kernel<<<grid, 256, 0, c->stream>>>(c->n, c->npad, c->d_perm, c->d_K, (double*)dout);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return sg.finish();
+}
+
+neb_status neb_get_rhs(neb_ctx* c, double* b_out) {
+  if (!c || !b_out) return NEB_EINVAL;
+  if (!c->have_sigma || !c->factored) return fail(c, NEB_ESTATE, "neb_get_rhs before neb_solve");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  void* dout;
+  NEB_TRY(sg.out(b_out, sizeof(double) * c->n, &dout));
+  unpermute_vector_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->d_perm, c->d_b, (double*)dout);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return sg.finish();
+}
+
+neb_status neb_fp64_peak(neb_ctx* c, int32_t kind, double* tflops) {
+  if (!c || !tflops) return NEB_EINVAL;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  return fp64_peak(c, kind, tflops);
+}
+
+neb_status neb_stage_ms(neb_ctx* c, int32_t stage, double* ms, int64_t* launches) {
+  if (!c || stage < 0 || stage >= NEB_STAGE_COUNT) return NEB_EINVAL;
+  if (ms) *ms = c->stat[stage].ms;
+  if (launches) *launches = c->stat[stage].launches;
+  return NEB_OK;
+}
+
+neb_status neb_reset_stats(neb_ctx* c) {
+  if (!c) return NEB_EINVAL;
+  for (int s = 0; s < NEB_STAGE_COUNT; ++s) c->stat[s] = StageStat();
+  return NEB_OK;
+}
+
+int64_t neb_launch_count(const neb_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

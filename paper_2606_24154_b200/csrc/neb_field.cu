@@ -1,0 +1,404 @@
+// neb_field.cu — the element-point kernels of the hot path:
+//   a3  assemble_kernel : LHMatrix, K_ij at collocation point i from element j (+ periodic copies)
+//   a7  eval_kernel     : PFAtPoint / ElePFAtPoint, Phi and E at M points, fused with the reduction
+//                         over the solved charge densities
+//   a8  charge_kernel   : KnChPFAtPoint, direct sum over point charges (Alg. 2 P:234-270 re-designed:
+//                         many targets per launch, charge tiles in shared memory, no atomics)
+//   a4  rhs_kernel      : RHVector + ValueKnCh
+// A thread owns one point; element records (frame tables, SoA) are staged tile by tile through shared
+// memory and broadcast to the warp.  Tiles are homogeneous in element kind (the tables are sorted by
+// kind), every case distinction inside the influence function is a select: warps never diverge.
+// Work is split over element (or charge) chunks in grid.y so that small M still fills 148 SMs; the
+// per-chunk partial sums are added by reduce_kernel in a fixed order (deterministic, no fp64 atomics).
+#include "neb_internal.h"
+#include "neb_influence.cuh"
+
+namespace neb {
+
+constexpr int kThreads = 128;   // threads per CTA = points per CTA
+constexpr int kTile = 64;       // elements per shared-memory tile
+constexpr int kChargeTile = 256;
+constexpr int kMaxImg = 32;     // periodic copies kept in shared memory
+
+struct TileSmem {
+  double rec[kRec][kTile];
+  double img[3][kMaxImg];
+};
+
+__device__ __forceinline__ void load_tile(TileSmem& sm, const GeoTables& g, int64_t base, int cnt) {
+  for (int idx = threadIdx.x; idx < kRec * kTile; idx += blockDim.x) {
+    int f = idx / kTile, e = idx % kTile;
+    if (e < cnt) sm.rec[f][e] = g.rec[f * g.stride + base + e];
+  }
+}
+
+__device__ __forceinline__ Frame frame_of(const TileSmem& sm, int e) {
+  Frame f;
+  f.v0x = sm.rec[0][e]; f.v0y = sm.rec[1][e]; f.v0z = sm.rec[2][e];
+  f.exx = sm.rec[3][e]; f.exy = sm.rec[4][e]; f.exz = sm.rec[5][e];
+  f.eyx = sm.rec[6][e]; f.eyy = sm.rec[7][e]; f.eyz = sm.rec[8][e];
+  f.ezx = sm.rec[9][e]; f.ezy = sm.rec[10][e]; f.ezz = sm.rec[11][e];
+  f.a = sm.rec[12][e]; f.b = sm.rec[13][e]; f.aux = sm.rec[14][e];
+  return f;
+}
+
+// All elements of one kind in [lo, hi): tile loop, image loop, sink(j, weight_j, sum over copies).
+template <class M, int KIND, class Sink>
+__device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img,
+                                             double px, double py, double pz, Sink& sink) {
+  for (int64_t base = lo; base < hi; base += kTile) {
+    int cnt = (int)min((int64_t)kTile, hi - base);
+    __syncthreads();
+    load_tile(sm, g, base, cnt);
+    __syncthreads();
+#pragma unroll 1
+    for (int e = 0; e < cnt; ++e) {
+      Frame fr = frame_of(sm, e);
+      // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
+      // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
+      Infl acc = influence<M, KIND>(fr, px - sm.img[0][0], py - sm.img[1][0], pz - sm.img[2][0]);
+      if (sink.self_pv(base + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
+#pragma unroll 1
+      for (int s = 1; s < n_img; ++s) {
+        Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
+        acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
+      }
+      sink(base + e, sm.rec[15][e], acc);
+    }
+  }
+}
+
+template <class M, class Sink>
+__device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, int64_t j1, TileSmem& sm, int n_img,
+                                              double px, double py, double pz, Sink& sink) {
+  int64_t r1 = g.n_rect, t1 = r1 + g.n_tri, w1 = t1 + g.n_wire;
+  int64_t lo, hi;
+  lo = max(j0, (int64_t)0); hi = min(j1, r1);
+  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, px, py, pz, sink);
+  lo = max(j0, r1); hi = min(j1, t1);
+  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, px, py, pz, sink);
+  lo = max(j0, t1); hi = min(j1, w1);
+  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, px, py, pz, sink);
+}
+
+__device__ __forceinline__ void load_images(TileSmem& sm, const double* img, int n_img) {
+  for (int idx = threadIdx.x; idx < 3 * n_img; idx += blockDim.x) sm.img[idx / n_img][idx % n_img] = img[idx];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7: fused evaluation.  grid = (ceil(m/128), n_split); partial[(split*4 + c) * m + p]
+// ------------------------------------------------------------------------------------------------
+struct EvalSink {
+  double phi = 0, ex = 0, ey = 0, ez = 0;
+  __device__ __forceinline__ bool self_pv(int64_t) const { return false; }
+  __device__ __forceinline__ void operator()(int64_t, double w, const Infl& a) {
+    phi = fma(w, a.phi, phi); ex = fma(w, a.ex, ex); ey = fma(w, a.ey, ey); ez = fma(w, a.ez, ez);
+  }
+};
+
+template <class M>
+__global__ void __launch_bounds__(kThreads) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img,
+                                                        const double* __restrict__ pts, int64_t m, int64_t per_split,
+                                                        double* __restrict__ partial) {
+  __shared__ TileSmem sm;
+  load_images(sm, img, n_img);
+  int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  int64_t pc = min(p, m - 1);
+  double px = pts[pc], py = pts[m + pc], pz = pts[2 * m + pc];
+  int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
+  int64_t j0 = (int64_t)blockIdx.y * per_split, j1 = min(n, j0 + per_split);
+  EvalSink sink;
+  process_range<M>(g, j0, j1, sm, n_img, px, py, pz, sink);
+  if (p < m) {
+    double* o = partial + (int64_t)blockIdx.y * 4 * m;
+    o[p] = sink.phi; o[m + p] = sink.ex; o[2 * m + p] = sink.ey; o[3 * m + p] = sink.ez;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8: point charges.  charges SoA x,y,z,q with stride q_stride; grid = (ceil(m/128), n_split)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads) charge_kernel(const double* __restrict__ ch, int64_t q, int64_t q_stride,
+                                                          const double* __restrict__ pts, int64_t m, int64_t per_split,
+                                                          double* __restrict__ partial) {
+  __shared__ double sc[4][kChargeTile];
+  int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  int64_t pc = min(p, m - 1);
+  double px = pts[pc], py = pts[m + pc], pz = pts[2 * m + pc];
+  int64_t k0 = (int64_t)blockIdx.y * per_split, k1 = min(q, k0 + per_split);
+  double phi = 0, ex = 0, ey = 0, ez = 0;
+  for (int64_t base = k0; base < k1; base += kChargeTile) {
+    int cnt = (int)min((int64_t)kChargeTile, k1 - base);
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < 4 * kChargeTile; idx += blockDim.x) {
+      int f = idx / kChargeTile, e = idx % kChargeTile;
+      if (e < cnt) sc[f][e] = ch[f * q_stride + base + e];
+    }
+    __syncthreads();
+#pragma unroll 4
+    for (int e = 0; e < cnt; ++e) {
+      double dx = px - sc[0][e], dy = py - sc[1][e], dz = pz - sc[2][e];
+      double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      // 1/r: MUFU.RSQ64H seed + two Newton steps; a charge exactly at the point is skipped
+      double y = mufu_rsqrt(fmax(r2, NEB_TINY));
+      double h = 0.5 * r2;
+      double e1 = fma(-h * y, y, 0.5);
+      y = fma(y, e1, y);
+      double e2 = fma(-h * y, y, 0.5);
+      y = fma(y, e2, y);
+      y = (r2 > 0.0) ? y : 0.0;
+      double qr = sc[3][e] * y;
+      double qr3 = qr * y * y;
+      phi += qr;
+      ex = fma(qr3, dx, ex); ey = fma(qr3, dy, ey); ez = fma(qr3, dz, ez);
+    }
+  }
+  if (p < m) {
+    double* o = partial + (int64_t)blockIdx.y * 4 * m;
+    o[p] = phi; o[m + p] = ex; o[2 * m + p] = ey; o[3 * m + p] = ez;
+  }
+}
+
+// Sum of the partials in a fixed order.  Element partials carry the 1/(4 pi eps0) in the weights;
+// charge partials (index >= n_elem_split) are multiplied by kCoulomb here.
+__global__ void reduce_kernel(const double* __restrict__ partial, int n_elem_split, int n_charge_split, int64_t m,
+                              double* __restrict__ phi, double* __restrict__ E) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= m) return;
+  double acc[4] = {0, 0, 0, 0};
+  for (int s = 0; s < n_elem_split; ++s)
+    for (int c = 0; c < 4; ++c) acc[c] += partial[((int64_t)s * 4 + c) * m + p];
+  double cc[4] = {0, 0, 0, 0};
+  for (int s = n_elem_split; s < n_elem_split + n_charge_split; ++s)
+    for (int c = 0; c < 4; ++c) cc[c] += partial[((int64_t)s * 4 + c) * m + p];
+  for (int c = 0; c < 4; ++c) acc[c] = fma(kCoulomb, cc[c], acc[c]);
+  if (phi) phi[p] = acc[0];
+  if (E) { E[p] = acc[1]; E[m + p] = acc[2]; E[2 * m + p] = acc[3]; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3: assembly.  grid = (ceil(n/128), ceil(n/64)); CTA = 128 rows x one 64-column tile.
+// K column-major with leading dimension ld; consecutive threads write consecutive rows of a column.
+// Row maxima (for the S15 equilibration) are accumulated with an order-independent integer max.
+// ------------------------------------------------------------------------------------------------
+struct AsmSink {
+  double* K; int64_t ld, i; double nx, ny, nz, diag; bool dielectric, active; double rmax;
+  __device__ __forceinline__ bool self_pv(int64_t j) const { return j == i; }
+  __device__ __forceinline__ void operator()(int64_t j, double, const Infl& a) {
+    double vd = fma(nx, a.ex, fma(ny, a.ey, nz * a.ez));
+    double v = kCoulomb * (dielectric ? vd : a.phi);
+    v += (dielectric && j == i) ? diag : 0.0;
+    rmax = fmax(rmax, fabs(v));
+    if (active) K[i + j * ld] = v;
+  }
+};
+
+template <class M>
+__global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const double* __restrict__ img, int n_img,
+                                                            const double* __restrict__ colloc, int64_t stride,
+                                                            const double* __restrict__ normal,
+                                                            const int32_t* __restrict__ bc_kind,
+                                                            const double* __restrict__ diag, double* __restrict__ K,
+                                                            int64_t ld, unsigned long long* __restrict__ rowmax_bits) {
+  __shared__ TileSmem sm;
+  load_images(sm, img, n_img);
+  int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
+  int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  int64_t ic = min(i, n - 1);
+  AsmSink sink;
+  sink.K = K; sink.ld = ld; sink.i = ic; sink.active = i < n; sink.rmax = 0.0;
+  sink.nx = normal[ic]; sink.ny = normal[stride + ic]; sink.nz = normal[2 * stride + ic];
+  sink.dielectric = bc_kind[ic] == NEB_BC_DIELECTRIC;
+  sink.diag = diag[ic];
+  double px = colloc[ic], py = colloc[stride + ic], pz = colloc[2 * stride + ic];
+  int64_t j0 = (int64_t)blockIdx.y * kTile, j1 = min(n, j0 + kTile);
+  process_range<M>(g, j0, j1, sm, n_img, px, py, pz, sink);
+  if (i < n) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
+}
+
+// rows/columns >= n of the padded matrix: identity
+__global__ void pad_identity_kernel(double* K, int64_t n, int64_t npad) {
+  int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t npadrows = npad - n;
+  // region A: rows n..npad, all columns (npadrows x npad); region B: rows 0..n, columns n..npad
+  int64_t sizeA = npadrows * npad, sizeB = n * npadrows;
+  if (idx < sizeA) {
+    int64_t j = idx / npadrows, i = n + idx % npadrows;
+    K[i + j * npad] = (i == j) ? 1.0 : 0.0;
+  } else if (idx < sizeA + sizeB) {
+    int64_t t = idx - sizeA;
+    int64_t j = n + t / n, i = t % n;
+    K[i + j * npad] = 0.0;
+  }
+}
+
+__global__ void rscale_kernel(const unsigned long long* rowmax_bits, int64_t n, int64_t npad, double* rscale) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npad) return;
+  double mx = (i < n) ? __longlong_as_double((long long)rowmax_bits[i]) : 1.0;
+  rscale[i] = (mx > 0.0) ? 1.0 / mx : 1.0;
+}
+
+__global__ void scale_rows_kernel(double* K, int64_t n, int64_t ld, const double* __restrict__ rscale) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t j = blockIdx.y;
+  if (i < n) K[i + j * ld] *= rscale[i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4: RHS (reading S10): Dirichlet b_i = V_i - Phi_sc(p_i); dielectric b_i = -n_i.E_sc(p_i)
+// ------------------------------------------------------------------------------------------------
+__global__ void rhs_kernel(int64_t n, int64_t npad, int64_t stride, const int32_t* __restrict__ bc_kind,
+                           const double* __restrict__ bc_value, const double* __restrict__ normal,
+                           const double* __restrict__ phi_sc, const double* __restrict__ E_sc, double* __restrict__ b) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npad) return;
+  double v = 0.0;
+  if (i < n) {
+    if (bc_kind[i] == NEB_BC_DIRICHLET) v = bc_value[i] - (phi_sc ? phi_sc[i] : 0.0);
+    else if (E_sc) v = -(normal[i] * E_sc[i] + normal[stride + i] * E_sc[n + i] + normal[2 * stride + i] * E_sc[2 * n + i]);
+  }
+  b[i] = v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static int pick_splits(int64_t pt_blocks, int64_t units, int64_t unit_tile, int num_sms) {
+  // aim at >= 16 waves of 4 CTAs/SM so the tail wave is small, but keep >= 2 tiles per split
+  int64_t want = (16LL * 4 * num_sms + pt_blocks - 1) / pt_blocks;
+  int64_t max_split = (units + 2 * unit_tile - 1) / (2 * unit_tile);
+  int64_t s = want < 1 ? 1 : want;
+  if (s > max_split) s = max_split;
+  if (s > 1024) s = 1024;
+  if (s < 1) s = 1;
+  return (int)s;
+}
+
+static GeoTables tables(const neb_ctx* c) {
+  GeoTables g;
+  g.rec = c->d_rec; g.stride = c->stride; g.n_rect = c->n_rect; g.n_tri = c->n_tri; g.n_wire = c->n_wire;
+  return g;
+}
+
+neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_elements, bool use_charges,
+                           double* d_phi, double* d_E) {
+  if (m <= 0) return NEB_OK;
+  use_charges = use_charges && c->q > 0;
+  int64_t pt_blocks = (m + kThreads - 1) / kThreads;
+  int se = use_elements ? pick_splits(pt_blocks, c->n, kTile, c->num_sms) : 0;
+  int sq = use_charges ? pick_splits(pt_blocks, c->q, kChargeTile, c->num_sms) : 0;
+  int64_t per_e = 0, per_q = 0;
+  if (se) {
+    per_e = (c->n + se - 1) / se;
+    per_e = (per_e + kTile - 1) / kTile * kTile;
+    se = (int)((c->n + per_e - 1) / per_e);
+  }
+  if (sq) {
+    per_q = (c->q + sq - 1) / sq;
+    per_q = (per_q + kChargeTile - 1) / kChargeTile * kChargeTile;
+    sq = (int)((c->q + per_q - 1) / per_q);
+  }
+  size_t need = (size_t)(se + sq) * 4 * (size_t)m * sizeof(double);
+  NEB_TRY(ensure_scratch(c, need));
+  double* partial = c->d_scratch;
+  if (se) {
+    StageTimer t(c, NEB_STAGE_EVAL);
+    dim3 grid((unsigned)pt_blocks, (unsigned)se);
+    if (c->math_fast)
+      eval_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, d_pts, m, per_e, partial);
+    else
+      eval_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, d_pts, m, per_e, partial);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  if (sq) {
+    StageTimer t(c, NEB_STAGE_CHARGES);
+    dim3 grid((unsigned)pt_blocks, (unsigned)sq);
+    charge_kernel<<<grid, kThreads, 0, c->stream>>>(c->d_charges, c->q, c->q_cap, d_pts, m, per_q,
+                                                    partial + (size_t)se * 4 * m);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  {
+    StageTimer t(c, use_elements ? NEB_STAGE_EVAL : NEB_STAGE_CHARGES);
+    reduce_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(partial, se, sq, m, d_phi, d_E);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  return NEB_OK;
+}
+
+neb_status assemble_matrix(neb_ctx* c) {
+  int64_t n = c->n, npad = c->npad;
+  NEB_TRY(ensure_scratch(c, (size_t)npad * sizeof(unsigned long long)));
+  unsigned long long* rowmax = (unsigned long long*)c->d_scratch;
+  NEB_CUDA(c, cudaMemsetAsync(rowmax, 0, (size_t)npad * sizeof(unsigned long long), c->stream));
+  {
+    StageTimer t(c, NEB_STAGE_ASSEMBLE);
+    dim3 grid((unsigned)((n + kThreads - 1) / kThreads), (unsigned)((n + kTile - 1) / kTile));
+    if (c->math_fast)
+      assemble_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, c->d_colloc, c->stride,
+                                                                   c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rowmax);
+    else
+      assemble_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, c->d_colloc, c->stride,
+                                                                  c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rowmax);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+    int64_t padcells = (npad - n) * npad + n * (npad - n);
+    if (padcells > 0) {
+      pad_identity_kernel<<<(unsigned)((padcells + 255) / 256), 256, 0, c->stream>>>(c->d_K, n, npad);
+      c->launches++;
+      NEB_CUDA(c, cudaGetLastError());
+    }
+  }
+  {
+    StageTimer t(c, NEB_STAGE_EQUIL);
+    rscale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(rowmax, n, npad, c->d_rscale);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  return NEB_OK;
+}
+
+// Applies the row scales in place (done at the first neb_solve, so that neb_get_matrix before it
+// returns the unscaled matrix without a second copy).
+neb_status scale_matrix_rows(neb_ctx* c) {
+  StageTimer t(c, NEB_STAGE_EQUIL);
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)c->n);
+  scale_rows_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, c->n, c->npad, c->d_rscale);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return NEB_OK;
+}
+
+neb_status form_rhs(neb_ctx* c) {
+  int64_t n = c->n;
+  double *phi = nullptr, *E = nullptr;
+  if (c->q > 0) {
+    // Phi_sc, E_sc at the collocation points: reuse d_x (npad >= n) for phi and a scratch tail for E.
+    // field_at_points uses d_scratch for its partials, so E lives in a dedicated allocation.
+    phi = c->d_x;
+    NEB_CUDA(c, cudaMallocAsync((void**)&E, (size_t)3 * n * sizeof(double), c->stream));
+    // collocation points are stored with stride c->stride; field_at_points wants stride m: pack
+    double* pts = nullptr;
+    NEB_CUDA(c, cudaMallocAsync((void**)&pts, (size_t)3 * n * sizeof(double), c->stream));
+    for (int k = 0; k < 3; ++k)
+      NEB_CUDA(c, cudaMemcpyAsync(pts + k * n, c->d_colloc + k * c->stride, (size_t)n * sizeof(double),
+                                  cudaMemcpyDeviceToDevice, c->stream));
+    neb_status st = field_at_points(c, n, pts, false, true, phi, E);
+    cudaFreeAsync(pts, c->stream);
+    if (st != NEB_OK) { cudaFreeAsync(E, c->stream); return st; }
+  }
+  {
+    StageTimer t(c, NEB_STAGE_RHS);
+    rhs_kernel<<<(unsigned)((c->npad + 255) / 256), 256, 0, c->stream>>>(n, c->npad, c->stride, c->d_bc_kind,
+                                                                         c->d_bc_value, c->d_normal, phi, E, c->d_b);
+    c->launches++;
+  }
+  if (E) cudaFreeAsync(E, c->stream);
+  NEB_CUDA(c, cudaGetLastError());
+  return NEB_OK;
+}
+
+}  // namespace neb

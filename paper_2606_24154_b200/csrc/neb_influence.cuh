@@ -1,0 +1,141 @@
+// neb_influence.cuh — a2: exact potential and field of a uniformly charged flat rectangle, right
+// triangle or thin wire at one point (integrals P:121, P:125 with reading S2,
+// P:131), evaluated in the element's local frame (element in the local XZ plane, Y = normal)
+// and rotated to global.  The paper does not print the closed forms; the ones used here are
+// derived in DESIGN.md §3 (edge form: one logarithm per edge, one arctangent per element) and are
+// branch-free: every case distinction (near/far field, foot of the perpendicular inside/outside an
+// edge, on-surface and on-edge limits) is a select, so that a warp never diverges — the reason
+// the paper gives for keeping this stage off the GPU does not apply.
+#pragma once
+#include "neb_math.cuh"
+
+namespace neb {
+
+// Frame-table record (a1), 16 doubles per element, stored SoA in global memory (field-major):
+//   0..2  v0      corner / right-angle vertex / wire start
+//   3..5  ex      unit vector along e1 (local X)
+//   6..8  ey      unit normal e2 x e1 / |e2 x e1| (local Y)        [wire: unused]
+//   9..11 ez      unit vector along e2 (local Z)                    [wire: unused]
+//   12    a       |e1|
+//   13    b       |e2|                                              [wire: radius r_w]
+//   14    aux     triangle: 1/hypotenuse; wire: 2 pi r_w            [rect: unused]
+//   15    w       weight: sigma_j / (4 pi eps0) for evaluation (set by neb_solve / neb_set_sigma)
+#define NEB_REC 16
+
+struct Infl {
+  double phi, ex, ey, ez;   // primed potential and GLOBAL primed field components
+};
+
+// ln[(R+ + l+)/(R- + l-)] of one straight edge: lm < lp are the abscissae of its ends along the
+// edge measured from the foot of the perpendicular from P, Rm/Rp the distances to its ends, R0sq the
+// squared distance from P to the edge's line, L = lp - lm.  Three algebraically equal forms chosen by
+// the position of the foot so that nothing cancels; far away (Rm+Rp > 8L) 2 atanh(L/(Rm+Rp)) keeps
+// full RELATIVE accuracy of the small value (the far-field sums cancel by a factor r/L).
+template <class M>
+__device__ __forceinline__ double edge_log(double lm, double lp, double Rm, double Rp, double R0sq, double L) {
+  double s = Rm + Rp;
+  double pp = Rp + fabs(lp), qq = Rm + fabs(lm);
+  bool cA = lm >= 0.0, cB = lp <= 0.0;
+  double N = cB ? qq : pp;
+  N = (cA || cB) ? N : pp * qq;
+  double D = cA ? qq : (cB ? pp : R0sq);
+  return M::log_ratio(N, D, s > 8.0 * L, L, s);
+}
+
+// Rectangle [0,a] x [0,b] in the local XZ plane; (X, Y, Z) local coordinates of P.
+// out: phi', local field (fx, fy, fz).
+template <class M>
+__device__ __forceinline__ void rect_local(double a, double b, double X, double Y, double Z, double& phi,
+                                           double& fx, double& fy, double& fz) {
+  double u1 = -X, u2 = a - X, w1 = -Z, w2 = b - Z, y = fabs(Y);
+  double yy = y * y;
+  double A1 = fma(u1, u1, yy), A2 = fma(u2, u2, yy);      // squared distances to the lines x = x_i
+  double B1 = fma(w1, w1, yy), B2 = fma(w2, w2, yy);      // squared distances to the lines z = z_j
+  double r11 = M::sqrt_nn(fma(w1, w1, A1)), r12 = M::sqrt_nn(fma(w2, w2, A1));
+  double r21 = M::sqrt_nn(fma(w1, w1, A2)), r22 = M::sqrt_nn(fma(w2, w2, A2));
+  double F1 = edge_log<M>(w1, w2, r11, r12, A1, b);       // edge x = 0
+  double F2 = edge_log<M>(w1, w2, r21, r22, A2, b);       // edge x = a
+  double G1 = edge_log<M>(u1, u2, r11, r21, B1, a);       // edge z = 0
+  double G2 = edge_log<M>(u1, u2, r12, r22, B2, a);       // edge z = b
+  // solid angle: two fan triangles (c11,c21,c22), (c11,c22,c12); tan(Omega_t/2) = 2A_t |d| / D_t with the
+  // triple product written as area x height (exact for a flat element: no far-field cancellation)
+  double p = u1 * u2, q = w1 * w2;
+  double d1122 = p + yy + q;
+  double D1 = fma(r11 * r21, r22, fma(p + B1, r22, fma(d1122, r21, (A2 + q) * r11)));
+  double D2 = fma(r11 * r22, r12, fma(d1122, r12, fma(A1 + q, r22, (p + B2) * r11)));
+  double Nn = a * b * y;
+  double om = 2.0 * M::atan2_pos(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));
+  phi = fma(u2, F2, fma(-u1, F1, fma(w2, G2, fma(-w1, G1, -y * om))));
+  fx = F2 - F1;
+  fz = G2 - G1;
+  fy = (Y > 0.0) ? om : ((Y < 0.0) ? -om : 0.0);          // S5: principal value on the surface
+}
+
+// Right triangle (0,0), (a,0), (0,b) in the local XZ plane, ih = 1/sqrt(a^2+b^2).
+template <class M>
+__device__ __forceinline__ void tri_local(double a, double b, double ih, double X, double Y, double Z, double& phi,
+                                          double& fx, double& fy, double& fz) {
+  double uA = -X, uB = a - X, wA = -Z, wC = b - Z, y = fabs(Y);
+  double yy = y * y;
+  double A0 = fma(uA, uA, yy), W0 = fma(wA, wA, yy);
+  double RA = M::sqrt_nn(fma(wA, wA, A0)), RB = M::sqrt_nn(fma(uB, uB, W0)), RC = M::sqrt_nn(fma(wC, wC, A0));
+  double fAB = edge_log<M>(uA, uB, RA, RB, W0, a);        // leg on the X axis, outward normal -Z, P0 = Z
+  double fCA = edge_log<M>(wA, wC, RA, RC, A0, b);        // leg on the Z axis, outward normal -X, P0 = X
+  double ca = a * ih, cb = b * ih;                        // hypotenuse B->C: t = (-ca, cb), m = (cb, ca)
+  double lm = fma(-ca, uB, cb * wA);
+  double h = (a * a + b * b) * ih;
+  double lp = lm + h;
+  double P0 = fma(cb, uB, ca * wA);
+  double fBC = edge_log<M>(lm, lp, RB, RC, fma(P0, P0, yy), h);
+  double dAB = fma(uA, uB, W0), dAC = fma(wA, wC, A0), dBC = fma(uA, uB, fma(wA, wC, yy));
+  double D = fma(RA * RB, RC, fma(dAB, RC, fma(dAC, RB, dBC * RA)));
+  double om = 2.0 * M::atan2_pos(a * b * y, D);
+  phi = fma(Z, fAB, fma(X, fCA, fma(P0, fBC, -y * om)));
+  fx = fma(cb, fBC, -fCA);
+  fz = fma(ca, fBC, -fAB);
+  fy = (Y > 0.0) ? om : ((Y < 0.0) ? -om : 0.0);
+}
+
+// Element record fields of one rect/tri element, as scalars (read from shared memory by the caller).
+struct Frame {
+  double v0x, v0y, v0z, exx, exy, exz, eyx, eyy, eyz, ezx, ezy, ezz, a, b, aux;
+};
+
+template <class M, int KIND>
+__device__ __forceinline__ Infl influence(const Frame& f, double px, double py, double pz) {
+  double dx = px - f.v0x, dy = py - f.v0y, dz = pz - f.v0z;
+  Infl o;
+  if (KIND == 2) {
+    // thin wire on the local X axis from 0 to a (reading S24); line density = 2 pi r_w sigma (aux)
+    double t = fma(dx, f.exx, fma(dy, f.exy, dz * f.exz));
+    double qx = fma(-t, f.exx, dx), qy = fma(-t, f.exy, dy), qz = fma(-t, f.exz, dz);
+    double rho2 = fma(qx, qx, fma(qy, qy, qz * qz));
+    double rw = f.b;
+    bool inside = rho2 < rw * rw;
+    double rho2c = inside ? rw * rw : rho2;
+    double lm = -t, lp = f.a - t;
+    double Rm = M::sqrt_nn(fma(lm, lm, rho2c)), Rp = M::sqrt_nn(fma(lp, lp, rho2c));
+    double ph = edge_log<M>(lm, lp, Rm, Rp, rho2c, f.a);
+    double iRm = M::div_pos(1.0, fmax(Rm, NEB_TINY)), iRp = M::div_pos(1.0, fmax(Rp, NEB_TINY));
+    double er = M::div_pos(fma(lp, iRp, -lm * iRm), fmax(rho2c, NEB_TINY));   // E'_rho / rho
+    double ea = iRp - iRm;
+    double sc = inside ? 0.0 : f.aux;
+    o.phi = f.aux * ph;
+    o.ex = sc * fma(er, qx, ea * f.exx);
+    o.ey = sc * fma(er, qy, ea * f.exy);
+    o.ez = sc * fma(er, qz, ea * f.exz);
+    return o;
+  }
+  double X = fma(dx, f.exx, fma(dy, f.exy, dz * f.exz));
+  double Y = fma(dx, f.eyx, fma(dy, f.eyy, dz * f.eyz));
+  double Z = fma(dx, f.ezx, fma(dy, f.ezy, dz * f.ezz));
+  double lx, ly, lz;
+  if (KIND == 0) rect_local<M>(f.a, f.b, X, Y, Z, o.phi, lx, ly, lz);
+  else tri_local<M>(f.a, f.b, f.aux, X, Y, Z, o.phi, lx, ly, lz);
+  o.ex = fma(lx, f.exx, fma(ly, f.eyx, lz * f.ezx));
+  o.ey = fma(lx, f.exy, fma(ly, f.eyy, lz * f.ezy));
+  o.ez = fma(lx, f.exz, fma(ly, f.eyz, lz * f.ezz));
+  return o;
+}
+
+}  // namespace neb

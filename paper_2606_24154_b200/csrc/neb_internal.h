@@ -1,0 +1,123 @@
+// neb_internal.h — declarations shared by the translation units of libneb.so (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/neb.h"
+
+namespace neb {
+
+constexpr double kEps0 = 8.8541878128e-12;                 // F/m (reading S3)
+constexpr double kCoulomb = 1.0 / (4.0 * 3.14159265358979323846 * kEps0);
+constexpr int kRec = 16;                                   // doubles per frame-table record
+constexpr int kPad = 128;                                  // matrix dimension is padded to a multiple of this
+
+// Frame tables (a1), elements sorted by kind: [rect | tri | wire].  SoA, field-major:
+// rec[f * stride + j], f < kRec (fields listed in neb_influence.cuh).
+struct GeoTables {
+  const double* rec;
+  int64_t stride;
+  int32_t n_rect, n_tri, n_wire;
+};
+
+struct StageStat {
+  double ms = 0.0;
+  int64_t launches = 0;
+};
+
+}  // namespace neb
+
+struct neb_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int num_sms = 0;
+  std::string err;
+
+  // options
+  int math_fast = 1;
+  int lu_nb = 64;
+  int profile = 0;
+
+  // geometry
+  int64_t n = 0, npad = 0, stride = 0;
+  int32_t n_rect = 0, n_tri = 0, n_wire = 0, n_img = 0;
+  double* d_rec = nullptr;        // kRec * stride
+  int32_t* d_perm = nullptr;      // sorted position -> caller index
+  double* d_colloc = nullptr;     // 3 * stride, sorted order
+  double* d_normal = nullptr;     // 3 * stride, sorted order
+  int32_t* d_bc_kind = nullptr;   // sorted
+  double* d_bc_value = nullptr;   // sorted
+  double* d_diag = nullptr;       // sorted: 1/(2 eps0 lambda) on dielectric rows, else 0
+  double* d_img = nullptr;        // 3 * n_img
+  int32_t* d_flag = nullptr;      // device error flags (validation, singular pivot)
+
+  // matrix / factors
+  double* d_K = nullptr;          // npad x npad column-major
+  double* d_rscale = nullptr;     // npad
+  int32_t* d_ipiv = nullptr;      // npad (0-based absolute row)
+  int32_t* d_rowperm = nullptr;   // npad: composed row permutation of the factorisation
+  double* d_b = nullptr;          // npad, unscaled RHS (sorted order)
+  double* d_x = nullptr;          // npad work vector
+  double* d_sigma = nullptr;      // n, caller order
+  void* d_panel_ws = nullptr;     // LU panel exchange buffers
+  bool assembled = false, factored = false, have_sigma = false;
+
+  // space charges: SoA x,y,z,q (4 * q_cap)
+  double* d_charges = nullptr;
+  int64_t q = 0, q_cap = 0;
+
+  // scratch for partial sums / staging
+  double* d_scratch = nullptr;
+  size_t scratch_bytes = 0;
+
+  // stats
+  int64_t launches = 0;
+  neb::StageStat stat[NEB_STAGE_COUNT];
+  cudaEvent_t ev0[NEB_STAGE_COUNT] = {}, ev1[NEB_STAGE_COUNT] = {};
+};
+
+namespace neb {
+
+// error helpers ---------------------------------------------------------------------------------
+neb_status fail(neb_ctx* c, neb_status st, const std::string& msg);
+#define NEB_CUDA(c, expr)                                                                         \
+  do {                                                                                            \
+    cudaError_t e_ = (expr);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return neb::fail((c), e_ == cudaErrorMemoryAllocation ? NEB_ENOMEM : NEB_ECUDA,             \
+                       std::string(#expr) + ": " + cudaGetErrorString(e_));                       \
+  } while (0)
+#define NEB_TRY(expr)                 \
+  do {                                \
+    neb_status s_ = (expr);           \
+    if (s_ != NEB_OK) return s_;      \
+  } while (0)
+
+neb_status ensure_scratch(neb_ctx* c, size_t bytes);
+
+struct StageTimer {   // records device time of a stage when profiling is on
+  neb_ctx* c;
+  int stage;
+  int64_t l0;
+  StageTimer(neb_ctx* c_, int stage_);
+  ~StageTimer();
+};
+
+// neb_field.cu ------------------------------------------------------------------------------------
+// Phi/E at m device points (SoA) from the elements (weights in rec field 15) and/or the charges.
+neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_elements, bool use_charges,
+                           double* d_phi, double* d_E);
+neb_status assemble_matrix(neb_ctx* c);   // a3 + S15 row scales (computed, not yet applied)
+neb_status scale_matrix_rows(neb_ctx* c); // applies the row scales in place
+neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
+
+// neb_lu.cu ---------------------------------------------------------------------------------------
+neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-scaled)
+neb_status lu_solve(neb_ctx* c);          // a6: d_x <- solution of (scaled) system for RHS d_b
+size_t lu_panel_ws_bytes(int num_sms);
+
+// neb_peaks.cu ------------------------------------------------------------------------------------
+neb_status fp64_peak(neb_ctx* c, int kind, double* tflops);
+
+}  // namespace neb

@@ -1,0 +1,480 @@
+// neb_lu.cu — a5/a6: dense fp64 LU with partial pivoting on the resident, row-scaled influence
+// matrix (InvertMatrix with OptLU, Alg. 1; readings S13 "keep the factors, no explicit
+// inverse", S15, S16), and the two triangular solves (Solve).
+//
+// Right-looking blocked factorisation, panel width NB = 64, matrix column-major with leading
+// dimension npad (a multiple of 128; the pad block is the identity, so every tile is full):
+//   panel_kernel   one cooperative launch per panel: each CTA keeps its slab of panel rows in shared
+//                  memory; per column one grid-wide exchange (candidate pivot + candidate row + diagonal
+//                  row through global memory, one grid barrier), then the rank-1 update in shared memory
+//   laswp_kernel   applies the panel's 64 row exchanges to the columns left and right of the panel
+//   trsm_kernel    U12 = L11^-1 A12, one thread per column, the column in registers
+//   gemm_kernel    A22 -= L21 U12 on the FP64 tensor cores: mma.sync.m8n8k4.f64 (SASS DMMA), 128x64 CTA
+//                  tiles, operands staged by cp.async into padded (conflict-free) shared memory
+// tcgen05/UMMA has no f64 kind, so the warp-level DMMA is the FP64 tensor path on sm_100a.
+#include <cooperative_groups.h>
+
+#include "neb_internal.h"
+
+namespace neb {
+
+constexpr int NB = 64;           // panel width
+constexpr int PANEL_THREADS = 256;
+
+// ------------------------------------------------------------------------------------------------
+// grid barrier for the cooperative panel kernel (all CTAs co-resident: cooperative launch)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(counter, 1u);
+    unsigned int v;
+    do {
+      asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+    } while (v < target);
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+struct PanelWs {          // global exchange buffers, double-buffered by step parity
+  unsigned int counter;   // monotone barrier counter (reset by the host before each launch)
+  int pad_[3];
+  double cand_val[2][160];
+  int cand_row[2][160];
+  double cand_vec[2][160][NB];
+  double diag_vec[2][NB];
+};
+
+size_t lu_panel_ws_bytes(int) { return sizeof(PanelWs); }
+
+// One panel: columns [k, k+NB), rows [k, npad).  CTA b owns rows [k + b*mc, k + (b+1)*mc) (mc a
+// multiple of 32), stored in shared memory column-major: sA[c * mc + r].
+__global__ void __launch_bounds__(PANEL_THREADS) panel_kernel(double* __restrict__ A, int64_t ld, int64_t npad, int64_t k,
+                                                              int mc, int32_t* __restrict__ ipiv, PanelWs* ws,
+                                                              int32_t* __restrict__ flag) {
+  extern __shared__ double sA[];
+  __shared__ double s_prow[NB], s_drow[NB];
+  __shared__ double s_wval[PANEL_THREADS / 32];
+  __shared__ int s_wrow[PANEL_THREADS / 32];
+  __shared__ int s_win_cta, s_win_row;
+  const int tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
+  const int64_t row0 = k + (int64_t)b * mc;
+  const int nrows = (int)max((int64_t)0, min((int64_t)mc, npad - row0));   // rows this CTA really owns
+  // load slab
+  for (int idx = tid; idx < mc * NB; idx += PANEL_THREADS) {
+    int r = idx % mc, c = idx / mc;
+    sA[idx] = (r < nrows) ? A[(row0 + r) + (k + c) * ld] : 0.0;
+  }
+  __syncthreads();
+  unsigned int epoch = 0;
+  for (int j = 0; j < NB; ++j) {
+    const int par = j & 1;
+    const int64_t dr = k + j;                      // diagonal row of this step
+    // (1) local pivot candidate: max |a[r][j]| over owned rows >= dr, ties -> lowest row
+    double best = -1.0;
+    int brow = 0x7fffffff;
+    for (int r = tid; r < nrows; r += PANEL_THREADS) {
+      int64_t gr = row0 + r;
+      if (gr >= dr) {
+        double v = fabs(sA[j * mc + r]);
+        if (!(v == v)) v = 0.0;                    // NaN never wins; caught by the zero-pivot test
+        if (v > best) { best = v; brow = (int)gr; }
+      }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      double ov = __shfl_down_sync(0xffffffffu, best, o);
+      int orow = __shfl_down_sync(0xffffffffu, brow, o);
+      if (ov > best || (ov == best && orow < brow)) { best = ov; brow = orow; }
+    }
+    if ((tid & 31) == 0) { s_wval[tid >> 5] = best; s_wrow[tid >> 5] = brow; }
+    __syncthreads();
+    if (tid == 0) {
+      for (int w = 1; w < PANEL_THREADS / 32; ++w)
+        if (s_wval[w] > best || (s_wval[w] == best && s_wrow[w] < brow)) { best = s_wval[w]; brow = s_wrow[w]; }
+      ws->cand_val[par][b] = best;
+      ws->cand_row[par][b] = brow;
+      s_win_row = brow;                            // local candidate row, for the publication below
+    }
+    __syncthreads();
+    {
+      int lrow = s_win_row;
+      if (tid < NB && lrow != 0x7fffffff) ws->cand_vec[par][b][tid] = sA[tid * mc + (int)(lrow - row0)];
+      if (tid < NB && dr >= row0 && dr < row0 + nrows) ws->diag_vec[par][tid] = sA[tid * mc + (int)(dr - row0)];
+    }
+    // (2) grid-wide exchange
+    epoch += (unsigned)G;
+    grid_barrier(&ws->counter, epoch);
+    // (3) global winner
+    if (tid < 32) {
+      double wv = -1.0; int wr = 0x7fffffff, wc = 0;
+      for (int c = tid; c < G; c += 32) {
+        double v = __ldcg(&ws->cand_val[par][c]);
+        int r = __ldcg(&ws->cand_row[par][c]);
+        if (v > wv || (v == wv && r < wr)) { wv = v; wr = r; wc = c; }
+      }
+      for (int o = 16; o > 0; o >>= 1) {
+        double ov = __shfl_down_sync(0xffffffffu, wv, o);
+        int orow = __shfl_down_sync(0xffffffffu, wr, o);
+        int oc = __shfl_down_sync(0xffffffffu, wc, o);
+        if (ov > wv || (ov == wv && orow < wr)) { wv = ov; wr = orow; wc = oc; }
+      }
+      if (tid == 0) {
+        s_win_cta = wc; s_win_row = wr;
+        if (b == 0) {
+          ipiv[dr] = wr;
+          if (!(wv > 0.0)) atomicOr(flag, 2);      // zero / NaN pivot: NEB_ESINGULAR
+        }
+      }
+    }
+    __syncthreads();
+    const int wrow = s_win_row, wcta = s_win_cta;
+    if (tid < NB) {
+      s_prow[tid] = __ldcg(&ws->cand_vec[par][wcta][tid]);
+      s_drow[tid] = __ldcg(&ws->diag_vec[par][tid]);
+    }
+    __syncthreads();
+    // (4) exchange rows dr <-> wrow inside the panel
+    if (wrow != (int)dr && tid < NB) {
+      if (wrow >= row0 && wrow < row0 + nrows) sA[tid * mc + (int)(wrow - row0)] = s_drow[tid];
+      if (dr >= row0 && dr < row0 + nrows) sA[tid * mc + (int)(dr - row0)] = s_prow[tid];
+    }
+    __syncthreads();
+    // (5) multipliers and rank-1 update of the columns to the right, rows below dr
+    const double piv = s_prow[j];
+    const double invp = (piv != 0.0) ? 1.0 / piv : 0.0;
+    const int ncol = NB - 1 - j;
+    for (int idx = tid; idx < mc * (ncol + 1); idx += PANEL_THREADS) {
+      int r = idx % mc, cc = idx / mc;             // cc = 0: the multiplier column itself
+      int64_t gr = row0 + r;
+      if (r < nrows && gr > dr) {
+        double l = sA[j * mc + r] * invp;
+        if (cc == 0) {
+          // written after every reader of this column in this pass has its own copy: readers below
+          // recompute l from the unscaled value, so defer the store to the second pass
+        } else {
+          int c = j + cc;
+          sA[c * mc + r] = fma(-l, s_prow[c], sA[c * mc + r]);
+        }
+      }
+    }
+    __syncthreads();
+    for (int r = tid; r < nrows; r += PANEL_THREADS)
+      if (row0 + r > dr) sA[j * mc + r] *= invp;
+    __syncthreads();
+  }
+  // write the factored slab back
+  for (int idx = tid; idx < mc * NB; idx += PANEL_THREADS) {
+    int r = idx % mc, c = idx / mc;
+    if (r < nrows) A[(row0 + r) + (k + c) * ld] = sA[idx];
+  }
+}
+
+// Row exchanges of one panel applied to every column outside it.  One thread per column.
+__global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t npad, int64_t k, const int32_t* __restrict__ ipiv) {
+  __shared__ int s_piv[NB];
+  if (threadIdx.x < NB) s_piv[threadIdx.x] = ipiv[k + threadIdx.x];
+  __syncthreads();
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= npad - NB) return;
+  if (c >= k) c += NB;                             // skip the panel's own columns
+  double* col = A + c * ld;
+  for (int t = 0; t < NB; ++t) {
+    int p = s_piv[t];
+    if (p != k + t) {
+      double a = col[k + t], bb = col[p];
+      col[k + t] = bb;
+      col[p] = a;
+    }
+  }
+}
+
+// U12 = L11^-1 A12: rows [k, k+NB), columns [k+NB, npad).  CTA = 256 threads on a slab of 64 columns held
+// in shared memory (sB[c][i], odd leading dimension: conflict-free), right-looking substitution.
+constexpr int TRSM_THREADS = 256;
+constexpr size_t TRSM_SMEM = (size_t)2 * NB * (NB + 1) * sizeof(double);
+__global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k) {
+  extern __shared__ double s_trsm[];
+  double(*sL)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm);                    // sL[i][j] = L11[i][j]
+  double(*sB)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm + NB * (NB + 1));     // sB[c][i]
+  const int tid = threadIdx.x, r = tid & (NB - 1), q = tid >> 6;     // q = 0..3
+  const int64_t c0 = k + NB + (int64_t)blockIdx.x * NB;
+  for (int j = q; j < NB; j += 4) sL[r][j] = A[(k + r) + (k + j) * ld];
+  for (int c = q; c < NB; c += 4) sB[c][r] = A[(k + r) + (c0 + c) * ld];
+  __syncthreads();
+  for (int j = 0; j < NB - 1; ++j) {
+    const double xj = sB[r][j];                   // thread (c = r, row group q)
+    for (int i = j + 1 + q; i < NB; i += 4) sB[r][i] = fma(-sL[i][j], xj, sB[r][i]);
+    __syncthreads();
+  }
+  for (int c = q; c < NB; c += 4) A[(k + r) + (c0 + c) * ld] = sB[c][r];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Trailing update C -= L * U with C = A[r0.., r0..] (m x m), L = A[r0.., k..k+64), U = A[k..k+64, r0..].
+// CTA tile 128 (rows) x 64 (cols), 8 warps as 4 (rows) x 2 (cols), warp tile 32 x 32 = 4 x 4 DMMA tiles.
+// The mma computes the transposed tile: mma row <-> C column, mma col <-> C row, so that each lane's
+// two accumulators are two consecutive rows of one column (16-byte global accesses).
+// ------------------------------------------------------------------------------------------------
+constexpr int GM = 128, GN = 64, GK = NB;
+constexpr int LDL = GM + 4;    // shared leading dimensions: stride mod 16 (in doubles) = 4 -> conflict-free
+constexpr int LDU = GK + 4;
+constexpr int GEMM_THREADS = 256;
+constexpr size_t GEMM_SMEM = (size_t)(GK * LDL + GN * LDU) * sizeof(double);
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t r0,
+                                                               int64_t m) {
+  extern __shared__ __align__(16) double smem[];
+  double* sL = smem;                 // sL[kk * LDL + i] = L[i][kk]
+  double* sU = smem + GK * LDL;      // sU[j * LDU + kk] = U[kk][j]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t i0 = r0 + (int64_t)blockIdx.x * GM;       // first row of the tile
+  const int64_t j0 = r0 + (int64_t)blockIdx.y * GN;       // first column
+  const int rows_here = (int)min((int64_t)GM, r0 + m - i0);   // 64 or 128
+  // stage operands: two k-halves as two cp.async groups
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    // L: 32 k-columns x 128 rows = 32 x 64 16-byte chunks
+    for (int idx = tid; idx < 32 * (GM / 2); idx += GEMM_THREADS) {
+      int kk = half * 32 + idx / (GM / 2), ch = idx % (GM / 2);
+      if (2 * ch < rows_here) cp_async16(sL + kk * LDL + 2 * ch, A + (i0 + 2 * ch) + (k + kk) * ld);
+    }
+    // U: 64 columns x 32 k-rows = 64 x 16 chunks
+    for (int idx = tid; idx < GN * 16; idx += GEMM_THREADS) {
+      int j = idx / 16, ch = idx % 16;
+      cp_async16(sU + j * LDU + half * 32 + 2 * ch, A + (k + half * 32 + 2 * ch) + (j0 + j) * ld);
+    }
+    cp_async_commit();
+  }
+  const int wr = warp & 3, wc = warp >> 2;                // warp tile origin: rows wr*32, cols wc*32
+  const int g = lane >> 2, t = lane & 3;
+  const bool active = wr * 32 < rows_here;
+  // accumulators start from C: acc[ni][mi] <-> C[i0 + wr*32 + mi*8 + 2t + {0,1}][j0 + wc*32 + ni*8 + g]
+  double acc[4][4][2];
+  if (active) {
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi) {
+        const double2 v = *reinterpret_cast<const double2*>(A + (i0 + wr * 32 + mi * 8 + 2 * t) + (j0 + wc * 32 + ni * 8 + g) * ld);
+        acc[ni][mi][0] = v.x; acc[ni][mi][1] = v.y;
+      }
+  }
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    if (half == 0) cp_async_wait<1>(); else cp_async_wait<0>();
+    __syncthreads();
+    if (active) {
+#pragma unroll 2
+      for (int k4 = half * 8; k4 < half * 8 + 8; ++k4) {
+        double fa[4], fb[4];
+        // mma A operand (row = C column n, col = k): U[k4*4 + t][n = g]
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) fa[ni] = sU[(wc * 32 + ni * 8 + g) * LDU + k4 * 4 + t];
+        // mma B operand (row = k, col = C row m): -L[m = g][k4*4 + t]
+#pragma unroll
+        for (int mi = 0; mi < 4; ++mi) fb[mi] = -sL[(k4 * 4 + t) * LDL + wr * 32 + mi * 8 + g];
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+          for (int mi = 0; mi < 4; ++mi) dmma884(acc[ni][mi][0], acc[ni][mi][1], fa[ni], fb[mi]);
+      }
+    }
+  }
+  if (active) {
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi)
+        *reinterpret_cast<double2*>(A + (i0 + wr * 32 + mi * 8 + 2 * t) + (j0 + wc * 32 + ni * 8 + g) * ld) =
+            make_double2(acc[ni][mi][0], acc[ni][mi][1]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6: triangular solves on the resident factors
+// ------------------------------------------------------------------------------------------------
+// Composes the row exchanges into one permutation: rowperm[i] = original row that ends in position i.
+__global__ void compose_perm_kernel(const int32_t* __restrict__ ipiv, int32_t* __restrict__ rowperm, int npad) {
+  extern __shared__ int s_perm[];
+  for (int i = threadIdx.x; i < npad; i += blockDim.x) s_perm[i] = i;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < npad; ++i) {
+      int p = ipiv[i];
+      if (p != i) { int tmp = s_perm[i]; s_perm[i] = s_perm[p]; s_perm[p] = tmp; }
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < npad; i += blockDim.x) rowperm[i] = s_perm[i];
+}
+
+__global__ void compose_perm_global_kernel(const int32_t* __restrict__ ipiv, int32_t* rowperm, int npad) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    for (int i = 0; i < npad; ++i) rowperm[i] = i;
+    for (int i = 0; i < npad; ++i) {
+      int p = ipiv[i];
+      if (p != i) { int tmp = rowperm[i]; rowperm[i] = rowperm[p]; rowperm[p] = tmp; }
+    }
+  }
+}
+
+__global__ void permute_scale_kernel(const double* __restrict__ b, const double* __restrict__ rscale,
+                                     const int32_t* __restrict__ rowperm, int64_t npad, double* __restrict__ x) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < npad) { int p = rowperm[i]; x[i] = b[p] * rscale[p]; }
+}
+
+// Diagonal block solve, one CTA of 64 threads.  lower: unit lower triangular; else upper.
+__global__ void __launch_bounds__(NB) diag_solve_kernel(const double* __restrict__ A, int64_t ld, int64_t kb, double* x, int lower) {
+  __shared__ double sT[NB][NB + 1];
+  __shared__ double sx[NB];
+  const int tid = threadIdx.x;
+  for (int j = 0; j < NB; ++j) sT[tid][j] = A[(kb + tid) + (kb + j) * ld];
+  sx[tid] = x[kb + tid];
+  __syncthreads();
+  if (lower) {
+    for (int j = 0; j < NB - 1; ++j) {
+      if (tid > j) sx[tid] = fma(-sT[tid][j], sx[j], sx[tid]);
+      __syncthreads();
+    }
+  } else {
+    for (int j = NB - 1; j >= 0; --j) {
+      if (tid == j) sx[j] = sx[j] / sT[j][j];
+      __syncthreads();
+      if (tid < j) sx[tid] = fma(-sT[tid][j], sx[j], sx[tid]);
+      __syncthreads();
+    }
+  }
+  x[kb + tid] = sx[tid];
+}
+
+// x[rows] -= A[rows, kb..kb+64) * x[kb..kb+64); rows = [r_lo, r_hi).  One thread per row.
+__global__ void gemv_update_kernel(const double* __restrict__ A, int64_t ld, int64_t kb, int64_t r_lo, int64_t r_hi, double* x) {
+  __shared__ double sx[NB];
+  if (threadIdx.x < NB) sx[threadIdx.x] = x[kb + threadIdx.x];
+  __syncthreads();
+  int64_t i = r_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= r_hi) return;
+  const double* a = A + i + kb * ld;
+  double acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;
+#pragma unroll 4
+  for (int j = 0; j < NB; j += 4) {
+    acc0 = fma(a[(j + 0) * ld], sx[j + 0], acc0);
+    acc1 = fma(a[(j + 1) * ld], sx[j + 1], acc1);
+    acc2 = fma(a[(j + 2) * ld], sx[j + 2], acc2);
+    acc3 = fma(a[(j + 3) * ld], sx[j + 3], acc3);
+  }
+  x[i] -= (acc0 + acc1) + (acc2 + acc3);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+neb_status lu_factor(neb_ctx* c) {
+  const int64_t npad = c->npad, ld = c->npad;
+  StageTimer tt(c, NEB_STAGE_LU);
+  static bool attr_set = false;
+  if (!attr_set) {
+    NEB_CUDA(c, cudaFuncSetAttribute(panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    NEB_CUDA(c, cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
+    NEB_CUDA(c, cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM));
+    attr_set = true;
+  }
+  PanelWs* ws = (PanelWs*)c->d_panel_ws;
+  for (int64_t k = 0; k < npad; k += NB) {
+    const int64_t mrows = npad - k;
+    // rows per CTA: multiple of 32, at most 200 KB of shared memory (390 rows -> 384)
+    int G = (int)min((int64_t)c->num_sms, (mrows + 63) / 64);
+    if (G > 148) G = 148;
+    int mc = (int)((mrows + G - 1) / G);
+    mc = (mc + 31) / 32 * 32;
+    size_t smem = (size_t)mc * NB * sizeof(double);
+    if (smem > 200 * 1024) return fail(c, NEB_ENOMEM, "LU panel slab exceeds shared memory: n too large for this build");
+    G = (int)((mrows + mc - 1) / mc);
+    NEB_CUDA(c, cudaMemsetAsync(&ws->counter, 0, sizeof(unsigned int), c->stream));
+    {
+      double* A = c->d_K;
+      int64_t ld_ = ld, npad_ = npad, k_ = k;
+      int mc_ = mc;
+      int32_t* ipiv = c->d_ipiv;
+      int32_t* flag = c->d_flag;
+      void* args[] = {&A, &ld_, &npad_, &k_, &mc_, &ipiv, &ws, &flag};
+      NEB_CUDA(c, cudaLaunchCooperativeKernel((void*)panel_kernel, dim3(G), dim3(PANEL_THREADS), args, smem, c->stream));
+      c->launches++;
+    }
+    {
+      int64_t ncols = npad - NB;
+      if (ncols > 0) {
+        laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, npad, k, c->d_ipiv);
+        c->launches++;
+      }
+    }
+    const int64_t r0 = k + NB, m = npad - r0;
+    if (m > 0) {
+      trsm_kernel<<<(unsigned)(m / NB), TRSM_THREADS, TRSM_SMEM, c->stream>>>(c->d_K, ld, k);
+      c->launches++;
+      StageTimer tg(c, NEB_STAGE_LU_GEMM);
+      dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(m / GN));
+      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, c->stream>>>(c->d_K, ld, k, r0, m);
+      c->launches++;
+    }
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  // composed permutation for the solves
+  if ((size_t)npad * sizeof(int) <= 200 * 1024) {
+    static bool attr2 = false;
+    if (!attr2) {
+      NEB_CUDA(c, cudaFuncSetAttribute(compose_perm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+      attr2 = true;
+    }
+    compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+  } else {
+    compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+  }
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return NEB_OK;
+}
+
+neb_status lu_solve(neb_ctx* c) {
+  const int64_t npad = c->npad, ld = c->npad;
+  StageTimer tt(c, NEB_STAGE_TRISOLVE);
+  permute_scale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(c->d_b, c->d_rscale, c->d_rowperm, npad, c->d_x);
+  c->launches++;
+  for (int64_t kb = 0; kb < npad; kb += NB) {          // forward: L y = P b
+    diag_solve_kernel<<<1, NB, 0, c->stream>>>(c->d_K, ld, kb, c->d_x, 1);
+    c->launches++;
+    int64_t lo = kb + NB;
+    if (lo < npad) {
+      gemv_update_kernel<<<(unsigned)((npad - lo + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, kb, lo, npad, c->d_x);
+      c->launches++;
+    }
+  }
+  for (int64_t kb = npad - NB; kb >= 0; kb -= NB) {    // backward: U x = y
+    diag_solve_kernel<<<1, NB, 0, c->stream>>>(c->d_K, ld, kb, c->d_x, 0);
+    c->launches++;
+    if (kb > 0) {
+      gemv_update_kernel<<<(unsigned)((kb + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, kb, 0, kb, c->d_x);
+      c->launches++;
+    }
+  }
+  NEB_CUDA(c, cudaGetLastError());
+  return NEB_OK;
+}
+
+}  // namespace neb

@@ -1,0 +1,466 @@
+"""Parity of the CUDA path (through the C ABI of include/neb.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  * Phi and |E|: max relative error 1e-10 for points farther than 1e-3 element sizes from every
+    element, 1e-7 otherwise (reading S18); denominators are floored at 1e-6 x the median magnitude so
+    that points where the field cancels to zero do not divide by zero;
+  * solved charge densities: 1e-9 relative, norm-wise (reading S14); LU residual 1e-13 (S16).
+The oracle runs in its long-double build ("ld") as the truth.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from workloads import configs as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_FAR, TOL_NEAR, TOL_SIGMA, TOL_K = 1e-10, 1e-7, 1e-9, 1e-10
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2606_24154_b200 as pkg
+    return pkg
+
+
+@pytest.fixture()
+def nb(P):
+    h = P.Neb()
+    yield h
+    h.close()
+
+
+def rel_err(got, want):
+    floor = 1e-6 * np.median(np.abs(want)) if want.size else 0.0
+    return np.abs(got - want) / np.maximum(np.abs(want), floor)
+
+
+def vec_rel_err(got, want):
+    mag = np.linalg.norm(want, axis=0)
+    floor = 1e-6 * np.median(mag) if mag.size else 0.0
+    return np.linalg.norm(got - want, axis=0) / np.maximum(mag, floor)
+
+
+def check_field(phi, E, phi_o, E_o, tol, what=""):
+    e1, e2 = rel_err(phi, phi_o).max(), vec_rel_err(E, E_o).max()
+    assert e1 <= tol, f"{what} Phi rel err {e1:.3e} > {tol}"
+    assert e2 <= tol, f"{what} |E| rel err {e2:.3e} > {tol}"
+
+
+def test_native_library_is_in_tree(P):
+    assert os.path.dirname(P.lib_path()) == os.path.dirname(P.__file__)
+    assert os.path.exists(P.lib_path())
+
+
+# ---------------------------------------------------------------------------------------------
+# a2: the influence function, one element at a time, both math policies
+# ---------------------------------------------------------------------------------------------
+def _single_element_points(pr, rs, m):
+    """Points around element 0: log-uniform distances 1e-3 L .. 3e3 L, plus in-plane and on-axis sets."""
+    v0, e1, e2 = pr.v0[:, 0], pr.e1[:, 0], pr.e2[:, 0]
+    L = max(np.linalg.norm(e1), np.linalg.norm(e2))
+    c = v0 + 0.5 * e1 + 0.5 * e2
+    u = rs.normal(size=(3, m))
+    u /= np.linalg.norm(u, axis=0)
+    dist = L * 10.0 ** rs.uniform(-3, 3.5, size=m)
+    pts = c[:, None] + u * dist
+    # in-plane points (d = 0 exactly in the local frame up to rounding), inside and outside
+    s, t = rs.uniform(-1.5, 2.5, size=m // 4), rs.uniform(-1.5, 2.5, size=m // 4)
+    inplane = v0[:, None] + e1[:, None] * s + e2[:, None] * t
+    # just above / below the surface over the interior
+    nrm = np.cross(e2, e1)
+    nrm /= np.linalg.norm(nrm)
+    s, t = rs.uniform(0.05, 0.45, size=m // 4), rs.uniform(0.05, 0.45, size=m // 4)
+    hgt = L * 10.0 ** rs.uniform(-6, -2, size=m // 4) * rs.choice([-1, 1], size=m // 4)
+    hover = v0[:, None] + e1[:, None] * s + e2[:, None] * t + nrm[:, None] * hgt
+    return np.concatenate([pts, inplane, hover], axis=1), dist
+
+
+@pytest.mark.parametrize("math", [1, 0])
+@pytest.mark.parametrize("kind", [W.RECT, W.TRI, W.WIRE])
+def test_influence_single_element(nb, orc, kind, math):
+    nb.set_option(0, math)
+    rs = np.random.RandomState(100 + kind)
+    for seed in range(4):
+        pr = W.random_elements(1, seed=50 + 7 * seed + kind, kinds=(kind,), size_mm=(0.05, 2.0))
+        pts, dist = _single_element_points(pr, rs, 2000)
+        if kind == W.WIRE:      # stay outside the wire's own volume, where the field is defined to be 0 (S24)
+            t = pr.e1[:, 0] / np.linalg.norm(pr.e1[:, 0])
+            d = pts - pr.v0[:, :1]
+            rho = np.linalg.norm(d - t[:, None] * (t @ d), axis=0)
+            pts = pts[:, rho > 1.5 * pr.radius[0]]
+        g = orc.Geometry(pr)
+        sig = np.array([1.0 / orc.K_COULOMB])
+        nb.assemble_problem(pr)
+        nb.set_sigma(sig)
+        phi, E = nb.eval(pts)
+        phi_o, E_o = orc.evaluate(g, sig, pts)
+        assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E))
+        # reading S18: 1e-10 beyond 1e-3 element sizes from the element, 1e-7 closer.  Distance measured to the
+        # element's bounding rectangle in its plane (a lower bound of the true distance for triangles)
+        v0, e1, e2 = pr.v0[:, 0], pr.e1[:, 0], pr.e2[:, 0]
+        a, b = np.linalg.norm(e1), np.linalg.norm(e2)
+        d = pts - v0[:, None]
+        X = (e1 / a) @ d
+        if kind == W.WIRE:
+            far = np.ones(pts.shape[1], dtype=bool)
+        else:
+            Z = (e2 / b) @ d
+            nrm = np.cross(e2 / b, e1 / a)
+            Y = nrm @ d
+            ox, oz = np.maximum(0, np.maximum(-X, X - a)), np.maximum(0, np.maximum(-Z, Z - b))
+            far = np.sqrt(ox ** 2 + oz ** 2 + Y ** 2) >= 1e-3 * max(a, b)
+        assert far.sum() > 1000 and (kind == W.WIRE or (~far).sum() > 50)
+        e_phi = np.abs(phi - phi_o) / np.abs(phi_o)
+        e_E = np.linalg.norm(E - E_o, axis=0) / np.linalg.norm(E_o, axis=0)
+        worst_far = max(e_phi[far].max(), e_E[far].max())
+        worst_near = max(e_phi[~far].max(initial=0.0), e_E[~far].max(initial=0.0))
+        assert worst_far <= TOL_FAR, (kind, math, seed, worst_far)
+        assert worst_near <= TOL_NEAR, (kind, math, seed, worst_near)
+
+
+def test_influence_singular_limits(nb, orc):
+    """On-surface, on-edge, at-vertex and edge-extension points: finite everywhere, Phi exact (S5, S6)."""
+    for kind in (W.RECT, W.TRI):
+        pr = W.random_elements(1, seed=3, kinds=(kind,), size_mm=(0.5, 1.0))
+        pr.v0[:] = 0.0
+        pr.e1[:, 0] = [1e-3, 0, 0]
+        pr.e2[:, 0] = [0, 0, 0.6e-3]
+        a, b = 1e-3, 0.6e-3
+        pts = np.array([[0.3 * a, 0, 0.2 * b],      # interior, on the surface
+                        [0.4 * a, 0, 0.0],          # on an edge
+                        [0.0, 0, 0.0],              # at a vertex
+                        [1.7 * a, 0, 0.0],          # on the extension of an edge
+                        [0.0, 0, -0.5 * b],
+                        [a, 0, 0.0],
+                        [0.5 * a, 0, 0.5 * b if kind == W.RECT else 0.3 * b]]).T.copy()
+        g = orc.Geometry(pr)
+        sig = np.array([1.0 / orc.K_COULOMB])
+        for math in (1, 0):
+            nb.set_option(0, math)
+            nb.assemble_problem(pr)
+            nb.set_sigma(sig)
+            phi, E = nb.eval(pts)
+            phi_o, E_o = orc.evaluate(g, sig, pts)
+            assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E))
+            assert np.max(np.abs(phi - phi_o) / np.abs(phi_o)) < 1e-12
+            assert np.all(E[1] == 0.0)              # principal value of the normal field on the surface
+
+
+# ---------------------------------------------------------------------------------------------
+# a3 / a7 on mixed random elements (all kinds, dielectric rows, periodic copies)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("math", [1, 0])
+def test_assembly_and_eval_random_mixed(nb, orc, math):
+    nb.set_option(0, math)
+    pr = W.random_elements(333, seed=5, m_points=3001, dielectric_fraction=0.3)     # ragged tails: 333, 3001
+    pr.img_shift = W.image_shifts(1, pitch_mm=9.0)
+    g = orc.Geometry(pr)
+    nb.assemble_problem(pr)
+    K, Ko = nb.get_matrix(), orc.assemble(g)
+    rowmax = np.abs(Ko).max(axis=1, keepdims=True)
+    assert np.max(np.abs(K - Ko) / rowmax) <= TOL_K
+    off = ~np.eye(pr.n, dtype=bool)                      # entry-wise too, where the entry is not a cancelled sum
+    big = off & (np.abs(Ko) > 1e-3 * rowmax)
+    assert np.max(np.abs(K - Ko)[big] / np.abs(Ko)[big]) <= TOL_K
+    sig = np.linspace(1e-6, 2e-6, pr.n)
+    nb.set_sigma(sig)
+    phi, E = nb.eval(pr.points)
+    phi_o, E_o = orc.evaluate(g, sig, pr.points)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "random mixed")
+
+
+def test_explicit_collocation_points(nb, orc):
+    pr = W.random_elements(40, seed=8, kinds=(W.RECT, W.TRI))
+    col = pr.centroids() + 1e-5 * pr.normals()
+    g = orc.Geometry(pr, colloc=col)
+    nb.assemble_problem(pr, colloc=col)
+    K, Ko = nb.get_matrix(), orc.assemble(g)
+    assert np.max(np.abs(K - Ko) / np.abs(Ko).max(axis=1, keepdims=True)) <= TOL_K
+
+
+# ---------------------------------------------------------------------------------------------
+# a3 + a5 + a6 + a7: whole pipeline, BASELINE configs
+# ---------------------------------------------------------------------------------------------
+def _pipeline(nb, orc, pr, pts=None, orc_mode="ld"):
+    g = orc.Geometry(pr)
+    Ko = orc.assemble(g, mode=orc_mode)
+    bo = orc.rhs(g, pr.charge_pos, pr.charge_q, mode=orc_mode)
+    so = orc.solve(Ko, bo, mode=orc_mode)
+    nb.assemble_problem(pr)
+    if pr.charge_q is not None:
+        nb.add_space_charge(pr.charge_pos, pr.charge_q)
+    K = nb.get_matrix()
+    s = nb.solve()
+    assert np.max(np.abs(K - Ko) / np.abs(Ko).max(axis=1, keepdims=True)) <= TOL_K
+    assert np.max(np.abs(s - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    b = nb.get_rhs()
+    res = np.max(np.abs(K @ s - b)) / (np.abs(K).sum(axis=1).max() * np.abs(s).max())
+    assert res <= 1e-13
+    if pts is not None:
+        phi, E = nb.eval(pts)
+        phi_o, E_o = orc.evaluate(g, so, pts, pr.charge_pos, pr.charge_q, mode=orc_mode)
+        check_field(phi, E, phi_o, E_o, TOL_FAR, pr.name)
+    return g, s, so
+
+
+def test_c0_plate(nb, orc):
+    pr = W.plate()
+    g, s, so = _pipeline(nb, orc, pr, pr.points)
+    S = s.reshape(16, 16)
+    assert np.max(np.abs(S - S.T)) < 1e-12 * S.max() and np.max(np.abs(S - S[::-1, ::-1])) < 1e-12 * S.max()
+    assert S.max() == pytest.approx(S[0, 0], rel=1e-12) and np.all(np.diff(S[8, 8:]) > 0)      # edge peaking
+    # on-axis field against brute-force quadrature of the solved piecewise-constant sigma
+    x, w = np.polynomial.legendre.leggauss(24)
+    p = pr.meta["side"] / 16
+    for h in (1e-3, 5e-3, 1e-2):
+        phi_q, ez_q = 0.0, 0.0
+        for j in range(pr.n):
+            cx, cy = pr.v0[0, j] + p / 2, pr.v0[1, j] + p / 2
+            X, Y = np.meshgrid(cx + x * p / 2, cy + x * p / 2, indexing="ij")
+            Wt = np.outer(w, w) * (p / 2) ** 2
+            r = np.sqrt(X ** 2 + Y ** 2 + h * h)
+            phi_q += s[j] * np.sum(Wt / r)
+            ez_q += s[j] * np.sum(Wt * h / r ** 3)
+        phi, E = nb.eval(np.array([[0.0], [0.0], [h]]))
+        assert abs(phi[0] - orc.K_COULOMB * phi_q) < 1e-9 * abs(phi[0])
+        assert abs(E[2, 0] - orc.K_COULOMB * ez_q) < 1e-8 * abs(E[2, 0])
+
+
+def test_c1_cube_reduced_and_capacitance_sequence(nb, orc):
+    caps = []
+    for ns in (8, 16, 24):
+        pr = W.cube(n_side=ns, m_points=2000)
+        if ns == 8:
+            _pipeline(nb, orc, pr, pr.points)
+        nb.assemble_problem(pr)
+        s = nb.solve()
+        area = np.linalg.norm(np.cross(pr.e1.T, pr.e2.T), axis=1)
+        caps.append(np.sum(s * area) / (4 * np.pi * orc.EPS0 * pr.meta["side"]))
+    assert caps[0] < caps[1] < caps[2] < 0.6608           # converges to 0.66078 from below
+    assert abs(caps[1] - 0.6589284) < 2e-7 and abs(caps[2] - 0.6596472) < 2e-7
+
+
+def test_c1_cube_full_size(nb, orc):
+    """BASELINE configs[1] in the launch configuration bench.py times: 6144 panels, 1e5 points.
+    sigma against the (fp64, OpenMP) oracle LU; Phi/E on sampled points; properties at every point."""
+    import torch
+    pr = W.cube()
+    g = orc.Geometry(pr)
+    nb.assemble_problem(pr)
+    K = nb.get_matrix()
+    rs = np.random.RandomState(1)
+    rows, cols = rs.randint(0, pr.n, 20000), rs.randint(0, pr.n, 20000)
+    Ks = orc.matrix_entries(g, rows, cols)
+    assert np.max(np.abs(K[rows, cols] - Ks) / np.abs(Ks)) <= TOL_K
+    s = nb.solve()
+    b = nb.get_rhs()
+    assert np.max(np.abs(K @ s - b)) / (np.abs(K).sum(axis=1).max() * np.abs(s).max()) <= 1e-13
+    so = orc.solve(orc.assemble(g, mode="f64"), orc.rhs(g), mode="f64")
+    assert np.max(np.abs(s - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    area = np.linalg.norm(np.cross(pr.e1.T, pr.e2.T), axis=1)
+    assert abs(np.sum(s * area) / (4 * np.pi * orc.EPS0 * pr.meta["side"]) - 0.6599709) < 2e-7
+    pts = torch.from_numpy(pr.points).cuda()
+    phi, E = nb.eval(pts)
+    phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    idx = rs.choice(pr.points.shape[1], 300, replace=False)
+    phi_o, E_o = orc.evaluate(g, so, pr.points[:, idx])
+    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C1 sampled")
+    inside = np.all(np.abs(pr.points) < 0.0045, axis=0)     # inside the conductor: Phi = 1 V, E = 0
+    assert inside.sum() > 1000
+    assert np.max(np.abs(phi[inside] - 1.0)) < 2e-3
+    assert np.all(phi[~inside] < 1.0 + 1e-6) and np.all(phi > 0)
+
+
+def test_c2_thgem_reduced(nb, orc):
+    """Config-2 geometry at pitch divisor 20 (N ~ 2400: rectangles + right triangles, Dirichlet and
+    dielectric rows): full sigma parity; the 8^3 grid spans the cell."""
+    pr = W.thgem(d=20, n_plane=16, n_grid=8)
+    assert np.any(pr.kind == W.TRI) and np.any(pr.bc_kind == W.DIELECTRIC)
+    _pipeline(nb, orc, pr, pr.points, orc_mode="f64")
+
+
+def test_c3_double_thgem_reduced_with_images(nb, orc):
+    pr = W.double_thgem(d=10, n_plane=10, m_points=500)
+    assert pr.n_img == 25
+    _pipeline(nb, orc, pr, pr.points, orc_mode="f64")
+
+
+def test_c2_thgem_full_size_sampled(nb, orc):
+    """BASELINE configs[2] at full size (N = 19400, 100^3 grid): sampled matrix entries, residual of the
+    GPU sigma against ORACLE-computed rows, sampled grid nodes; mirror symmetry of the whole map."""
+    import torch
+    pr = W.thgem()
+    g = orc.Geometry(pr)
+    nb.assemble_problem(pr)
+    s = nb.solve()
+    rs = np.random.RandomState(2)
+    rows = rs.choice(pr.n, 48, replace=False)
+    R, Cc = np.repeat(rows, pr.n), np.tile(np.arange(pr.n), rows.size)
+    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)
+    b = orc.rhs(g, mode="f64")[rows]
+    res = np.abs(Krows @ s - b) / (np.abs(Krows).sum(axis=1) * np.abs(s).max())
+    assert res.max() <= 1e-12
+    pts = torch.from_numpy(pr.points).cuda()
+    phi, E = nb.eval(pts)
+    phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    idx = rs.choice(pr.points.shape[1], 64, replace=False)
+    phi_o, E_o = orc.evaluate(g, s, pr.points[:, idx], mode="ld")
+    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C2 sampled")
+    # the cell is mirror symmetric in x and in y: Phi(x,y,z) = Phi(-x,y,z) = Phi(x,-y,z), E_x odd in x
+    G = phi.reshape(100, 100, 100)                          # [z, y, x]
+    scale = np.abs(G).max()
+    assert np.max(np.abs(G - G[:, :, ::-1])) < 1e-9 * scale and np.max(np.abs(G - G[:, ::-1, :])) < 1e-9 * scale
+    Ex = E[0].reshape(100, 100, 100)
+    assert np.max(np.abs(Ex + Ex[:, :, ::-1])) < 1e-9 * np.abs(E).max()
+    assert phi.min() > -2000.0 - 1e-6 and phi.max() < 1e-6  # maximum principle between the electrodes
+
+
+# ---------------------------------------------------------------------------------------------
+# a4 / a8 / a9: space charge, RHS, re-solve on resident factors, push
+# ---------------------------------------------------------------------------------------------
+def test_space_charge_direct_sum(nb, orc):
+    pr = W.plate()
+    rs = np.random.RandomState(7)
+    q = 4097                                                # ragged against the 256-charge tile
+    pos = rs.normal(size=(3, q)) * 2e-3
+    ch = rs.choice([-1.0, 1.0], size=q) * W.Q_E
+    nb.assemble_problem(pr)
+    nb.set_sigma(np.zeros(pr.n))
+    nb.add_space_charge(pos, ch)
+    pts = np.concatenate([rs.normal(size=(3, 1000)) * 3e-3, pos[:, :50]], axis=1)      # incl. points ON charges
+    phi, E = nb.eval(pts)
+    phi_o, E_o = orc.point_charges(pts, pos, ch)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "point charges")
+    # append instead of replace
+    nb.add_space_charge(pos[:, :100], ch[:100], replace=False)
+    phi2, _ = nb.eval(pts)
+    phi_o2, _ = orc.point_charges(pts, np.concatenate([pos, pos[:, :100]], axis=1), np.concatenate([ch, ch[:100]]))
+    assert rel_err(phi2, phi_o2).max() <= TOL_FAR
+    nb.add_space_charge(None, None, replace=True)           # q = 0 clears
+    phi3, E3 = nb.eval(pts)
+    assert np.all(phi3 == 0.0) and np.all(E3 == 0.0)
+
+
+def test_rhs_and_resolve_with_space_charge(nb, orc):
+    pr = W.thgem(d=10, n_plane=8, n_grid=4)
+    rs = np.random.RandomState(3)
+    pr.charge_pos = rs.normal(size=(3, 3000)) * 1e-4
+    pr.charge_q = np.full(3000, W.Q_E * 1e4)
+    g, s, so = _pipeline(nb, orc, pr, pr.points, orc_mode="ld")
+    b = nb.get_rhs()
+    bo = orc.rhs(g, pr.charge_pos, pr.charge_q)
+    assert np.max(np.abs(b - bo) / np.maximum(np.abs(bo), 1e-6 * np.abs(bo).max())) <= TOL_FAR
+    # re-solve on the resident factors with moved charges (S13)
+    pos2 = pr.charge_pos + 2e-5
+    nb.add_space_charge(pos2, pr.charge_q, replace=True)
+    s2 = nb.solve()
+    so2 = orc.solve(orc.assemble(g), orc.rhs(g, pos2, pr.charge_q))
+    assert np.max(np.abs(s2 - so2)) <= TOL_SIGMA * np.max(np.abs(so2))
+    assert np.max(np.abs(s2 - s)) > 1e-6 * np.max(np.abs(s))                         # it really changed
+
+
+def test_c4_dynamic_loop_reduced(nb, orc):
+    """BASELINE configs[4] loop (eval E at the charges -> push -> RHS -> re-solve on resident LU) on the
+    reduced C3 geometry with 2000 charges, 3 steps, against the same loop written with the oracle."""
+    import torch
+    pr = W.space_charge(W.double_thgem(d=10, n_plane=10, m_points=0), q_count=2000)
+    pr.charge_q = pr.charge_q * 1e5                          # make the charges matter at this size
+    mu_dt = pr.meta["mu"] * pr.meta["dt"] * 1e3
+    g = orc.Geometry(pr)
+    lu = orc.LU(orc.assemble(g, mode="f64"), mode="f64")
+    pos_o = pr.charge_pos.copy()
+    nb.assemble_problem(pr)
+    pos = torch.from_numpy(pr.charge_pos.copy()).cuda()
+    ch = torch.from_numpy(pr.charge_q).cuda()
+    nb.add_space_charge(pos, ch)
+    nb.solve_resident()
+    so = lu.solve(orc.rhs(g, pos_o, pr.charge_q))
+    for step in range(3):
+        _, E = nb.eval(pos, want_phi=False)
+        _, E_o = orc.evaluate(g, so, pos_o, pos_o, pr.charge_q)
+        assert vec_rel_err(E.cpu().numpy(), E_o).max() <= 1e-8, step
+        nb.push(pos, E, mu_dt)
+        pos_o = orc.push(pos_o, E_o, mu_dt, 1.0)
+        nb.add_space_charge(pos, ch, replace=True)
+        s = nb.solve()
+        so = lu.solve(orc.rhs(g, pos_o, pr.charge_q))
+        assert np.max(np.abs(pos.cpu().numpy() - pos_o)) <= 1e-12 * np.max(np.abs(pos_o))
+        assert np.max(np.abs(s - so)) <= TOL_SIGMA * np.max(np.abs(so)), step
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases and error behaviour of the ABI
+# ---------------------------------------------------------------------------------------------
+def test_edge_cases_and_errors(nb, P, orc):
+    with pytest.raises(P.NebError) as e:
+        nb.solve()
+    assert e.value.status == 3                               # NEB_ESTATE
+    pr = W.plate(n_side=1)                                   # a single element
+    nb.assemble_problem(pr)
+    with pytest.raises(P.NebError):
+        nb.eval(np.zeros((3, 1)))                            # no sigma yet
+    s = nb.solve()
+    a = pr.meta["side"]
+    assert abs(s[0] - 1.0 / (orc.K_COULOMB * 4 * a * np.log(1 + np.sqrt(2)))) < 1e-13 * s[0]   # closed form
+    phi, E = nb.eval(np.zeros((3, 0)))                       # empty point set
+    assert phi.shape == (0,) and E.shape == (3, 0)
+    with pytest.raises(P.NebError) as e:
+        nb.get_matrix()                                      # factors have overwritten it
+    assert e.value.status == 3
+    bad = W.plate(n_side=2)
+    bad.kind[1] = 7
+    with pytest.raises(P.NebError) as e:
+        nb.assemble_problem(bad)
+    assert e.value.status == 1                               # NEB_EINVAL
+    bad = W.plate(n_side=2)
+    bad.e1[:, 2] = 0.0
+    with pytest.raises(P.NebError) as e:
+        nb.assemble_problem(bad)
+    assert e.value.status == 1
+    dup = W.plate(n_side=2)                                  # two coincident panels: identical rows
+    dup.v0[:, 1] = dup.v0[:, 0]
+    nb.assemble_problem(dup)
+    with pytest.raises(P.NebError) as e:
+        nb.solve()
+    assert e.value.status == 4                               # NEB_ESINGULAR
+    shifts = W.image_shifts(1)[:, 1:]                        # image set without the zero shift
+    ok = W.plate(n_side=2)
+    ok.img_shift = shifts
+    with pytest.raises(P.NebError) as e:
+        nb.assemble_problem(ok)
+    assert e.value.status == 1
+
+
+def test_host_and_device_pointers_agree(nb):
+    import torch
+    pr = W.cube(n_side=4, m_points=777)
+    nb.assemble_problem(pr)
+    s_host = nb.solve()
+    s_dev = torch.empty(pr.n, dtype=torch.float64, device="cuda")
+    nb.solve(out=s_dev)
+    assert np.array_equal(s_dev.cpu().numpy(), s_host)
+    phi_h, E_h = nb.eval(pr.points)
+    phi_d, E_d = nb.eval(torch.from_numpy(pr.points).cuda())
+    assert np.array_equal(phi_d.cpu().numpy(), phi_h) and np.array_equal(E_d.cpu().numpy(), E_h)
+    pinned = torch.from_numpy(pr.points).pin_memory()
+    phi_p, _ = nb.eval(pinned)
+    assert np.array_equal(phi_p.numpy(), phi_h)
+    # run to run reproducibility: fixed-order partial sums, no fp64 atomics
+    phi_2, E_2 = nb.eval(pr.points)
+    assert np.array_equal(phi_2, phi_h) and np.array_equal(E_2, E_h)
+
+
+def test_fp64_peaks_and_stats(nb):
+    dfma, dmma = nb.fp64_peak(0), nb.fp64_peak(1)
+    assert 20.0 < dfma < 60.0 and 20.0 < dmma < 80.0         # B200: ~37 TFLOP/s both
+    nb.set_option(2, 1)
+    nb.reset_stats()
+    pr = W.plate()
+    nb.assemble_problem(pr)
+    nb.solve()
+    nb.eval(pr.points)
+    st = nb.stage_ms()
+    assert st["assemble"][1] >= 1 and st["lu"][1] >= 4 and st["eval"][1] >= 2 and st["eval"][0] > 0
+    assert nb.launch_count() > 10
