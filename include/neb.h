@@ -62,9 +62,10 @@ enum {
   NEB_STAGE_LU_GEMM = 4,  /* a5 trailing update (DMMA) only, subset of LU      */
   NEB_STAGE_RHS = 5,      /* a4                                                */
   NEB_STAGE_TRISOLVE = 6, /* a6                                                */
-  NEB_STAGE_EVAL = 7,     /* a7 fused element kernel                           */
-  NEB_STAGE_CHARGES = 8,  /* a8 point-charge direct sum                        */
-  NEB_STAGE_COUNT = 9
+  NEB_STAGE_EVAL = 7,     /* a7 fused element kernel alone                     */
+  NEB_STAGE_CHARGES = 8,  /* a8 point-charge direct sum kernel                 */
+  NEB_STAGE_REDUCE = 9,   /* fixed-order sum of the per-chunk partials of a7/a8 */
+  NEB_STAGE_COUNT = 10
 };
 
 /* Creates a context on `device`.  `cuda_stream` is a cudaStream_t (e.g. torch's current stream),

@@ -10,7 +10,7 @@ from . import build as _build
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
 NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE = 0, 1, 2
-STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges"]
+STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -331,28 +331,34 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1..65000 and kind, v0, e1, e2, bc_kind non-NULL");
   if (n_img < 0 || n_img > 32 || (n_img > 0 && !img_shift)) return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= 32");
   NEB_CUDA(c, cudaSetDevice(c->device));
-  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
-  free_problem(c);
-  c->n = n;
-  c->npad = (n + kPad - 1) / kPad * kPad;
-  c->stride = c->npad;
+  const bool reuse = (c->n == n && c->d_K != nullptr);   // same size as the last problem: keep the buffers
+  if (!reuse) {
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    free_problem(c);
+    c->n = n;
+    c->npad = (n + kPad - 1) / kPad * kPad;
+    c->stride = c->npad;
+  }
+  c->assembled = c->factored = c->have_sigma = false;
   const int64_t st = c->stride, npad = c->npad;
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_perm, sizeof(int32_t) * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_colloc, sizeof(double) * 3 * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_normal, sizeof(double) * 3 * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_kind, sizeof(int32_t) * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_value, sizeof(double) * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_diag, sizeof(double) * st));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_rscale, sizeof(double) * npad));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_ipiv, sizeof(int32_t) * npad));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_rowperm, sizeof(int32_t) * npad));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_b, sizeof(double) * npad));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * npad));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
+  if (!reuse) {
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_perm, sizeof(int32_t) * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_colloc, sizeof(double) * 3 * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_normal, sizeof(double) * 3 * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_kind, sizeof(int32_t) * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_bc_value, sizeof(double) * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_diag, sizeof(double) * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_rscale, sizeof(double) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_ipiv, sizeof(int32_t) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_rowperm, sizeof(int32_t) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_b, sizeof(double) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * 32));
+  }
   c->n_img = n_img > 0 ? n_img : 1;
-  NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * c->n_img));
   NEB_CUDA(c, cudaMemsetAsync(c->d_img, 0, sizeof(double) * 3 * c->n_img, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_rec, 0, sizeof(double) * kRec * st, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int32_t), c->stream));

@@ -321,7 +321,7 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
     NEB_CUDA(c, cudaGetLastError());
   }
   {
-    StageTimer t(c, use_elements ? NEB_STAGE_EVAL : NEB_STAGE_CHARGES);
+    StageTimer t(c, NEB_STAGE_REDUCE);
     reduce_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(partial, se, sq, m, d_phi, d_E);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
