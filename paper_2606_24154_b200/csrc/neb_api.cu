@@ -319,6 +319,7 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
       if (value != 64) return fail(c, NEB_EINVAL, "this build supports LU panel width 64 only");
       return NEB_OK;
     case NEB_OPT_PROFILE: c->profile = value ? 1 : 0; return NEB_OK;
+    case NEB_OPT_LU_PANEL: c->panel_mode = value ? 1 : 0; return NEB_OK;
     default: return fail(c, NEB_EINVAL, "unknown option");
   }
 }

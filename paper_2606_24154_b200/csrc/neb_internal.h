@@ -38,6 +38,7 @@ struct neb_ctx {
   int math_fast = 1;
   int lu_nb = 64;
   int profile = 0;
+  int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
 
   // geometry
   int64_t n = 0, npad = 0, stride = 0;
@@ -116,6 +117,10 @@ neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
 neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-scaled)
 neb_status lu_solve(neb_ctx* c);          // a6: d_x <- solution of (scaled) system for RHS d_b
 size_t lu_panel_ws_bytes(int num_sms);
+
+// neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
+int64_t panel_cluster_max_rows(neb_ctx* c);
+neb_status panel_cluster_launch(neb_ctx* c, int64_t k);
 
 // neb_peaks.cu ------------------------------------------------------------------------------------
 neb_status fp64_peak(neb_ctx* c, int kind, double* tflops);

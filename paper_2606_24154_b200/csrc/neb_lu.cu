@@ -396,6 +396,7 @@ neb_status lu_factor(neb_ctx* c) {
     attr_set = true;
   }
   PanelWs* ws = (PanelWs*)c->d_panel_ws;
+  const int64_t cluster_rows = panel_cluster_max_rows(c);
   for (int64_t k = 0; k < npad; k += NB) {
     const int64_t mrows = npad - k;
     // rows per CTA: multiple of 32, at most 200 KB of shared memory (390 rows -> 384)
@@ -406,8 +407,10 @@ neb_status lu_factor(neb_ctx* c) {
     size_t smem = (size_t)mc * NB * sizeof(double);
     if (smem > 200 * 1024) return fail(c, NEB_ENOMEM, "LU panel slab exceeds shared memory: n too large for this build");
     G = (int)((mrows + mc - 1) / mc);
-    NEB_CUDA(c, cudaMemsetAsync(&ws->counter, 0, sizeof(unsigned int), c->stream));
-    {
+    if (c->panel_mode == 0 && mrows <= cluster_rows) {
+      NEB_TRY(panel_cluster_launch(c, k));
+    } else {
+      NEB_CUDA(c, cudaMemsetAsync(&ws->counter, 0, sizeof(unsigned int), c->stream));
       double* A = c->d_K;
       int64_t ld_ = ld, npad_ = npad, k_ = k;
       int mc_ = mc;
