@@ -248,12 +248,12 @@ __global__ void push_kernel(int64_t n3, double* __restrict__ pos, const double* 
 
 static void free_problem(neb_ctx* c) {
   void* ptrs[] = {c->d_rec, c->d_perm, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_img,
-                  c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma};
+                  c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma, c->d_dinv};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   c->d_rec = nullptr; c->d_perm = nullptr; c->d_colloc = nullptr; c->d_normal = nullptr; c->d_bc_kind = nullptr;
   c->d_bc_value = nullptr; c->d_diag = nullptr; c->d_img = nullptr; c->d_K = nullptr; c->d_rscale = nullptr;
-  c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr;
+  c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr; c->d_dinv = nullptr;
   c->assembled = c->factored = c->have_sigma = false;
   c->n = c->npad = c->stride = 0;
 }
@@ -354,7 +354,8 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaMalloc((void**)&c->d_ipiv, sizeof(int32_t) * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_rowperm, sizeof(int32_t) * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_b, sizeof(double) * npad));
-    NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * 2 * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_dinv, sizeof(double) * 2 * (npad / 64) * 4096));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * 32));

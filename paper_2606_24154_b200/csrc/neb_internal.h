@@ -59,7 +59,8 @@ struct neb_ctx {
   int32_t* d_ipiv = nullptr;      // npad (0-based absolute row)
   int32_t* d_rowperm = nullptr;   // npad: composed row permutation of the factorisation
   double* d_b = nullptr;          // npad, unscaled RHS (sorted order)
-  double* d_x = nullptr;          // npad work vector
+  double* d_x = nullptr;          // 2 * npad: running right-hand side + solved blocks
+  double* d_dinv = nullptr;       // inverses of the 64x64 diagonal blocks of L and U: 2 * (npad/64) * 4096
   double* d_sigma = nullptr;      // n, caller order
   void* d_panel_ws = nullptr;     // LU panel exchange buffers
   bool assembled = false, factored = false, have_sigma = false;

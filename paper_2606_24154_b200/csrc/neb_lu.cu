@@ -190,25 +190,40 @@ __global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t npad, i
   }
 }
 
-// U12 = L11^-1 A12: rows [k, k+NB), columns [k+NB, npad).  CTA = 256 threads on a slab of 64 columns held
-// in shared memory (sB[c][i], odd leading dimension: conflict-free), right-looking substitution.
+// U12 = L11^-1 A12: rows [k, k+NB), columns [k+NB, npad).  CTA = 256 threads on a slab of 64 columns.
+// Thread (c = tid & 63, q = tid >> 6) keeps rows q, q+4, ..., q+60 of column c in registers; at step j the
+// owner of row j broadcasts x_j through shared memory (double-buffered: one barrier per step) and every
+// thread updates its rows below j with L11 read from shared memory (warp-uniform address: broadcast).
 constexpr int TRSM_THREADS = 256;
-constexpr size_t TRSM_SMEM = (size_t)2 * NB * (NB + 1) * sizeof(double);
+constexpr size_t TRSM_SMEM = (size_t)(NB * (NB + 1) + 2 * NB) * sizeof(double);
 __global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k) {
   extern __shared__ double s_trsm[];
-  double(*sL)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm);                    // sL[i][j] = L11[i][j]
-  double(*sB)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm + NB * (NB + 1));     // sB[c][i]
-  const int tid = threadIdx.x, r = tid & (NB - 1), q = tid >> 6;     // q = 0..3
+  double(*sL)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm);     // sL[i][j] = L11[i][j]
+  double* sX = s_trsm + NB * (NB + 1);                                    // sX[(j & 1) * NB + c]
+  const int tid = threadIdx.x, c = tid & (NB - 1), q = tid >> 6;         // q = 0..3
   const int64_t c0 = k + NB + (int64_t)blockIdx.x * NB;
-  for (int j = q; j < NB; j += 4) sL[r][j] = A[(k + r) + (k + j) * ld];
-  for (int c = q; c < NB; c += 4) sB[c][r] = A[(k + r) + (c0 + c) * ld];
+  for (int j = q; j < NB; j += 4) sL[c][j] = A[(k + c) + (k + j) * ld];
+  double x[NB / 4];
+  // column c of the slab: rows q + 4t.  Loaded through shared memory would be coalesced; direct loads hit
+  // whole 32-byte sectors across the 4 row groups of a column, which the L2 absorbs.
+#pragma unroll
+  for (int t = 0; t < NB / 4; ++t) x[t] = A[(k + q + 4 * t) + (c0 + c) * ld];
   __syncthreads();
+#pragma unroll
   for (int j = 0; j < NB - 1; ++j) {
-    const double xj = sB[r][j];                   // thread (c = r, row group q)
-    for (int i = j + 1 + q; i < NB; i += 4) sB[r][i] = fma(-sL[i][j], xj, sB[r][i]);
+    if (q == (j & 3)) sX[(j & 1) * NB + c] = x[j >> 2];
     __syncthreads();
+    const double xj = sX[(j & 1) * NB + c];
+#pragma unroll
+    for (int t = 0; t < NB / 4; ++t) {
+      if (4 * t + 3 > j) {                       // some row of this group may lie below j (compile-time prune)
+        const int i = q + 4 * t;
+        if (i > j) x[t] = fma(-sL[i][j], xj, x[t]);
+      }
+    }
   }
-  for (int c = q; c < NB; c += 4) A[(k + r) + (c0 + c) * ld] = sB[c][r];
+#pragma unroll
+  for (int t = 0; t < NB / 4; ++t) A[(k + q + 4 * t) + (c0 + c) * ld] = x[t];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -309,14 +324,28 @@ __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restric
 // a6: triangular solves on the resident factors
 // ------------------------------------------------------------------------------------------------
 // Composes the row exchanges into one permutation: rowperm[i] = original row that ends in position i.
-__global__ void compose_perm_kernel(const int32_t* __restrict__ ipiv, int32_t* __restrict__ rowperm, int npad) {
-  extern __shared__ int s_perm[];
+// The exchanges are sequential by nature, but few (the matrix is close to diagonally dominant): the
+// positions that really exchange are marked in parallel in a bit mask, one thread walks the set bits.
+__global__ void __launch_bounds__(1024) compose_perm_kernel(const int32_t* __restrict__ ipiv, int32_t* __restrict__ rowperm, int npad) {
+  extern __shared__ int s_perm[];            // npad ints, then (npad+31)/32 mask words
+  unsigned* s_mask = reinterpret_cast<unsigned*>(s_perm + npad);
+  const int nwords = (npad + 31) / 32;
   for (int i = threadIdx.x; i < npad; i += blockDim.x) s_perm[i] = i;
+  for (int w = threadIdx.x >> 5; w < nwords; w += blockDim.x >> 5) {
+    int i = w * 32 + (threadIdx.x & 31);
+    unsigned m = __ballot_sync(0xffffffffu, i < npad && ipiv[i] != i);
+    if ((threadIdx.x & 31) == 0) s_mask[w] = m;
+  }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int i = 0; i < npad; ++i) {
-      int p = ipiv[i];
-      if (p != i) { int tmp = s_perm[i]; s_perm[i] = s_perm[p]; s_perm[p] = tmp; }
+    for (int w = 0; w < nwords; ++w) {
+      unsigned m = s_mask[w];
+      while (m) {
+        int i = w * 32 + __ffs(m) - 1;
+        m &= m - 1;
+        int p = ipiv[i];
+        int tmp = s_perm[i]; s_perm[i] = s_perm[p]; s_perm[p] = tmp;
+      }
     }
   }
   __syncthreads();
@@ -339,47 +368,86 @@ __global__ void permute_scale_kernel(const double* __restrict__ b, const double*
   if (i < npad) { int p = rowperm[i]; x[i] = b[p] * rscale[p]; }
 }
 
-// Diagonal block solve, one CTA of 64 threads.  lower: unit lower triangular; else upper.
-__global__ void __launch_bounds__(NB) diag_solve_kernel(const double* __restrict__ A, int64_t ld, int64_t kb, double* x, int lower) {
-  __shared__ double sT[NB][NB + 1];
-  __shared__ double sx[NB];
-  const int tid = threadIdx.x;
-  for (int j = 0; j < NB; ++j) sT[tid][j] = A[(kb + tid) + (kb + j) * ld];
-  sx[tid] = x[kb + tid];
+// Inverses of the 64x64 diagonal blocks of L (unit lower) and U (upper), once per factorisation, so that a
+// solve step is a matrix-vector product instead of a 64-step substitution.  grid = (nblocks, 2), 64 threads;
+// thread c computes column c of the inverse by substitution.  dinv[(which * nblk + blk) * 4096 + i + 64 j].
+__global__ void __launch_bounds__(NB) diag_inv_kernel(const double* __restrict__ A, int64_t ld, double* __restrict__ dinv, int nblk) {
+  extern __shared__ double s_dinv[];
+  double(*sT)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_dinv);                     // sT[i][j]
+  double(*sXc)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_dinv + NB * (NB + 1));    // sXc[k][c]
+  const int c = threadIdx.x, blk = blockIdx.x, upper = blockIdx.y;
+  const int64_t kb = (int64_t)blk * NB;
+  for (int j = 0; j < NB; ++j) sT[c][j] = A[(kb + c) + (kb + j) * ld];
   __syncthreads();
-  if (lower) {
-    for (int j = 0; j < NB - 1; ++j) {
-      if (tid > j) sx[tid] = fma(-sT[tid][j], sx[j], sx[tid]);
-      __syncthreads();
+  if (!upper) {
+    for (int i = 0; i < NB; ++i) {
+      double acc = (i == c) ? 1.0 : 0.0;
+      for (int kk = c; kk < i; ++kk) acc = fma(-sT[i][kk], sXc[kk][c], acc);
+      sXc[i][c] = (i < c) ? 0.0 : acc;
     }
   } else {
-    for (int j = NB - 1; j >= 0; --j) {
-      if (tid == j) sx[j] = sx[j] / sT[j][j];
-      __syncthreads();
-      if (tid < j) sx[tid] = fma(-sT[tid][j], sx[j], sx[tid]);
-      __syncthreads();
+    for (int i = NB - 1; i >= 0; --i) {
+      double acc = (i == c) ? 1.0 : 0.0;
+      for (int kk = i + 1; kk <= c; ++kk) acc = fma(-sT[i][kk], sXc[kk][c], acc);
+      sXc[i][c] = (i > c) ? 0.0 : acc / sT[i][i];
     }
   }
-  x[kb + tid] = sx[tid];
+  __syncthreads();
+  double* out = dinv + ((int64_t)upper * nblk + blk) * (NB * NB);
+  for (int j = 0; j < NB; ++j) out[c + NB * j] = sXc[c][j];
 }
 
-// x[rows] -= A[rows, kb..kb+64) * x[kb..kb+64); rows = [r_lo, r_hi).  One thread per row.
-__global__ void gemv_update_kernel(const double* __restrict__ A, int64_t ld, int64_t kb, int64_t r_lo, int64_t r_hi, double* x) {
-  __shared__ double sx[NB];
-  if (threadIdx.x < NB) sx[threadIdx.x] = x[kb + threadIdx.x];
-  __syncthreads();
-  int64_t i = r_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= r_hi) return;
-  const double* a = A + i + kb * ld;
-  double acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;
+// One block step of a triangular solve, ONE launch: every CTA first forms x_B = Dinv_B * x[kb..kb+64)
+// (a 64x64 matrix-vector product, recomputed per CTA: 32 KB from L2) and then updates its 64 rows,
+// x[i] -= A[i, kb..kb+64) . x_B.  CTA 0 also stores x_B.  256 threads = 64 rows x 4 column groups of 16.
+// rows to update: [r_lo, r_hi); grid.x = ceil((r_hi - r_lo) / 64), at least 1.
+__global__ void __launch_bounds__(256) tri_step_kernel(const double* __restrict__ A, int64_t ld, const double* __restrict__ dinv_blk,
+                                                       int64_t kb, int64_t r_lo, int64_t r_hi, double* x) {
+  __shared__ double s_part[4][NB];
+  __shared__ double s_xb[NB];
+  const int tid = threadIdx.x, r = tid & (NB - 1), g = tid >> 6;
+  {
+    double acc = 0.0;
 #pragma unroll 4
-  for (int j = 0; j < NB; j += 4) {
-    acc0 = fma(a[(j + 0) * ld], sx[j + 0], acc0);
-    acc1 = fma(a[(j + 1) * ld], sx[j + 1], acc1);
-    acc2 = fma(a[(j + 2) * ld], sx[j + 2], acc2);
-    acc3 = fma(a[(j + 3) * ld], sx[j + 3], acc3);
+    for (int jj = 0; jj < 16; ++jj) {
+      const int j = g * 16 + jj;
+      acc = fma(dinv_blk[r + NB * j], x[kb + j], acc);
+    }
+    s_part[g][r] = acc;
   }
-  x[i] -= (acc0 + acc1) + (acc2 + acc3);
+  __syncthreads();
+  if (tid < NB) s_xb[tid] = (s_part[0][tid] + s_part[1][tid]) + (s_part[2][tid] + s_part[3][tid]);
+  __syncthreads();
+  const int64_t i = r_lo + (int64_t)blockIdx.x * NB + r;
+  double acc = 0.0;
+  if (i < r_hi) {
+    const double* a = A + i + (kb + g * 16) * ld;
+    double a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+#pragma unroll
+    for (int jj = 0; jj < 16; jj += 4) {
+      a0 = fma(a[(jj + 0) * ld], s_xb[g * 16 + jj + 0], a0);
+      a1 = fma(a[(jj + 1) * ld], s_xb[g * 16 + jj + 1], a1);
+      a2 = fma(a[(jj + 2) * ld], s_xb[g * 16 + jj + 2], a2);
+      a3 = fma(a[(jj + 3) * ld], s_xb[g * 16 + jj + 3], a3);
+    }
+    acc = (a0 + a1) + (a2 + a3);
+  }
+  __syncthreads();               // s_part is reused; everyone has read it
+  s_part[g][r] = acc;
+  __syncthreads();
+  if (tid < NB) {
+    const int64_t ii = r_lo + (int64_t)blockIdx.x * NB + tid;
+    if (ii < r_hi) x[ii] -= (s_part[0][tid] + s_part[1][tid]) + (s_part[2][tid] + s_part[3][tid]);
+  }
+  // the block's own solution: written last, by CTA 0 only; no CTA of this launch reads x[kb..kb+64) after
+  // its first barrier... but other CTAs may still be reading it: CTA 0 therefore writes to a staging slot
+  if (blockIdx.x == 0 && tid < NB) x[ld + kb + tid] = s_xb[tid];
+}
+
+// x[0..npad) <- staging copy x[npad..2 npad) (the solved blocks)
+__global__ void tri_finish_kernel(int64_t npad, double* x) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < npad) x[i] = x[npad + i];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -393,6 +461,7 @@ neb_status lu_factor(neb_ctx* c) {
     NEB_CUDA(c, cudaFuncSetAttribute(panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     NEB_CUDA(c, cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
     NEB_CUDA(c, cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM));
+    NEB_CUDA(c, cudaFuncSetAttribute(diag_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * NB * (NB + 1) * sizeof(double))));
     attr_set = true;
   }
   PanelWs* ws = (PanelWs*)c->d_panel_ws;
@@ -439,17 +508,22 @@ neb_status lu_factor(neb_ctx* c) {
     NEB_CUDA(c, cudaGetLastError());
   }
   // composed permutation for the solves
-  if ((size_t)npad * sizeof(int) <= 200 * 1024) {
+  if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
     static bool attr2 = false;
     if (!attr2) {
       NEB_CUDA(c, cudaFuncSetAttribute(compose_perm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
       attr2 = true;
     }
-    compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+    compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * sizeof(unsigned), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
   } else {
     compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
   }
   c->launches++;
+  {
+    const int nblk = (int)(npad / NB);
+    diag_inv_kernel<<<dim3(nblk, 2), NB, 2 * NB * (NB + 1) * sizeof(double), c->stream>>>(c->d_K, ld, c->d_dinv, nblk);
+    c->launches++;
+  }
   NEB_CUDA(c, cudaGetLastError());
   return NEB_OK;
 }
@@ -459,23 +533,23 @@ neb_status lu_solve(neb_ctx* c) {
   StageTimer tt(c, NEB_STAGE_TRISOLVE);
   permute_scale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(c->d_b, c->d_rscale, c->d_rowperm, npad, c->d_x);
   c->launches++;
+  // d_x holds two vectors: [0, npad) the running right-hand side, [npad, 2 npad) the solved blocks
+  const int nblk = (int)(npad / NB);
   for (int64_t kb = 0; kb < npad; kb += NB) {          // forward: L y = P b
-    diag_solve_kernel<<<1, NB, 0, c->stream>>>(c->d_K, ld, kb, c->d_x, 1);
+    const int64_t lo = kb + NB;
+    const unsigned grid = (unsigned)max((int64_t)1, (npad - lo + NB - 1) / NB);
+    tri_step_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, ld, c->d_dinv + (kb / NB) * (NB * NB), kb, lo, npad, c->d_x);
     c->launches++;
-    int64_t lo = kb + NB;
-    if (lo < npad) {
-      gemv_update_kernel<<<(unsigned)((npad - lo + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, kb, lo, npad, c->d_x);
-      c->launches++;
-    }
   }
+  tri_finish_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(npad, c->d_x);
+  c->launches++;
   for (int64_t kb = npad - NB; kb >= 0; kb -= NB) {    // backward: U x = y
-    diag_solve_kernel<<<1, NB, 0, c->stream>>>(c->d_K, ld, kb, c->d_x, 0);
+    const unsigned grid = (unsigned)max((int64_t)1, (kb + NB - 1) / NB);
+    tri_step_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, ld, c->d_dinv + ((int64_t)nblk + kb / NB) * (NB * NB), kb, 0, kb, c->d_x);
     c->launches++;
-    if (kb > 0) {
-      gemv_update_kernel<<<(unsigned)((kb + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, kb, 0, kb, c->d_x);
-      c->launches++;
-    }
   }
+  tri_finish_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(npad, c->d_x);
+  c->launches++;
   NEB_CUDA(c, cudaGetLastError());
   return NEB_OK;
 }
