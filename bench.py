@@ -122,6 +122,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2606_24154_b200 as P
+    from paper_2606_24154_b200 import parallel
     from workloads import configs as W
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -182,11 +183,7 @@ def main():
             e1.record()
         barrier()
         ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return parallel.max_over_ranks(ms, dev)
 
     for _ in range(args.warmup):
         step_resident()

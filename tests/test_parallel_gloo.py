@@ -1,0 +1,64 @@
+"""Host-side multi-rank logic on CPU: world_size 2, gloo (shard over points, no data-path
+collective; max-over-ranks timing; optional all-gather of the outputs)."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2606_24154_b200 import parallel
+
+
+def test_shard_bounds_tile_exactly():
+    for m in (0, 1, 7, 100000, 100001):
+        for world in (1, 2, 3, 8):
+            b = [parallel.shard_bounds(m, world, r) for r in range(world)]
+            assert b[0][0] == 0 and b[-1][1] == m
+            assert all(b[r][1] == b[r + 1][0] for r in range(world - 1))
+            sizes = [e - s for s, e in b]
+            assert max(sizes) - min(sizes) <= 1
+
+
+class _FakeNeb:
+    """Stands in for a solved context: 'evaluates' a known function of the points on the CPU."""
+
+    def eval(self, pts):
+        return pts[0] * 2.0 + pts[2], torch.stack([pts[0], pts[1] * 3.0, -pts[2]])
+
+
+def _worker(rank, world, port, m, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        g = torch.Generator().manual_seed(0)
+        pts = torch.rand((3, m), generator=g, dtype=torch.float64)          # same points on every rank
+        phi, E = parallel.eval_sharded(_FakeNeb(), pts, gather=True)
+        ok = torch.equal(phi, pts[0] * 2.0 + pts[2]) and torch.equal(E, torch.stack([pts[0], pts[1] * 3.0, -pts[2]]))
+        s, e = parallel.shard_bounds(m, world, rank)
+        phi_l, _ = parallel.eval_sharded(_FakeNeb(), pts, gather=False)
+        ok = ok and phi_l.shape[0] == e - s
+        t = parallel.max_over_ranks(10.0 + rank)
+        q.put((rank, bool(ok), t))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_gloo():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    world, m = 2, 1001                                   # odd: slabs differ by one
+    procs = [ctx.Process(target=_worker, args=(r, world, port, m, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [r[1] for r in res] == [True, True]
+    assert [r[2] for r in res] == [11.0, 11.0]           # max over ranks, identical everywhere
