@@ -22,7 +22,6 @@ import json
 import os
 import subprocess
 import sys
-import threading
 import time
 
 import numpy as np
@@ -33,27 +32,40 @@ sys.path.insert(0, ROOT)
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
 # algorithmic FP64 work of one (point, element copy) evaluation of (Phi', E') — hand count of the closed
-# forms in DESIGN.md §6 (FMA = 2 flop): rectangle 393, right triangle 327, wire 150, point charge 30
-FLOP_PER_PAIR = {"rect": 393.0, "tri": 327.0, "wire": 150.0, "charge": 30.0}
+# forms in DESIGN.md §6 (FMA = 2 flop): rectangle 361, right triangle 301, wire 144, point charge 30
+FLOP_PER_PAIR = {"rect": 361.0, "tri": 301.0, "wire": 144.0, "charge": 30.0}
 CONFIG = {"workload": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
           "n_elements": 6144, "m_points": 100000, "step": "assemble+solve(LU)+eval",
           "l2": "256 MiB buffer written between timed steps; matrix (302 MB) exceeds L2"}
 
 
-def _clock_sampler(stop, out):
-    q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+class ClockSampler:
+    """One long-running `nvidia-smi -lms 100` for the timed region (no per-sample process spawn)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
-    idx = os.environ.get("LOCAL_RANK", "0")
-    while not stop.is_set():
+
+    def __init__(self):
+        self.p = None
+
+    def start(self):
         try:
-            r = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", idx],
-                               capture_output=True, text=True, timeout=5)
-            f = [x.strip() for x in r.stdout.strip().split(",")]
-            if len(f) >= 6:
-                out.append(f)
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", os.environ.get("LOCAL_RANK", "0")], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
-            pass
-        stop.wait(0.1)
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return []
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        rows = [[x.strip() for x in line.split(",")] for line in out.strip().splitlines()]
+        return [r for r in rows if len(r) >= 6]
 
 
 def _clocks_summary(samples):
@@ -188,14 +200,12 @@ def main():
     for _ in range(args.warmup):
         step_resident()
     torch.cuda.synchronize()
-    samples, stop = [], threading.Event()
-    th = threading.Thread(target=_clock_sampler, args=(stop, samples), daemon=True)
-    th.start()
+    sampler = ClockSampler()
+    sampler.start()
     l0 = nb.launch_count()
     ms = timed(step_resident, args.steps)
     launches = nb.launch_count() - l0
-    stop.set()
-    th.join(timeout=3)
+    samples = sampler.stop()
 
     for _ in range(2):
         step_e2e()
