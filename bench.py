@@ -32,8 +32,8 @@ sys.path.insert(0, ROOT)
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
 # algorithmic FP64 work of one (point, element copy) evaluation of (Phi', E') — hand count of the closed
-# forms in DESIGN.md §6 (FMA = 2 flop): rectangle 361, right triangle 301, wire 144, point charge 30
-FLOP_PER_PAIR = {"rect": 361.0, "tri": 301.0, "wire": 144.0, "charge": 30.0}
+# forms in DESIGN.md §6 (FMA = 2 flop): rectangle 348, right triangle 291, wire 139, point charge 30
+FLOP_PER_PAIR = {"rect": 348.0, "tri": 291.0, "wire": 139.0, "charge": 30.0}
 CONFIG = {"workload": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
           "n_elements": 6144, "m_points": 100000, "step": "assemble+solve(LU)+eval",
           "l2": "256 MiB buffer written between timed steps; matrix (302 MB) exceeds L2"}

@@ -96,8 +96,11 @@ struct EvalSink {
   }
 };
 
+#ifndef NEB_EVAL_MINB
+#define NEB_EVAL_MINB 4
+#endif
 template <class M>
-__global__ void __launch_bounds__(kThreads) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img,
+__global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img,
                                                         const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                         double* __restrict__ partial) {
   __shared__ TileSmem sm;

@@ -31,15 +31,24 @@ struct Infl {
 // squared distance from P to the edge's line, L = lp - lm.  Three algebraically equal forms chosen by
 // the position of the foot so that nothing cancels; far away (Rm+Rp > 8L) 2 atanh(L/(Rm+Rp)) keeps
 // full RELATIVE accuracy of the small value (the far-field sums cancel by a factor r/L).
+// om >= 0 with the sign of Y, and 0 when Y == 0 (integer operations only)
+__device__ __forceinline__ double signed_or_zero(double om, double Y) {
+  const int hy = __double2hiint(Y), ly = __double2loint(Y);
+  const bool zero = (((hy & 0x7fffffff) | ly) == 0);
+  const int ho = (__double2hiint(om) & 0x7fffffff) | (hy & 0x80000000);
+  return zero ? 0.0 : __hiloint2double(ho, __double2loint(om));
+}
+
 template <class M>
 __device__ __forceinline__ double edge_log(double lm, double lp, double Rm, double Rp, double R0sq, double L) {
   double s = Rm + Rp;
   double pp = Rp + fabs(lp), qq = Rm + fabs(lm);
-  bool cA = lm >= 0.0, cB = lp <= 0.0;
+  // sign tests on the high word (integer pipe); a zero abscissa may fall in either case, all three forms agree there
+  bool cA = __double2hiint(lm) >= 0, cB = __double2hiint(lp) < 0;
   double N = cB ? qq : pp;
   N = (cA || cB) ? N : pp * qq;
   double D = cA ? qq : (cB ? pp : R0sq);
-  return M::log_ratio(N, D, s > 8.0 * L, L, s);
+  return M::log_ratio(N, D, M::kNeedsFar && s > 8.0 * L, L, s);
 }
 
 // Rectangle [0,a] x [0,b] in the local XZ plane; (X, Y, Z) local coordinates of P.
@@ -68,7 +77,7 @@ __device__ __forceinline__ void rect_local(double a, double b, double X, double 
   phi = fma(u2, F2, fma(-u1, F1, fma(w2, G2, fma(-w1, G1, -y * om))));
   fx = F2 - F1;
   fz = G2 - G1;
-  fy = (Y > 0.0) ? om : ((Y < 0.0) ? -om : 0.0);          // S5: principal value on the surface
+  fy = signed_or_zero(om, Y);                             // S5: principal value on the surface
 }
 
 // Right triangle (0,0), (a,0), (0,b) in the local XZ plane, ih = 1/sqrt(a^2+b^2).
@@ -93,7 +102,7 @@ __device__ __forceinline__ void tri_local(double a, double b, double ih, double 
   phi = fma(Z, fAB, fma(X, fCA, fma(P0, fBC, -y * om)));
   fx = fma(cb, fBC, -fCA);
   fz = fma(ca, fBC, -fAB);
-  fy = (Y > 0.0) ? om : ((Y < 0.0) ? -om : 0.0);
+  fy = signed_or_zero(om, Y);
 }
 
 // Element record fields of one rect/tri element, as scalars (read from shared memory by the caller).

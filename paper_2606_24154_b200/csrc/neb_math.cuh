@@ -34,8 +34,10 @@ __device__ __forceinline__ double mufu_rsqrt(double x) {
 // arithmetic, coefficients rounded to double and re-checked):
 //   atanh(z)/z = 1 + w A(w), w = z^2 <= 0.0403, degree 7: max relative error 7.5e-19
 //   atan(t)/t  = 1 + w B(w), w = t^2 <= 0.0719, degree 8: max relative error 1.3e-18
-static __constant__ double kAtanhC[8] = {0.3333333333333333, 0.20000000000004114, 0.14285714283573475, 0.11111111534886074,
-                                         0.09090867974834849, 0.0769446730129734, 0.06604199001390682, 0.06809533021415161};
+//   (stored doubled: the kernel needs 2 atanh)
+static __constant__ double kAtanhC[8] = {2 * 0.3333333333333333, 2 * 0.20000000000004114, 2 * 0.14285714283573475,
+                                         2 * 0.11111111534886074, 2 * 0.09090867974834849, 2 * 0.0769446730129734,
+                                         2 * 0.06604199001390682, 2 * 0.06809533021415161};
 static __constant__ double kAtanC[9] = {-0.3333333333333333, 0.19999999999996848, -0.14285714284542553, 0.11111110943140809,
                                         -0.09090896999665297, 0.0769181700719147, -0.06654898512832812, 0.05715903312379015,
                                         -0.03956311994071827};
@@ -46,6 +48,7 @@ __device__ __forceinline__ double clamp_tiny(double x) {
 }
 
 struct MathLib {
+  static constexpr bool kNeedsFar = true;    // libm path: far field through log1p
   static __device__ __forceinline__ double sqrt_nn(double x) { return sqrt(x); }
   static __device__ __forceinline__ double div_pos(double a, double b) { return a / b; }
   // ln(N/D) for N >= D > 0 in the near field, or 2 atanh(L/s) in the far field (s > 8 L)
@@ -59,15 +62,15 @@ struct MathLib {
 };
 
 struct MathFast {
+  static constexpr bool kNeedsFar = false;   // z = L/s whenever the exponent fold is zero
   // sqrt(x), x >= 0 finite (x = 0 -> 0).  One coupled Newton step on (g ~ sqrt x, h ~ 1/(2 sqrt x))
-  // from the 2^-23 seed, then one residual correction: 7 DFMA-class ops + 1 DMNMX + 1 MUFU.
+  // from the 2^-23 seed, then one residual correction: 6 DFMA-class ops + 1 integer clamp + 1 MUFU.
   static __device__ __forceinline__ double sqrt_nn(double x) {
     double y = mufu_rsqrt(clamp_tiny(x));
     double g = x * y, h = 0.5 * y;
     double r = fma(-g, h, 0.5);
-    g = fma(g, r, g);
-    h = fma(h, r, h);
-    double d = fma(-g, g, x);
+    g = fma(g, r, g);                 // relative error ~2^-45
+    double d = fma(-g, g, x);         // residual; the seed-accurate h is enough for the correction term
     return fma(d, h, g);
   }
   // 1/b for b > 0 finite normal: cubic step from the seed (error e^3 ~ 2^-69), 3 DFMA + 1 MUFU
@@ -89,10 +92,12 @@ struct MathFast {
     // e = round(pseudo-log2(N/D)) from the exponent/mantissa bits: N/(D 2^e) in [0.666, 1.502]
     int hN = __double2hiint(N), hD = __double2hiint(D);
     int e = ((hN - hD) + 0x80000) >> 20;
-    e = far ? 0 : e;
+    // N/D = (s+L)/(s-L) identically, so (N-D)/(N+D) = L/s: whenever e = 0 (ratio within [0.666, 1.5], which
+    // includes the whole far field) z is taken as L/s, which has no cancellation at all
+    (void)far;
     double D2 = __hiloint2double(hD + (e << 20), __double2loint(D));
-    double zn = far ? L : (N - D2);
-    double zd = far ? s : (N + D2);
+    double zn = (e == 0) ? L : (N - D2);
+    double zd = (e == 0) ? s : (N + D2);
     double z = zn * rcp_pos(zd);                 // |z| <= 0.2004
     double w = z * z;
     double p = kAtanhC[7];
@@ -103,8 +108,7 @@ struct MathFast {
     p = fma(p, w, kAtanhC[2]);
     p = fma(p, w, kAtanhC[1]);
     p = fma(p, w, kAtanhC[0]);
-    double zz = z + z;
-    double t = fma(zz * w, p, zz);               // 2 atanh(z)
+    double t = z * fma(w, p, 2.0);               // 2 atanh(z) = z (2 + w 2A(w)); coefficients hold 2A
     // e as a double without a conversion instruction: (2^52 + 2^31 + e) - (2^52 + 2^31)
     double ed = __hiloint2double(0x43300000, e ^ 0x80000000) - 4503601774854144.0;
     return fma(ed, 0.693147180559945309417, t);
@@ -128,9 +132,9 @@ struct MathFast {
     p = fma(p, w, kAtanC[2]);
     p = fma(p, w, kAtanC[1]);
     p = fma(p, w, kAtanC[0]);
-    double a = fma(t * w, p, t) + (big ? 0.52359877559829887308 : 0.0);   // + pi/6
+    double a = fma(t, fma(w, p, 1.0), big ? 0.52359877559829887308 : 0.0);   // atan(t) + pi/6
     a = (y > ax) ? (NEB_HALF_PI - a) : a;
-    a = (x < 0.0) ? (NEB_PI - a) : a;
+    a = (__double2hiint(x) < 0) ? (NEB_PI - a) : a;
     return a;
   }
 };
