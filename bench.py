@@ -31,9 +31,12 @@ sys.path.insert(0, ROOT)
 
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
-# algorithmic FP64 work of one (point, element copy) evaluation of (Phi', E') — hand count of the closed
-# forms in DESIGN.md §6 (FMA = 2 flop): rectangle 348, right triangle 291, wire 139, point charge 30
-FLOP_PER_PAIR = {"rect": 348.0, "tri": 291.0, "wire": 139.0, "charge": 30.0}
+# FP64 work of one (point, element copy) evaluation of (Phi', E') on the path that >99 % of the pairs of a field
+# map take (warp-uniform far branch), counted in the SASS of eval_kernel<MathFast> (FMA = 2 flop):
+# rectangle 113 DFMA + 38 DMUL + 15 DADD = 279 flop in 167 FP64-pipe instructions (the near branch: 323 flop,
+# 206 instructions); right triangle 232 flop; wire 139; point charge 30
+FLOP_PER_PAIR = {"rect": 279.0, "tri": 232.0, "wire": 139.0, "charge": 30.0}
+FP64_INSTR_PER_PAIR = {"rect": 167.0}
 CONFIG = {"workload": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
           "n_elements": 6144, "m_points": 100000, "step": "assemble+solve(LU)+eval",
           "l2": "256 MiB buffer written between timed steps; matrix (302 MB) exceeds L2"}
@@ -243,6 +246,7 @@ def main():
                          "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process "
                                         "(nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2)",
                          "flop_per_pair": FLOP_PER_PAIR["rect"], "kernel_ms": eval_ms,
+                         "fp64_pipe_slot_frac": FP64_INSTR_PER_PAIR["rect"] * m * n / (eval_ms * 1e-3) / (0.5e12 * dfma_peak),
                          "pairs_per_s_kernel": m * n / (eval_ms * 1e-3),
                          "field_map_points_per_s": m / (eval_ms * 1e-3)},
             "stages_ms": stages,

@@ -64,7 +64,7 @@ struct Staging {   // temporaries of one ABI call
     if (!p || bytes == 0) return NEB_OK;
     if (is_device_ptr(p)) { *out = p; return NEB_OK; }
     void* d = nullptr;
-    NEB_CUDA(c, cudaMallocAsync(&d, bytes, c->stream));
+    NEB_CUDA(c, cudaMallocFromPoolAsync(&d, bytes, c->pool, c->stream));
     temps.push_back(d);
     NEB_CUDA(c, cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, c->stream));
     *out = d;
@@ -78,7 +78,7 @@ struct Staging {   // temporaries of one ABI call
     if (!p || bytes == 0) return NEB_OK;
     if (is_device_ptr(p)) { *dev = p; return NEB_OK; }
     void* d = nullptr;
-    NEB_CUDA(c, cudaMallocAsync(&d, bytes, c->stream));
+    NEB_CUDA(c, cudaMallocFromPoolAsync(&d, bytes, c->pool, c->stream));
     temps.push_back(d);
     outs.push_back({d, p, bytes});
     *dev = d;
@@ -191,6 +191,7 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
     double w = (k == NEB_RECT) ? 0.5 : (1.0 / 3.0);
     for (int c = 0; c < 3; ++c) cp[c] = p0[c] + w * (a1[c] + a2[c]);
     if (k == NEB_TRI) aux = 1.0 / sqrt(la * la + lb * lb);
+    else aux = la * lb;
   }
   if (colloc_in) { cp[0] = colloc_in[j]; cp[1] = colloc_in[n + j]; cp[2] = colloc_in[2 * n + j]; }
   double* r = rec + s;
@@ -199,6 +200,13 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
   r[6 * stride] = ey[0]; r[7 * stride] = ey[1]; r[8 * stride] = ey[2];
   r[9 * stride] = ez[0]; r[10 * stride] = ez[1]; r[11 * stride] = ez[2];
   r[12 * stride] = la; r[13 * stride] = lb; r[14 * stride] = aux; r[15 * stride] = 0.0;
+  {
+    // far-field radius of the warp-uniform shortcut (neb_influence.cuh): 2.5 longest edges beyond the reach from v0
+    double diag = sqrt(la * la + lb * lb);
+    double lmax = (k == NEB_TRI) ? diag : fmax(la, fabs(lb));
+    double rf = 2.5 * lmax + diag;
+    r[16 * stride] = rf * rf;
+  }
   for (int c = 0; c < 3; ++c) { colloc[c * stride + s] = cp[c]; normal[c * stride + s] = ey[c]; }
   int bk = bc_kind_in[j];
   if (bk != NEB_BC_DIRICHLET && bk != NEB_BC_DIELECTRIC) { atomicOr(flag, 16); bk = NEB_BC_DIRICHLET; }
@@ -283,6 +291,18 @@ neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
   bool ok = cudaMalloc((void**)&c->d_flag, sizeof(int32_t)) == cudaSuccess &&
             cudaMemset(c->d_flag, 0, sizeof(int32_t)) == cudaSuccess &&
             cudaMalloc(&c->d_panel_ws, lu_panel_ws_bytes(c->num_sms)) == cudaSuccess;
+  if (ok) {
+    // staging temporaries come from a pool of the context's own that keeps its memory across synchronisations
+    // (the default pool hands everything back to the driver at each sync: milliseconds per re-allocation)
+    cudaMemPoolProps pp = {};
+    pp.allocType = cudaMemAllocationTypePinned;
+    pp.handleTypes = cudaMemHandleTypeNone;
+    pp.location.type = cudaMemLocationTypeDevice;
+    pp.location.id = device;
+    unsigned long long keep = ~0ULL;
+    ok = cudaMemPoolCreate(&c->pool, &pp) == cudaSuccess &&
+         cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep) == cudaSuccess;
+  }
   for (int s = 0; ok && s < NEB_STAGE_COUNT; ++s)
     ok = cudaEventCreate(&c->ev0[s]) == cudaSuccess && cudaEventCreate(&c->ev1[s]) == cudaSuccess;
   if (!ok) {
@@ -302,6 +322,7 @@ void neb_destroy(neb_ctx* c) {
   if (c->d_panel_ws) cudaFree(c->d_panel_ws);
   if (c->d_charges) cudaFree(c->d_charges);
   if (c->d_scratch) cudaFree(c->d_scratch);
+  if (c->pool) cudaMemPoolDestroy(c->pool);
   for (int s = 0; s < NEB_STAGE_COUNT; ++s) {
     if (c->ev0[s]) cudaEventDestroy(c->ev0[s]);
     if (c->ev1[s]) cudaEventDestroy(c->ev1[s]);
@@ -390,7 +411,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_img is a stack buffer
   }
   int32_t* d_counts = nullptr;
-  NEB_CUDA(c, cudaMallocAsync((void**)&d_counts, 3 * sizeof(int32_t), c->stream));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&d_counts, 3 * sizeof(int32_t), c->pool, c->stream));
   sg.temps.push_back(d_counts);
   {
     StageTimer t(c, NEB_STAGE_GEOMETRY);

@@ -38,7 +38,7 @@ __device__ __forceinline__ Frame frame_of(const TileSmem& sm, int e) {
   f.exx = sm.rec[3][e]; f.exy = sm.rec[4][e]; f.exz = sm.rec[5][e];
   f.eyx = sm.rec[6][e]; f.eyy = sm.rec[7][e]; f.eyz = sm.rec[8][e];
   f.ezx = sm.rec[9][e]; f.ezy = sm.rec[10][e]; f.ezz = sm.rec[11][e];
-  f.a = sm.rec[12][e]; f.b = sm.rec[13][e]; f.aux = sm.rec[14][e];
+  f.a = sm.rec[12][e]; f.b = sm.rec[13][e]; f.aux = sm.rec[14][e]; f.far2 = sm.rec[16][e];
   return f;
 }
 
@@ -56,7 +56,7 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
       Frame fr = frame_of(sm, e);
       // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
       // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
-      Infl acc = influence<M, KIND>(fr, px - sm.img[0][0], py - sm.img[1][0], pz - sm.img[2][0]);
+      Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
       if (sink.self_pv(base + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
 #pragma unroll 1
       for (int s = 1; s < n_img; ++s) {
@@ -382,10 +382,10 @@ neb_status form_rhs(neb_ctx* c) {
     // Phi_sc, E_sc at the collocation points: reuse d_x (npad >= n) for phi and a scratch tail for E.
     // field_at_points uses d_scratch for its partials, so E lives in a dedicated allocation.
     phi = c->d_x;
-    NEB_CUDA(c, cudaMallocAsync((void**)&E, (size_t)3 * n * sizeof(double), c->stream));
+    NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&E, (size_t)3 * n * sizeof(double), c->pool, c->stream));
     // collocation points are stored with stride c->stride; field_at_points wants stride m: pack
     double* pts = nullptr;
-    NEB_CUDA(c, cudaMallocAsync((void**)&pts, (size_t)3 * n * sizeof(double), c->stream));
+    NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&pts, (size_t)3 * n * sizeof(double), c->pool, c->stream));
     for (int k = 0; k < 3; ++k)
       NEB_CUDA(c, cudaMemcpyAsync(pts + k * n, c->d_colloc + k * c->stride, (size_t)n * sizeof(double),
                                   cudaMemcpyDeviceToDevice, c->stream));

@@ -18,9 +18,11 @@ namespace neb {
 //   9..11 ez      unit vector along e2 (local Z)                    [wire: unused]
 //   12    a       |e1|
 //   13    b       |e2|                                              [wire: radius r_w]
-//   14    aux     triangle: 1/hypotenuse; wire: 2 pi r_w            [rect: unused]
+//   14    aux     rectangle: a b; triangle: 1/hypotenuse; wire: 2 pi r_w
 //   15    w       weight: sigma_j / (4 pi eps0) for evaluation (set by neb_solve / neb_set_sigma)
-#define NEB_REC 16
+//   16    far2    (2.5 Lmax + diag)^2, Lmax = longest edge, diag = sqrt(a^2+b^2): a point at least that far
+//                 (squared) from v0 is >= 2.5 Lmax away from every point of the element      [wire: unused]
+#define NEB_REC 17
 
 struct Infl {
   double phi, ex, ey, ez;   // primed potential and GLOBAL primed field components
@@ -53,27 +55,49 @@ __device__ __forceinline__ double edge_log(double lm, double lp, double Rm, doub
 
 // Rectangle [0,a] x [0,b] in the local XZ plane; (X, Y, Z) local coordinates of P.
 // out: phi', local field (fx, fy, fz).
+// Far field, decided per WARP (one vote, no divergence): when every lane's point is at least 2.5 Lmax away from
+// the element, every edge has R- + R+ >= 5 L and the solid angle is < 0.16 sr, so the case selections of edge_log
+// and the argument reduction of the arctangent are dead code; the far branch evaluates the SAME closed form
+// (2 atanh(L/s) per edge, one arctangent) without them.  ~99 % of the pairs of a field map take it.
+// r0sq = squared distance from the point to v0 (already needed for the corner radius).
 template <class M>
-__device__ __forceinline__ void rect_local(double a, double b, double X, double Y, double Z, double& phi,
+__device__ __forceinline__ bool warp_is_far(double r0sq, double far2) {
+  if (!M::kFarPath) return false;
+  return __all_sync(0xffffffffu, r0sq >= far2);
+}
+
+template <class M>
+__device__ __forceinline__ void rect_local(double a, double b, double ab, double far2, double X, double Y, double Z, double& phi,
                                            double& fx, double& fy, double& fz) {
   double u1 = -X, u2 = a - X, w1 = -Z, w2 = b - Z, y = fabs(Y);
   double yy = y * y;
   double A1 = fma(u1, u1, yy), A2 = fma(u2, u2, yy);      // squared distances to the lines x = x_i
   double B1 = fma(w1, w1, yy), B2 = fma(w2, w2, yy);      // squared distances to the lines z = z_j
-  double r11 = M::sqrt_nn(fma(w1, w1, A1)), r12 = M::sqrt_nn(fma(w2, w2, A1));
+  double q11 = fma(w1, w1, A1);
+  const bool far = warp_is_far<M>(q11, far2);
+  double r11 = M::sqrt_nn(q11), r12 = M::sqrt_nn(fma(w2, w2, A1));
   double r21 = M::sqrt_nn(fma(w1, w1, A2)), r22 = M::sqrt_nn(fma(w2, w2, A2));
-  double F1 = edge_log<M>(w1, w2, r11, r12, A1, b);       // edge x = 0
-  double F2 = edge_log<M>(w1, w2, r21, r22, A2, b);       // edge x = a
-  double G1 = edge_log<M>(u1, u2, r11, r21, B1, a);       // edge z = 0
-  double G2 = edge_log<M>(u1, u2, r12, r22, B2, a);       // edge z = b
+  double F1, F2, G1, G2, om;
+  if (far) {
+    F1 = M::far_log(b, r11 + r12);
+    F2 = M::far_log(b, r21 + r22);
+    G1 = M::far_log(a, r11 + r21);
+    G2 = M::far_log(a, r12 + r22);
+  } else {
+    F1 = edge_log<M>(w1, w2, r11, r12, A1, b);            // edge x = 0
+    F2 = edge_log<M>(w1, w2, r21, r22, A2, b);            // edge x = a
+    G1 = edge_log<M>(u1, u2, r11, r21, B1, a);            // edge z = 0
+    G2 = edge_log<M>(u1, u2, r12, r22, B2, a);            // edge z = b
+  }
   // solid angle: two fan triangles (c11,c21,c22), (c11,c22,c12); tan(Omega_t/2) = 2A_t |d| / D_t with the
   // triple product written as area x height (exact for a flat element: no far-field cancellation)
   double p = u1 * u2, q = w1 * w2;
   double d1122 = p + yy + q;
   double D1 = fma(r11 * r21, r22, fma(p + B1, r22, fma(d1122, r21, (A2 + q) * r11)));
   double D2 = fma(r11 * r22, r12, fma(d1122, r12, fma(A1 + q, r22, (p + B2) * r11)));
-  double Nn = a * b * y;
-  double om = 2.0 * M::atan2_pos(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));
+  double Nn = ab * y;
+  if (far) om = 2.0 * M::far_atan2(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));
+  else om = 2.0 * M::atan2_pos(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));
   phi = fma(u2, F2, fma(-u1, F1, fma(w2, G2, fma(-w1, G1, -y * om))));
   fx = F2 - F1;
   fz = G2 - G1;
@@ -82,23 +106,32 @@ __device__ __forceinline__ void rect_local(double a, double b, double X, double 
 
 // Right triangle (0,0), (a,0), (0,b) in the local XZ plane, ih = 1/sqrt(a^2+b^2).
 template <class M>
-__device__ __forceinline__ void tri_local(double a, double b, double ih, double X, double Y, double Z, double& phi,
-                                          double& fx, double& fy, double& fz) {
+__device__ __forceinline__ void tri_local(double a, double b, double ih, double far2, double X, double Y, double Z,
+                                          double& phi, double& fx, double& fy, double& fz) {
   double uA = -X, uB = a - X, wA = -Z, wC = b - Z, y = fabs(Y);
   double yy = y * y;
   double A0 = fma(uA, uA, yy), W0 = fma(wA, wA, yy);
-  double RA = M::sqrt_nn(fma(wA, wA, A0)), RB = M::sqrt_nn(fma(uB, uB, W0)), RC = M::sqrt_nn(fma(wC, wC, A0));
-  double fAB = edge_log<M>(uA, uB, RA, RB, W0, a);        // leg on the X axis, outward normal -Z, P0 = Z
-  double fCA = edge_log<M>(wA, wC, RA, RC, A0, b);        // leg on the Z axis, outward normal -X, P0 = X
+  double qA = fma(wA, wA, A0);
+  const bool far = warp_is_far<M>(qA, far2);
+  double RA = M::sqrt_nn(qA), RB = M::sqrt_nn(fma(uB, uB, W0)), RC = M::sqrt_nn(fma(wC, wC, A0));
   double ca = a * ih, cb = b * ih;                        // hypotenuse B->C: t = (-ca, cb), m = (cb, ca)
-  double lm = fma(-ca, uB, cb * wA);
   double h = (a * a + b * b) * ih;
-  double lp = lm + h;
   double P0 = fma(cb, uB, ca * wA);
-  double fBC = edge_log<M>(lm, lp, RB, RC, fma(P0, P0, yy), h);
+  double fAB, fCA, fBC;
+  if (far) {
+    fAB = M::far_log(a, RA + RB);
+    fCA = M::far_log(b, RA + RC);
+    fBC = M::far_log(h, RB + RC);
+  } else {
+    fAB = edge_log<M>(uA, uB, RA, RB, W0, a);             // leg on the X axis, outward normal -Z, P0 = Z
+    fCA = edge_log<M>(wA, wC, RA, RC, A0, b);             // leg on the Z axis, outward normal -X, P0 = X
+    double lm = fma(-ca, uB, cb * wA);
+    double lp = lm + h;
+    fBC = edge_log<M>(lm, lp, RB, RC, fma(P0, P0, yy), h);
+  }
   double dAB = fma(uA, uB, W0), dAC = fma(wA, wC, A0), dBC = fma(uA, uB, fma(wA, wC, yy));
   double D = fma(RA * RB, RC, fma(dAB, RC, fma(dAC, RB, dBC * RA)));
-  double om = 2.0 * M::atan2_pos(a * b * y, D);
+  double om = 2.0 * (far ? M::far_atan2(a * b * y, D) : M::atan2_pos(a * b * y, D));
   phi = fma(Z, fAB, fma(X, fCA, fma(P0, fBC, -y * om)));
   fx = fma(cb, fBC, -fCA);
   fz = fma(ca, fBC, -fAB);
@@ -107,7 +140,7 @@ __device__ __forceinline__ void tri_local(double a, double b, double ih, double 
 
 // Element record fields of one rect/tri element, as scalars (read from shared memory by the caller).
 struct Frame {
-  double v0x, v0y, v0z, exx, exy, exz, eyx, eyy, eyz, ezx, ezy, ezz, a, b, aux;
+  double v0x, v0y, v0z, exx, exy, exz, eyx, eyy, eyz, ezx, ezy, ezz, a, b, aux, far2;
 };
 
 template <class M, int KIND>
@@ -139,8 +172,8 @@ __device__ __forceinline__ Infl influence(const Frame& f, double px, double py, 
   double Y = fma(dx, f.eyx, fma(dy, f.eyy, dz * f.eyz));
   double Z = fma(dx, f.ezx, fma(dy, f.ezy, dz * f.ezz));
   double lx, ly, lz;
-  if (KIND == 0) rect_local<M>(f.a, f.b, X, Y, Z, o.phi, lx, ly, lz);
-  else tri_local<M>(f.a, f.b, f.aux, X, Y, Z, o.phi, lx, ly, lz);
+  if (KIND == 0) rect_local<M>(f.a, f.b, f.aux, f.far2, X, Y, Z, o.phi, lx, ly, lz);
+  else tri_local<M>(f.a, f.b, f.aux, f.far2, X, Y, Z, o.phi, lx, ly, lz);
   o.ex = fma(lx, f.exx, fma(ly, f.eyx, lz * f.ezx));
   o.ey = fma(lx, f.exy, fma(ly, f.eyy, lz * f.ezy));
   o.ez = fma(lx, f.exz, fma(ly, f.eyz, lz * f.ezz));

@@ -10,7 +10,7 @@ namespace neb {
 
 constexpr double kEps0 = 8.8541878128e-12;                 // F/m (reading S3)
 constexpr double kCoulomb = 1.0 / (4.0 * 3.14159265358979323846 * kEps0);
-constexpr int kRec = 16;                                   // doubles per frame-table record
+constexpr int kRec = 17;                                   // doubles per frame-table record
 constexpr int kPad = 128;                                  // matrix dimension is padded to a multiple of this
 
 // Frame tables (a1), elements sorted by kind: [rect | tri | wire].  SoA, field-major:
@@ -31,6 +31,7 @@ struct StageStat {
 struct neb_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
+  cudaMemPool_t pool = nullptr;   // staging temporaries (stream-ordered, memory kept across syncs)
   int num_sms = 0;
   std::string err;
 

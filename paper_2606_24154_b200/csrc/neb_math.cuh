@@ -49,6 +49,9 @@ __device__ __forceinline__ double clamp_tiny(double x) {
 
 struct MathLib {
   static constexpr bool kNeedsFar = true;    // libm path: far field through log1p
+  static constexpr bool kFarPath = false;    // no warp-uniform far-field shortcut: this policy is the plain reference
+  static __device__ __forceinline__ double far_log(double, double) { return 0.0; }
+  static __device__ __forceinline__ double far_atan2(double, double) { return 0.0; }
   static __device__ __forceinline__ double sqrt_nn(double x) { return sqrt(x); }
   static __device__ __forceinline__ double div_pos(double a, double b) { return a / b; }
   // ln(N/D) for N >= D > 0 in the near field, or 2 atanh(L/s) in the far field (s > 8 L)
@@ -63,6 +66,7 @@ struct MathLib {
 
 struct MathFast {
   static constexpr bool kNeedsFar = false;   // z = L/s whenever the exponent fold is zero
+  static constexpr bool kFarPath = true;     // warp-uniform shortcut when every lane is >= 2.5 edge lengths away
   // sqrt(x), x >= 0 finite (x = 0 -> 0).  One coupled Newton step on (g ~ sqrt x, h ~ 1/(2 sqrt x))
   // from the 2^-23 seed, then one residual correction: 6 DFMA-class ops + 1 integer clamp + 1 MUFU.
   static __device__ __forceinline__ double sqrt_nn(double x) {
@@ -112,6 +116,36 @@ struct MathFast {
     // e as a double without a conversion instruction: (2^52 + 2^31 + e) - (2^52 + 2^31)
     double ed = __hiloint2double(0x43300000, e ^ 0x80000000) - 4503601774854144.0;
     return fma(ed, 0.693147180559945309417, t);
+  }
+  // Far field (s >= 5 L, i.e. z <= 0.2, guaranteed by the caller): ln[(s+L)/(s-L)] = 2 atanh(L/s) with the same
+  // polynomial as log_ratio's e == 0 case, but no case selection, no exponent fold: 15 FP64 instructions + 1 MUFU.
+  static __device__ __forceinline__ double far_log(double L, double s) {
+    double z = L * rcp_pos(s);
+    double w = z * z;
+    double p = kAtanhC[7];
+    p = fma(p, w, kAtanhC[6]);
+    p = fma(p, w, kAtanhC[5]);
+    p = fma(p, w, kAtanhC[4]);
+    p = fma(p, w, kAtanhC[3]);
+    p = fma(p, w, kAtanhC[2]);
+    p = fma(p, w, kAtanhC[1]);
+    p = fma(p, w, kAtanhC[0]);
+    return z * fma(w, p, 2.0);
+  }
+  // atan(y/x) for x > 0, 0 <= y <= tan(pi/12) x (guaranteed by the caller in the far field): no argument reduction
+  static __device__ __forceinline__ double far_atan2(double y, double x) {
+    double t = y * rcp_pos(x);
+    double w = t * t;
+    double p = kAtanC[8];
+    p = fma(p, w, kAtanC[7]);
+    p = fma(p, w, kAtanC[6]);
+    p = fma(p, w, kAtanC[5]);
+    p = fma(p, w, kAtanC[4]);
+    p = fma(p, w, kAtanC[3]);
+    p = fma(p, w, kAtanC[2]);
+    p = fma(p, w, kAtanC[1]);
+    p = fma(p, w, kAtanC[0]);
+    return fma(t * w, p, t);
   }
   static __device__ __forceinline__ double atan2_pos(double y, double x) {
     y = fabs(y);                                          // rounding noise may make a zero numerator negative
