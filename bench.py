@@ -226,6 +226,15 @@ def main():
     flush.fill_(1)
     step_resident()
     stages = {k: round(v[0], 4) for k, v in nb.stage_ms().items()}
+    # the trailing update alone is only timed without look-ahead (with it, it overlaps the next panel)
+    nb.set_option(P.binding.NEB_OPT_LU_LOOKAHEAD, 0)
+    nb.reset_stats()
+    flush.fill_(1)
+    step_resident()
+    serial = nb.stage_ms()
+    stages["lu_gemm"] = round(serial["lu_gemm"][0], 4)
+    stages["lu_no_lookahead"] = round(serial["lu"][0], 4)
+    nb.set_option(P.binding.NEB_OPT_LU_LOOKAHEAD, 1)
     nb.set_option(P.binding.NEB_OPT_PROFILE, 0)
     dfma_peak, dmma_peak = nb.fp64_peak(0), nb.fp64_peak(1)
     flop_eval = FLOP_PER_PAIR["rect"] * m * n

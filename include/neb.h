@@ -51,8 +51,11 @@ enum {
   NEB_OPT_MATH = 0,     /* 1 (default): hand-written log/atan2/sqrt/rcp sequences; 0: CUDA libm  */
   NEB_OPT_LU_BLOCK = 1, /* LU panel width nb; this build supports 64 only                        */
   NEB_OPT_PROFILE = 2,  /* 1: record per-stage CUDA-event timings (neb_stage_ms); default 0      */
-  NEB_OPT_LU_PANEL = 3  /* 0 (default): cluster/DSMEM panel kernel where the panel fits (<= 8192 rows),
+  NEB_OPT_LU_PANEL = 3, /* 0 (default): cluster/DSMEM panel kernel where the panel fits (<= 8192 rows),
                            grid-wide cooperative kernel above; 1: grid-wide kernel only          */
+  NEB_OPT_LU_LOOKAHEAD = 4 /* 1 (default): panel k+1 is factored on an internal stream while the trailing
+                           update of panel k runs (cluster panels only); 0: one stream, and
+                           NEB_STAGE_LU_GEMM is then timed alone                                 */
 };
 
 /* Stages for neb_stage_ms. */

@@ -303,6 +303,13 @@ neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
     ok = cudaMemPoolCreate(&c->pool, &pp) == cudaSuccess &&
          cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep) == cudaSuccess;
   }
+  if (ok) {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);   // hi = numerically lowest = greatest priority
+    ok = cudaStreamCreateWithPriority(&c->side_stream, cudaStreamNonBlocking, hi) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->ev_next, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->ev_panel, cudaEventDisableTiming) == cudaSuccess;
+  }
   for (int s = 0; ok && s < NEB_STAGE_COUNT; ++s)
     ok = cudaEventCreate(&c->ev0[s]) == cudaSuccess && cudaEventCreate(&c->ev1[s]) == cudaSuccess;
   if (!ok) {
@@ -323,6 +330,9 @@ void neb_destroy(neb_ctx* c) {
   if (c->d_charges) cudaFree(c->d_charges);
   if (c->d_scratch) cudaFree(c->d_scratch);
   if (c->pool) cudaMemPoolDestroy(c->pool);
+  if (c->side_stream) { cudaStreamSynchronize(c->side_stream); cudaStreamDestroy(c->side_stream); }
+  if (c->ev_next) cudaEventDestroy(c->ev_next);
+  if (c->ev_panel) cudaEventDestroy(c->ev_panel);
   for (int s = 0; s < NEB_STAGE_COUNT; ++s) {
     if (c->ev0[s]) cudaEventDestroy(c->ev0[s]);
     if (c->ev1[s]) cudaEventDestroy(c->ev1[s]);
@@ -341,6 +351,7 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
       return NEB_OK;
     case NEB_OPT_PROFILE: c->profile = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_LU_PANEL: c->panel_mode = value ? 1 : 0; return NEB_OK;
+    case NEB_OPT_LU_LOOKAHEAD: c->lu_lookahead = value ? 1 : 0; return NEB_OK;
     default: return fail(c, NEB_EINVAL, "unknown option");
   }
 }

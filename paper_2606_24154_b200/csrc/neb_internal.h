@@ -31,6 +31,8 @@ struct StageStat {
 struct neb_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t side_stream = nullptr;   // LU look-ahead: next panel, concurrent with the trailing update
+  cudaEvent_t ev_next = nullptr, ev_panel = nullptr;
   cudaMemPool_t pool = nullptr;   // staging temporaries (stream-ordered, memory kept across syncs)
   int num_sms = 0;
   std::string err;
@@ -39,6 +41,7 @@ struct neb_ctx {
   int math_fast = 1;
   int lu_nb = 64;
   int profile = 0;
+  int lu_lookahead = 1; // 1: factor panel k+1 on the side stream while panel k's trailing update runs
   int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
 
   // geometry
@@ -122,7 +125,7 @@ size_t lu_panel_ws_bytes(int num_sms);
 
 // neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
 int64_t panel_cluster_max_rows(neb_ctx* c);
-neb_status panel_cluster_launch(neb_ctx* c, int64_t k);
+neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream);
 
 // neb_peaks.cu ------------------------------------------------------------------------------------
 neb_status fp64_peak(neb_ctx* c, int kind, double* tflops);

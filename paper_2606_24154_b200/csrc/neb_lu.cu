@@ -171,14 +171,16 @@ __global__ void __launch_bounds__(PANEL_THREADS) panel_kernel(double* __restrict
   }
 }
 
-// Row exchanges of one panel applied to every column outside it.  One thread per column.
-__global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t npad, int64_t k, const int32_t* __restrict__ ipiv) {
+// Row exchanges of panel k applied to the columns [c_lo, c_hi), minus the columns [skip_lo, skip_hi) (the panel's
+// own, and with look-ahead the next panel's, which were exchanged ahead of the others).  One thread per column.
+__global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, const int32_t* __restrict__ ipiv, int64_t c_lo,
+                             int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
   __shared__ int s_piv[NB];
   if (threadIdx.x < NB) s_piv[threadIdx.x] = ipiv[k + threadIdx.x];
   __syncthreads();
-  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= npad - NB) return;
-  if (c >= k) c += NB;                             // skip the panel's own columns
+  int64_t c = c_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= skip_lo) c += skip_hi - skip_lo;
+  if (c >= c_hi) return;
   double* col = A + c * ld;
   for (int t = 0; t < NB; ++t) {
     int p = s_piv[t];
@@ -196,12 +198,12 @@ __global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t npad, i
 // thread updates its rows below j with L11 read from shared memory (warp-uniform address: broadcast).
 constexpr int TRSM_THREADS = 256;
 constexpr size_t TRSM_SMEM = (size_t)(NB * (NB + 1) + 2 * NB) * sizeof(double);
-__global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k) {
+__global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t c_first) {
   extern __shared__ double s_trsm[];
   double(*sL)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm);     // sL[i][j] = L11[i][j]
   double* sX = s_trsm + NB * (NB + 1);                                    // sX[(j & 1) * NB + c]
   const int tid = threadIdx.x, c = tid & (NB - 1), q = tid >> 6;         // q = 0..3
-  const int64_t c0 = k + NB + (int64_t)blockIdx.x * NB;
+  const int64_t c0 = c_first + (int64_t)blockIdx.x * NB;
   for (int j = q; j < NB; j += 4) sL[c][j] = A[(k + c) + (k + j) * ld];
   double x[NB / 4];
   // column c of the slab: rows q + 4t.  Loaded through shared memory would be coalesced; direct loads hit
@@ -252,13 +254,13 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 }
 
 __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t r0,
-                                                               int64_t m) {
+                                                               int64_t m, int64_t c_first) {
   extern __shared__ __align__(16) double smem[];
   double* sL = smem;                 // sL[kk * LDL + i] = L[i][kk]
   double* sU = smem + GK * LDL;      // sU[j * LDU + kk] = U[kk][j]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t i0 = r0 + (int64_t)blockIdx.x * GM;       // first row of the tile
-  const int64_t j0 = r0 + (int64_t)blockIdx.y * GN;       // first column
+  const int64_t j0 = c_first + (int64_t)blockIdx.y * GN;  // first column
   const int rows_here = (int)min((int64_t)GM, r0 + m - i0);   // 64 or 128
   // stage operands: two k-halves as two cp.async groups
 #pragma unroll
@@ -465,45 +467,76 @@ neb_status lu_factor(neb_ctx* c) {
     attr_set = true;
   }
   PanelWs* ws = (PanelWs*)c->d_panel_ws;
-  const int64_t cluster_rows = panel_cluster_max_rows(c);
-  for (int64_t k = 0; k < npad; k += NB) {
+  const int64_t cluster_rows = c->panel_mode == 0 ? panel_cluster_max_rows(c) : 0;
+  cudaStream_t S1 = c->stream, S2 = c->side_stream;
+
+  // panel k on stream st: the cluster kernel where the panel fits, else the grid-wide cooperative kernel
+  auto launch_panel = [&](int64_t k, cudaStream_t st) -> neb_status {
     const int64_t mrows = npad - k;
+    if (mrows <= cluster_rows) return panel_cluster_launch(c, k, st);
     // rows per CTA: multiple of 32, at most 200 KB of shared memory (390 rows -> 384)
     int G = (int)min((int64_t)c->num_sms, (mrows + 63) / 64);
-    if (G > 148) G = 148;
     int mc = (int)((mrows + G - 1) / G);
     mc = (mc + 31) / 32 * 32;
     size_t smem = (size_t)mc * NB * sizeof(double);
     if (smem > 200 * 1024) return fail(c, NEB_ENOMEM, "LU panel slab exceeds shared memory: n too large for this build");
     G = (int)((mrows + mc - 1) / mc);
-    if (c->panel_mode == 0 && mrows <= cluster_rows) {
-      NEB_TRY(panel_cluster_launch(c, k));
-    } else {
-      NEB_CUDA(c, cudaMemsetAsync(&ws->counter, 0, sizeof(unsigned int), c->stream));
-      double* A = c->d_K;
-      int64_t ld_ = ld, npad_ = npad, k_ = k;
-      int mc_ = mc;
-      int32_t* ipiv = c->d_ipiv;
-      int32_t* flag = c->d_flag;
-      void* args[] = {&A, &ld_, &npad_, &k_, &mc_, &ipiv, &ws, &flag};
-      NEB_CUDA(c, cudaLaunchCooperativeKernel((void*)panel_kernel, dim3(G), dim3(PANEL_THREADS), args, smem, c->stream));
-      c->launches++;
-    }
-    {
-      int64_t ncols = npad - NB;
-      if (ncols > 0) {
-        laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, c->stream>>>(c->d_K, ld, npad, k, c->d_ipiv);
-        c->launches++;
-      }
-    }
+    NEB_CUDA(c, cudaMemsetAsync(&ws->counter, 0, sizeof(unsigned int), st));
+    double* A = c->d_K;
+    int64_t ld_ = ld, npad_ = npad, k_ = k;
+    int32_t* ipiv = c->d_ipiv;
+    int32_t* flag = c->d_flag;
+    void* args[] = {&A, &ld_, &npad_, &k_, &mc, &ipiv, &ws, &flag};
+    NEB_CUDA(c, cudaLaunchCooperativeKernel((void*)panel_kernel, dim3(G), dim3(PANEL_THREADS), args, smem, st));
+    c->launches++;
+    return NEB_OK;
+  };
+  // row exchanges of panel k on the columns [c_lo, c_hi) \ [skip_lo, skip_hi)
+  auto laswp = [&](int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
+    const int64_t ncols = (c_hi - c_lo) - (skip_hi - skip_lo);
+    if (ncols <= 0) return;
+    laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, S1>>>(c->d_K, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
+    c->launches++;
+  };
+  // U12 and the trailing update of panel k restricted to the columns [c_first, c_first + ncols)
+  auto update = [&](int64_t k, int64_t c_first, int64_t ncols, bool timed) {
+    if (ncols <= 0) return;
     const int64_t r0 = k + NB, m = npad - r0;
-    if (m > 0) {
-      trsm_kernel<<<(unsigned)(m / NB), TRSM_THREADS, TRSM_SMEM, c->stream>>>(c->d_K, ld, k);
-      c->launches++;
+    trsm_kernel<<<(unsigned)(ncols / NB), TRSM_THREADS, TRSM_SMEM, S1>>>(c->d_K, ld, k, c_first);
+    c->launches++;
+    dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
+    if (timed) {
       StageTimer tg(c, NEB_STAGE_LU_GEMM);
-      dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(m / GN));
-      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, c->stream>>>(c->d_K, ld, k, r0, m);
+      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, S1>>>(c->d_K, ld, k, r0, m, c_first);
       c->launches++;
+    } else {
+      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, S1>>>(c->d_K, ld, k, r0, m, c_first);
+      c->launches++;
+    }
+  };
+
+  // Right-looking with a look-ahead of one panel: as soon as panel k is factored, ITS update is applied to the 64
+  // columns of panel k+1 first; panel k+1 is then factored on the side stream (one cluster: 16 SMs) while the main
+  // stream updates the rest of the trailing matrix on the other SMs.  Only where the next panel runs on a cluster
+  // (the grid-wide panel kernel needs every SM).  The trailing update is timed alone only without look-ahead.
+  NEB_TRY(launch_panel(0, S1));
+  for (int64_t k = 0; k < npad; k += NB) {
+    const int64_t r0 = k + NB, m = npad - r0;
+    const bool ahead = c->lu_lookahead && S2 && m > NB && m <= cluster_rows;
+    if (ahead) {
+      laswp(k, r0, r0 + NB, r0 + NB, r0 + NB);
+      update(k, r0, NB, false);
+      NEB_CUDA(c, cudaEventRecord(c->ev_next, S1));
+      NEB_CUDA(c, cudaStreamWaitEvent(S2, c->ev_next, 0));
+      NEB_TRY(launch_panel(r0, S2));
+      NEB_CUDA(c, cudaEventRecord(c->ev_panel, S2));
+      laswp(k, 0, npad, k, r0 + NB);
+      update(k, r0 + NB, m - NB, false);
+      NEB_CUDA(c, cudaStreamWaitEvent(S1, c->ev_panel, 0));
+    } else {
+      laswp(k, 0, npad, k, r0);
+      update(k, r0, m, !c->lu_lookahead);
+      if (m > 0) NEB_TRY(launch_panel(r0, S1));
     }
     NEB_CUDA(c, cudaGetLastError());
   }

@@ -280,7 +280,7 @@ int panel_cluster_max_ctas(neb_ctx* c) {
 
 int64_t panel_cluster_max_rows(neb_ctx* c) { return (int64_t)panel_cluster_max_ctas(c) * PC_THREADS; }
 
-neb_status panel_cluster_launch(neb_ctx* c, int64_t k) {
+neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream) {
   const int64_t mrows = c->npad - k;
   int cs = 1;
   while ((int64_t)cs * PC_THREADS < mrows) cs <<= 1;
@@ -288,7 +288,7 @@ neb_status panel_cluster_launch(neb_ctx* c, int64_t k) {
   cfg.gridDim = dim3(cs);
   cfg.blockDim = dim3(PC_THREADS);
   cfg.dynamicSmemBytes = sizeof(PcSmem);
-  cfg.stream = c->stream;
+  cfg.stream = stream;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;

@@ -448,7 +448,7 @@ def test_edge_cases_and_errors(nb, P, orc):
     assert e.value.status == 1
 
 
-def test_lu_panel_kernels_agree(nb, orc):
+def test_lu_panel_kernels_agree(nb, orc, P):
     """The cluster/DSMEM panel kernel (default where the panel fits) and the grid-wide cooperative one give
     the same pivots, hence the same sigma; a matrix that needs many row exchanges exercises both."""
     pr = W.random_elements(700, seed=21, kinds=(W.RECT, W.TRI), dielectric_fraction=0.5, size_mm=(0.05, 0.3))
@@ -461,6 +461,14 @@ def test_lu_panel_kernels_agree(nb, orc):
         sig[mode] = nb.solve()
         assert np.max(np.abs(sig[mode] - so)) <= TOL_SIGMA * np.max(np.abs(so)), mode
     assert np.max(np.abs(sig[0] - sig[1])) <= 1e-12 * np.max(np.abs(so))
+    # look-ahead (panel k+1 on the side stream while panel k's trailing update runs) only reorders launches:
+    # the arithmetic is the same, so sigma is bit-identical with and without it
+    nb.set_option(3, 0)
+    nb.set_option(P.binding.NEB_OPT_LU_LOOKAHEAD, 0)
+    nb.assemble_problem(pr)
+    s_serial = nb.solve()
+    nb.set_option(P.binding.NEB_OPT_LU_LOOKAHEAD, 1)
+    assert np.array_equal(s_serial, sig[0])
 
 
 def test_host_and_device_pointers_agree(nb):
