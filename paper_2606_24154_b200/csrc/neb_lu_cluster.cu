@@ -10,8 +10,13 @@
 // registers.  Pivoting is implicit: rows never move, each thread tracks the POSITION its row currently
 // occupies (`pos`), which reproduces LAPACK's sequential row exchanges exactly (ipiv[dr] = position of
 // the winner at that time; ties -> lowest position).  Per column: warp argmax -> the winning lane publishes
-// its row in shared memory -> CTA candidate -> cluster barrier -> every CTA reads the 16 candidates and
-// the winner's row through DSMEM -> rank-1 update in registers.  Between the two 32-column halves the
+// its row in shared memory -> warp 0 forms the CTA's candidate and PUSHES it (value, position, row) into the
+// shared memory of every CTA of the cluster (remote stores) -> one cluster barrier (arrive.release /
+// wait.acquire) -> every WARP finds the global winner among the 16 local candidate slots by itself (no second
+// CTA barrier, no remote read on the critical path; letting all 16 x 16 warps read the winner's row remotely was
+// measured slower: 64 KB through one SM's shared-memory port per column) -> rank-1 update in registers.
+// (Starting the next column's search before the rest of the update was also measured slower: the extra live
+// registers spill, and spilled locals miss the L1 after every cluster barrier.)  Between the two 32-column halves the
 // pivot rows are gathered in CTA 0, which solves the 32x32 triangular system for U12; every row then
 // applies the rank-32 update from its own multipliers (stashed in shared memory).  At the end every
 // thread writes its row to its final position.
@@ -32,20 +37,14 @@ constexpr int PC_MAX_CTAS = 16;
 struct PcSmem {
   double L[PC_H][PC_THREADS];         // first-half rows of this CTA's threads: L[c][tid]
   double pub[2][PC_WARPS][PC_H];      // per-warp candidate rows, double-buffered by step parity
+  double crow[2][PC_MAX_CTAS][PC_H];  // candidate row of every CTA of the cluster (pushed by its warp 0), by parity
+  unsigned long long cval[2][PC_MAX_CTAS];   // |value| bits of every CTA's candidate
+  int cpos[2][PC_MAX_CTAS];           // its position (INT_MAX: that CTA has no row left)
   double U[PC_H][PC_H];               // local copy of U12
   double Lp[PC_H][PC_H + 1];          // CTA 0: gathered pivot rows, first half (unit lower L11 / U11)
   double Bp[PC_H][PC_H + 1];          // CTA 0: gathered pivot rows, second half -> U12
-  double prow[PC_H];                  // winner row of the current column
-  unsigned whi[PC_WARPS], wlo[PC_WARPS];   // per-warp candidates: |value| bits and position
-  int wpos[PC_WARPS];
-  unsigned chi[2], clo[2];            // this CTA's candidate, by parity
-  int cpos[2];
-  int cwarp[2];
-  double invp;
-  int win_pos;
-#ifdef NEB_PANEL_TRACE
-  long long dbg[12];
-#endif
+  unsigned whi[2][PC_WARPS], wlo[2][PC_WARPS];   // per-warp candidates by parity: |value| bits and position
+  int wpos[2][PC_WARPS];
 };
 
 // Warp-wide argmax of (|value|, lowest position) with three REDUX.SYNC instead of a 5-round shuffle
@@ -82,15 +81,18 @@ __device__ __forceinline__ double pivot_rcp(double x) {
 // them alone; after 32/PC_BS blocks the window is back in natural order.
 constexpr int PC_BS = 4;
 #ifdef NEB_PANEL_TRACE
-#define PC_MARK(id) do { if (tid == 0 && rank == 0 && dr0 == 0 && (j == 9 || j == 10)) { sm.dbg[id] = clock64(); if (id == 8) { for (int q_ = 1; q_ < 9; ++q_) printf("j %d mark %d +%lld\n", j, q_, sm.dbg[q_] - sm.dbg[q_ - 1]); } } } while (0)
+#define PC_MARK(i) do { if (tid == 0) { long long t_ = clock64(); tr[i] += t_ - tl; tl = t_; } } while (0)
 #else
-#define PC_MARK(id)
+#define PC_MARK(i)
 #endif
 __device__ __forceinline__ void factor_half(double (&a)[PC_H], int& pos, bool valid, int64_t dr0, PcSmem& sm,
                                             cg::cluster_group& cluster, int ncta, int32_t* __restrict__ ipiv,
                                             int32_t* __restrict__ flag) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned rank = cluster.block_rank();
+#ifdef NEB_PANEL_TRACE
+  long long tr[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tl = clock64();
+#endif
 #pragma unroll 1
   for (int blk = 0; blk < PC_H / PC_BS; ++blk) {
     const int width = PC_H - blk * PC_BS;          // live columns of the window: indices 0 .. width-1
@@ -99,7 +101,6 @@ __device__ __forceinline__ void factor_half(double (&a)[PC_H], int& pos, bool va
       const int j = blk * PC_BS + jj;
       const int par = j & 1;
       const int dr = (int)dr0 + j;
-      PC_MARK(0);
       const bool act = valid && pos >= dr;
       double v = fabs(a[jj]);
       if (!(v == v)) v = 0.0;                      // NaN never wins; caught by the zero-pivot test
@@ -110,64 +111,64 @@ __device__ __forceinline__ void factor_half(double (&a)[PC_H], int& pos, bool va
 #pragma unroll
         for (int c = jj; c < PC_H; ++c) sm.pub[par][warp][c] = a[c];
       }
-      if (lane == 0) { sm.whi[warp] = mh; sm.wlo[warp] = ml; sm.wpos[warp] = mp; }
-      PC_MARK(1);
+      if (lane == 0) { sm.whi[par][warp] = mh; sm.wlo[par][warp] = ml; sm.wpos[par][warp] = mp; }
+      PC_MARK(0);
       __syncthreads();
-      PC_MARK(2);
+      PC_MARK(1);
       if (warp == 0) {
+        // the CTA's candidate (value, position, row), pushed into every CTA of the cluster (its own included)
         const bool in = lane < PC_WARPS;
-        const unsigned h = in ? sm.whi[lane] : 0u, l = in ? sm.wlo[lane] : 0u;
-        const int p = in ? sm.wpos[lane] : 0x7fffffff;
+        const unsigned h = in ? sm.whi[par][lane] : 0u, l = in ? sm.wlo[par][lane] : 0u;
+        const int p = in ? sm.wpos[par][lane] : 0x7fffffff;
         unsigned ch, cl;
         int cp;
         warp_argmax(h, l, p, ch, cl, cp);
         const unsigned who = __ballot_sync(0xffffffffu, in && p == cp && p != 0x7fffffff);
-        if (lane == 0) { sm.chi[par] = ch; sm.clo[par] = cl; sm.cpos[par] = cp; sm.cwarp[par] = who ? __ffs(who) - 1 : 0; }
-      }
-      PC_MARK(3);
-      cluster.sync();
-      PC_MARK(4);
-      if (warp == 0) {
-        unsigned h = 0u, l = 0u;
-        int p = 0x7fffffff, w = 0;
+        const int cw = who ? __ffs(who) - 1 : 0;
+        // finished columns (rotated to the tail of the window) and unused ones carry 0: the update skips them
+        const double x = (lane >= jj && lane < width && cp != 0x7fffffff) ? sm.pub[par][cw][lane] : 0.0;
+        for (int r = 0; r < ncta; ++r) cluster.map_shared_rank(&sm, r)->crow[par][rank][lane] = x;
         if (lane < ncta) {
-          const PcSmem* rs = cluster.map_shared_rank(&sm, lane);
-          h = rs->chi[par]; l = rs->clo[par]; p = rs->cpos[par]; w = rs->cwarp[par];
-        }
-        unsigned gh, gl;
-        int gp;
-        warp_argmax(h, l, p, gh, gl, gp);
-        const bool any = gp != 0x7fffffff;
-        const unsigned who = __ballot_sync(0xffffffffu, any && p == gp);
-        const int gc = who ? __ffs(who) - 1 : 0;
-        const int gw = __shfl_sync(0xffffffffu, w, gc);
-        PC_MARK(5);
-        const PcSmem* ws = cluster.map_shared_rank(&sm, gc);
-        double x = (lane >= jj && lane < width && any) ? ws->pub[par][gw][lane] : 0.0;
-        sm.prow[lane] = x;
-        double piv = __shfl_sync(0xffffffffu, x, jj);
-        if (lane == 0) {
-          sm.win_pos = any ? gp : dr;
-          sm.invp = pivot_rcp(piv);
-          if (rank == 0) {
-            ipiv[dr] = any ? gp : dr;
-            if (!any || !(fabs(piv) > 0.0)) atomicOr(flag, 2);
-          }
+          PcSmem* rs = cluster.map_shared_rank(&sm, lane);
+          rs->cval[par][rank] = ((unsigned long long)ch << 32) | cl;
+          rs->cpos[par][rank] = cp;
         }
       }
-      PC_MARK(6);
-      __syncthreads();
-      PC_MARK(7);
-      const int wp = sm.win_pos;
-      const double invp = sm.invp;
+      PC_MARK(2);
+      cluster.barrier_arrive();                    // release: the pushes above are visible after the wait
+      PC_MARK(3);
+      cluster.barrier_wait();
+      PC_MARK(4);
+      // every warp picks the global winner from its CTA's own copy of the candidates
+      unsigned h = 0u, l = 0u;
+      int p = 0x7fffffff;
+      if (lane < ncta) {
+        const unsigned long long cv = sm.cval[par][lane];
+        h = (unsigned)(cv >> 32); l = (unsigned)cv; p = sm.cpos[par][lane];
+      }
+      unsigned gh, gl;
+      int gp;
+      warp_argmax(h, l, p, gh, gl, gp);
+      const bool any = gp != 0x7fffffff;
+      const unsigned gwho = __ballot_sync(0xffffffffu, any && p == gp);
+      const int gc = gwho ? __ffs(gwho) - 1 : 0;
+      const double* prow = sm.crow[par][gc];
+      const double piv = prow[jj];
+      const double invp = pivot_rcp(piv);
+      const int wp = any ? gp : dr;
+      if (rank == 0 && tid == 0) {
+        ipiv[dr] = wp;
+        if (!any || !(fabs(piv) > 0.0)) atomicOr(flag, 2);
+      }
+      PC_MARK(5);
       pos = (pos == dr) ? wp : ((pos == wp) ? dr : pos);
       if (valid && pos > dr) {
-        const double l = a[jj] * invp;
-        a[jj] = l;
+        const double lmul = a[jj] * invp;
+        a[jj] = lmul;
 #pragma unroll
-        for (int c = jj + 1; c < PC_H; ++c) a[c] = fma(-l, sm.prow[c], a[c]);
+        for (int c = jj + 1; c < PC_H; ++c) a[c] = fma(-lmul, prow[c], a[c]);
       }
-      PC_MARK(8);
+      PC_MARK(6);
     }
     // rotate the window by PC_BS: finished columns go to the tail
     double t[PC_BS];
@@ -177,7 +178,13 @@ __device__ __forceinline__ void factor_half(double (&a)[PC_H], int& pos, bool va
     for (int c = 0; c < PC_H - PC_BS; ++c) a[c] = a[c + PC_BS];
 #pragma unroll
     for (int c = 0; c < PC_BS; ++c) a[PC_H - PC_BS + c] = t[c];
+    PC_MARK(7);
   }
+#ifdef NEB_PANEL_TRACE
+  if (tid == 0 && dr0 == 0)
+    printf("rank %u: argmax+pub %lld sync %lld cta+push %lld arrive %lld wait %lld global %lld update %lld rotate %lld (cycles, 32 columns)\n",
+           rank, tr[0], tr[1], tr[2], tr[3], tr[4], tr[5], tr[6], tr[7]);
+#endif
 }
 
 __global__ void __launch_bounds__(PC_THREADS, 1) panel_cluster_kernel(double* __restrict__ A, int64_t ld, int64_t npad,
