@@ -192,40 +192,55 @@ __global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, cons
   }
 }
 
-// U12 = L11^-1 A12: rows [k, k+NB), columns [k+NB, npad).  CTA = 256 threads on a slab of 64 columns.
-// Thread (c = tid & 63, q = tid >> 6) keeps rows q, q+4, ..., q+60 of column c in registers; at step j the
-// owner of row j broadcasts x_j through shared memory (double-buffered: one barrier per step) and every
-// thread updates its rows below j with L11 read from shared memory (warp-uniform address: broadcast).
-constexpr int TRSM_THREADS = 256;
-constexpr size_t TRSM_SMEM = (size_t)(NB * (NB + 1) + 2 * NB) * sizeof(double);
+// U12 = L11^-1 A12: rows [k, k+NB), columns [c_first + 64 b, c_first + 64 (b+1)) for CTA b.  One THREAD per column,
+// the whole column (64 rows) in registers: no barrier inside the 63 dependent steps.  The substitution runs as 16
+// rolled iterations of 4 steps on a register WINDOW that is rotated by 4 rows per iteration (static register indices,
+// a loop body that stays in the instruction cache; the fully unrolled form was fetch-bound).  L11 sits in shared
+// memory column-major with 64 rows of zeros below it, so window rows past the block's end are left alone.
+constexpr int TRSM_THREADS = NB;
+constexpr int TRSM_LD = 2 * NB;
+constexpr size_t TRSM_SMEM = (size_t)NB * TRSM_LD * sizeof(double);
 __global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t c_first) {
-  extern __shared__ double s_trsm[];
-  double(*sL)[NB + 1] = reinterpret_cast<double(*)[NB + 1]>(s_trsm);     // sL[i][j] = L11[i][j]
-  double* sX = s_trsm + NB * (NB + 1);                                    // sX[(j & 1) * NB + c]
-  const int tid = threadIdx.x, c = tid & (NB - 1), q = tid >> 6;         // q = 0..3
-  const int64_t c0 = c_first + (int64_t)blockIdx.x * NB;
-  for (int j = q; j < NB; j += 4) sL[c][j] = A[(k + c) + (k + j) * ld];
-  double x[NB / 4];
-  // column c of the slab: rows q + 4t.  Loaded through shared memory would be coalesced; direct loads hit
-  // whole 32-byte sectors across the 4 row groups of a column, which the L2 absorbs.
+  extern __shared__ __align__(16) double s_trsm[];             // s_trsm[j * TRSM_LD + i] = L11[i][j], 0 for i >= NB
+  const int tid = threadIdx.x;
+  double* col = A + k + (c_first + (int64_t)blockIdx.x * NB + tid) * ld;
+  double x[NB];
+  {
+    // thread j stages column j of L11: 32 independent 16-byte loads in flight (a rolled element loop over 64
+    // threads would pay one L2 round trip per element)
+    const double* lcol = A + k + (k + tid) * ld;
 #pragma unroll
-  for (int t = 0; t < NB / 4; ++t) x[t] = A[(k + q + 4 * t) + (c0 + c) * ld];
-  __syncthreads();
+    for (int i = 0; i < NB; i += 2) {
+      const double2 v = *reinterpret_cast<const double2*>(lcol + i);
+      x[i] = v.x; x[i + 1] = v.y;
+    }
 #pragma unroll
-  for (int j = 0; j < NB - 1; ++j) {
-    if (q == (j & 3)) sX[(j & 1) * NB + c] = x[j >> 2];
-    __syncthreads();
-    const double xj = sX[(j & 1) * NB + c];
-#pragma unroll
-    for (int t = 0; t < NB / 4; ++t) {
-      if (4 * t + 3 > j) {                       // some row of this group may lie below j (compile-time prune)
-        const int i = q + 4 * t;
-        if (i > j) x[t] = fma(-sL[i][j], xj, x[t]);
-      }
+    for (int i = 0; i < NB; i += 2) {
+      *reinterpret_cast<double2*>(s_trsm + tid * TRSM_LD + i) = make_double2(x[i], x[i + 1]);
+      *reinterpret_cast<double2*>(s_trsm + tid * TRSM_LD + NB + i) = make_double2(0.0, 0.0);
     }
   }
 #pragma unroll
-  for (int t = 0; t < NB / 4; ++t) A[(k + q + 4 * t) + (c0 + c) * ld] = x[t];
+  for (int i = 0; i < NB; i += 2) {
+    const double2 v = *reinterpret_cast<const double2*>(col + i);
+    x[i] = v.x; x[i + 1] = v.y;
+  }
+  __syncthreads();
+#pragma unroll 1
+  for (int it = 0; it < NB / 4; ++it) {
+    const double* Lw = s_trsm + (it * 4) * TRSM_LD + it * 4;    // Lw[b * TRSM_LD + a] = L11[j0 + a][j0 + b], j0 = 4 it
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const double xj = x[b];
+#pragma unroll
+      for (int a = b + 1; a < NB; ++a) x[a] = fma(-Lw[b * TRSM_LD + a], xj, x[a]);
+    }
+    *reinterpret_cast<double2*>(col + it * 4) = make_double2(x[0], x[1]);
+    *reinterpret_cast<double2*>(col + it * 4 + 2) = make_double2(x[2], x[3]);
+#pragma unroll
+    for (int a = 0; a < NB - 4; ++a) x[a] = x[a + 4];
+    x[NB - 4] = 0.0; x[NB - 3] = 0.0; x[NB - 2] = 0.0; x[NB - 1] = 0.0;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
