@@ -332,6 +332,73 @@ def test_c2_thgem_full_size_sampled(nb, orc):
     assert phi.min() > -2000.0 - 20.0 and phi.max() < 20.0
 
 
+def _rows_geometry(orc, g, rows):
+    """The oracle's view of a few collocation rows (for orc.rhs on sampled rows)."""
+    gs = object.__new__(orc.Geometry)
+    gs.n = int(rows.size)
+    for name in ("e1", "e2", "colloc"):
+        setattr(gs, name, np.ascontiguousarray(getattr(g, name)[:, rows]))
+    gs.bc_kind = np.ascontiguousarray(g.bc_kind[rows])
+    gs.bc_value = np.ascontiguousarray(g.bc_value[rows])
+    return gs
+
+
+def test_c3_c4_full_size_sampled(nb, orc):
+    """BASELINE configs[3] and [4] at FULL size on one GPU: N = 49928 panels with 5x5 image copies (fp64 matrix
+    of 20 GB, 6.2e10 pair evaluations), LU, then (C3) a 2e5-point slab of the 1e7 seeded points and (C4) one
+    step of the space-charge loop with all 1e6 charges: E at the charges from the panels and from all other
+    charges, push, RHS update, re-solve on the resident factors.  The oracle cannot factor 50k x 50k in test
+    time, so parity is (a) the residual of the GPU sigma against ORACLE-computed matrix rows and right-hand
+    sides on sampled rows and (b) Phi/E on sampled points / charges."""
+    import torch
+    if torch.cuda.get_device_properties(0).total_memory < 60e9:
+        pytest.skip("needs ~25 GB of device memory")
+    pr = W.space_charge(W.double_thgem())
+    assert pr.n > 45000 and pr.n_img == 25 and pr.points.shape[1] == 10_000_000 and pr.charge_q.shape[0] == 1_000_000
+    g = orc.Geometry(pr)
+    rs = np.random.RandomState(34)
+    rows = rs.choice(pr.n, 16, replace=False)
+    R, Cc = np.repeat(rows, pr.n), np.tile(np.arange(pr.n), rows.size)
+    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)
+    gs = _rows_geometry(orc, g, rows)
+    # ---- C3: assemble, factor, solve, evaluate
+    nb.assemble_problem(pr)
+    s = nb.solve()
+    res = np.abs(Krows @ s - orc.rhs(gs, mode="f64")) / (np.abs(Krows).sum(axis=1) * np.abs(s).max())
+    assert res.max() <= 1e-12
+    m = 200_000
+    pts = torch.from_numpy(np.ascontiguousarray(pr.points[:, :m])).cuda()
+    phi, E = nb.eval(pts)
+    phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    idx = rs.choice(m, 32, replace=False)
+    phi_o, E_o = orc.evaluate(g, s, pr.points[:, idx], mode="ld")
+    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C3 sampled")
+    assert phi.min() > -2000.0 - 40.0 and phi.max() < 40.0       # maximum principle up to the mesh error
+    # ---- C4: one full-size step on the resident factors
+    pos = torch.from_numpy(pr.charge_pos.copy()).cuda()
+    ch = torch.from_numpy(pr.charge_q).cuda()
+    nb.add_space_charge(pos, ch)
+    s1 = nb.solve()
+    b1 = orc.rhs(gs, pr.charge_pos, pr.charge_q, mode="f64")
+    assert np.max(np.abs(nb.get_rhs()[rows] - b1) / np.maximum(np.abs(b1), 1e-6 * np.abs(b1).max())) <= TOL_FAR
+    res = np.abs(Krows @ s1 - b1) / (np.abs(Krows).sum(axis=1) * np.abs(s1).max())
+    assert res.max() <= 1e-12
+    assert np.max(np.abs(s1 - s)) > 0.0                          # the charges changed the right-hand side
+    _, Eq = nb.eval(pos, want_phi=False)                         # 1.25e12 element pairs + 1e12 charge pairs
+    cidx = rs.choice(pr.charge_q.shape[0], 16, replace=False)
+    _, Eq_o = orc.evaluate(g, s1, pr.charge_pos[:, cidx], pr.charge_pos, pr.charge_q, mode="ld")
+    assert vec_rel_err(Eq.cpu().numpy()[:, cidx], Eq_o).max() <= TOL_FAR
+    mu_dt = pr.meta["mu"] * pr.meta["dt"]
+    nb.push(pos, Eq, mu_dt)
+    pos_o = orc.push(pr.charge_pos[:, cidx], Eq_o, pr.meta["mu"], pr.meta["dt"])
+    assert np.max(np.abs(pos.cpu().numpy()[:, cidx] - pos_o)) <= 1e-12 * np.max(np.abs(pos_o))
+    nb.add_space_charge(pos, ch, replace=True)
+    s2 = nb.solve()
+    b2 = orc.rhs(gs, pos.cpu().numpy(), pr.charge_q, mode="f64")
+    res = np.abs(Krows @ s2 - b2) / (np.abs(Krows).sum(axis=1) * np.abs(s2).max())
+    assert res.max() <= 1e-12
+
+
 # ---------------------------------------------------------------------------------------------
 # a4 / a8 / a9: space charge, RHS, re-solve on resident factors, push
 # ---------------------------------------------------------------------------------------------
