@@ -37,9 +37,35 @@ UNIT = "pairs/s"
 # 206 instructions); right triangle 232 flop; wire 139; point charge 30
 FLOP_PER_PAIR = {"rect": 279.0, "tri": 232.0, "wire": 139.0, "charge": 30.0}
 FP64_INSTR_PER_PAIR = {"rect": 167.0}
-CONFIG = {"workload": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
-          "n_elements": 6144, "m_points": 100000, "step": "assemble+solve(LU)+eval",
-          "l2": "256 MiB buffer written between timed steps; matrix (302 MB) exceeds L2"}
+L2_NOTE = "256 MiB buffer written between timed steps; the matrix exceeds L2"
+WORKLOADS = {
+    "C1": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
+    "C2": "C2 THGEM cell: rectangles + right triangles, dielectric rows, 100^3 grid (BASELINE configs[2])",
+    "C3": "C3 double THGEM: 5x5 image copies, points uniform in the cell (BASELINE configs[3])",
+    "C4": "C4 space charge on the C3 geometry: per step E at the charges (panels + all other charges), push, "
+          "RHS update, re-solve on the resident LU factors (BASELINE configs[4]); assembly + LU done once before",
+}
+
+
+def make_config(name, pr, m, q=0):
+    cfg = {"workload": WORKLOADS[name], "n_elements": int(pr.n), "m_points": int(m), "image_copies": int(max(1, pr.n_img)),
+           "step": "assemble+solve(LU)+eval" if name != "C4" else "eval(charges)+push+rhs+re-solve", "l2": L2_NOTE}
+    if q:
+        cfg["charges"] = int(q)
+    return cfg
+
+
+def load_problem(name, m_cap=None, seed_shift=0):
+    from workloads import configs as W
+    if name == "C1":
+        return W.cube(seed=1 + seed_shift)
+    if name == "C2":
+        return W.thgem()
+    if name == "C3":
+        return W.double_thgem(m_points=m_cap or 10_000_000, seed=3 + seed_shift)
+    if name == "C4":
+        return W.space_charge(W.double_thgem(m_points=0), q_count=m_cap or 1_000_000, seed=4 + seed_shift)
+    raise SystemExit(f"unknown workload {name}")
 
 
 class ClockSampler:
@@ -81,43 +107,57 @@ def _clocks_summary(samples):
             "reasons": reasons}
 
 
-def cpu_baseline_run(pr, n_rows=1024, n_pts=20000):
-    """The oracle as it stands (fp64 build, OpenMP on every host core) on a bounded sample of C1."""
+def cpu_baseline_run(pr, n_rows=None, n_pts=None, with_lu=False):
+    """The oracle as it stands (fp64 build, OpenMP on every host core): assembly rows 0..n_rows-1 and the first
+    n_pts points (None = all); with_lu also factorises and solves, i.e. the whole step."""
     import oracle
     g = oracle.Geometry(pr)
-    rows = np.repeat(np.arange(n_rows), pr.n)
-    cols = np.tile(np.arange(pr.n), n_rows)
-    sig = np.full(pr.n, 1e-8)
+    m = pr.points.shape[1]
+    n_rows = pr.n if n_rows is None else min(n_rows, pr.n)
+    n_pts = m if n_pts is None else min(n_pts, m)
+    copies = max(1, pr.n_img)
     t0 = time.perf_counter()
-    oracle.matrix_entries(g, rows, cols, mode="f64")
+    if with_lu:
+        K = oracle.assemble(g, mode="f64")
+        sig = oracle.solve(K, oracle.rhs(g, mode="f64"), mode="f64")
+        n_rows = pr.n
+    else:
+        rows = np.repeat(np.arange(n_rows), pr.n)
+        cols = np.tile(np.arange(pr.n), n_rows)
+        sig = np.full(pr.n, 1e-8)
+        oracle.matrix_entries(g, rows, cols, mode="f64")
     oracle.evaluate(g, sig, pr.points[:, :n_pts], mode="f64")
     dt = time.perf_counter() - t0
-    pairs = n_rows * pr.n + n_pts * pr.n
+    pairs = copies * (n_rows * pr.n + n_pts * pr.n)
+    what = (f"the whole step: assembly {pr.n}x{pr.n}, LU solve, eval at all {n_pts} points" if with_lu and n_pts == m else
+            f"assembly rows 0..{n_rows - 1} ({n_rows}x{pr.n}x{copies} pairs) + eval of the first {n_pts} points "
+            f"({n_pts}x{pr.n}x{copies} pairs)" + (", LU solve included" if with_lu else "; LU not sampled"))
     return {"value": pairs / dt, "unit": UNIT, "cores": oracle.threads("f64"), "kind": "oracle",
-            "sample": f"assembly rows 0..{n_rows - 1} ({n_rows}x{pr.n} pairs) + eval of the first {n_pts} points "
-                      f"({n_pts}x{pr.n} pairs) of C1, fp64 build, gcc -O2 -fopenmp; LU not sampled", "seconds": dt}
+            "sample": what + "; fp64 build, gcc -O2 -fopenmp", "seconds": dt}
 
 
 def run_reference(args):
+    """Reference arm = the oracle (there is no reference code): rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from workloads import configs as W
-    pr = W.cube()
-    n_rows, n_pts = 256, 4000
+    pr = load_problem(args.workload, args.m_points)
+    copies = max(1, pr.n_img)
+    n_rows, n_pts = max(1, 1024 // copies), max(1, 20000 // copies)
     for _ in range(args.warmup):
-        cpu_baseline_run(pr, 32, 200)
+        cpu_baseline_run(pr, max(1, n_rows // 32), max(1, n_pts // 100))
     t = []
     base = None
     for _ in range(args.steps):
         base = cpu_baseline_run(pr, n_rows, n_pts)
         t.append(base["seconds"])
-    pairs = n_rows * pr.n + n_pts * pr.n
+    pairs = copies * (min(n_rows, pr.n) * pr.n + min(n_pts, pr.points.shape[1]) * pr.n)
     value = pairs * len(t) / sum(t)
     base["value"] = value
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * sum(t) / len(t), "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": CONFIG, "cpu_baseline": base,
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": make_config(args.workload, pr, pr.points.shape[1]), "cpu_baseline": base,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
@@ -128,11 +168,15 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours")
+    ap.add_argument("--workload", default="C1", choices=sorted(WORKLOADS),
+                    help="C1 is the bench line; C2..C4 are one-off full-size runs recorded under profiles/")
+    ap.add_argument("--m-points", type=int, default=None, help="cap on the evaluation points (C3) / charges (C4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    args.warmup = max(args.warmup, 3)
+    if args.workload == "C1":
+        args.warmup = max(args.warmup, 3)          # the bench line; C2..C4 one-off runs may use fewer (long steps)
 
     import torch
     import torch.distributed as dist
@@ -148,40 +192,81 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    pr = W.cube(seed=1 + rank)                     # same geometry on every rank, its own points
-    n, m = pr.n, pr.points.shape[1]
-    pairs_step = n * n + m * n
+    name = args.workload
+    pr = load_problem(name, args.m_points, seed_shift=rank)   # same geometry on every rank, its own points / charges
+    is_c4 = name == "C4"
+    pts_np = pr.charge_pos if is_c4 else pr.points
+    n, m = pr.n, pts_np.shape[1]
+    copies = max(1, pr.n_img)
+    q = m if is_c4 else 0
+    # pair evaluations per step (image copies count as pairs; C4: + charge-charge and charge-collocation pairs)
+    pairs_step = copies * m * n + (q * q + n * q if is_c4 else copies * n * n)
     nb = P.Neb(local)
 
     def t_dev(a, dtype):
-        return torch.from_numpy(np.ascontiguousarray(a)).to(dtype).to(dev)
+        return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dtype).to(dev)
 
-    d = dict(kind=t_dev(pr.kind, torch.int32), v0=t_dev(pr.v0, torch.float64), e1=t_dev(pr.e1, torch.float64),
-             e2=t_dev(pr.e2, torch.float64), bc_kind=t_dev(pr.bc_kind, torch.int32), bc_value=t_dev(pr.bc_value, torch.float64))
-    d_pts = t_dev(pr.points, torch.float64)
+    def pin(a):
+        return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+
+    geo = dict(kind=(pr.kind, torch.int32), v0=(pr.v0, torch.float64), e1=(pr.e1, torch.float64), e2=(pr.e2, torch.float64),
+               bc_kind=(pr.bc_kind, torch.int32), bc_value=(pr.bc_value, torch.float64), radius=(pr.radius, torch.float64),
+               eps_plus=(pr.eps_plus, torch.float64), eps_minus=(pr.eps_minus, torch.float64),
+               img_shift=(pr.img_shift, torch.float64))
+    d = {k: t_dev(a, t) for k, (a, t) in geo.items()}
+    h = {k: pin(None if a is None else np.asarray(a).astype(np.int32 if t == torch.int32 else np.float64))
+         for k, (a, t) in geo.items()}
+    d_pts = t_dev(pts_np, torch.float64)
     d_sig = torch.empty(n, dtype=torch.float64, device=dev)
     d_phi = torch.empty(m, dtype=torch.float64, device=dev)
     d_E = torch.empty((3, m), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
-    def step_resident():
-        nb.assemble(d["kind"], d["v0"], d["e1"], d["e2"], d["bc_kind"], d["bc_value"])
-        nb.solve(out=d_sig)
-        nb.eval(d_pts, phi=d_phi, E=d_E)
-
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    h = dict(kind=pin(pr.kind), v0=pin(pr.v0), e1=pin(pr.e1), e2=pin(pr.e2), bc_kind=pin(pr.bc_kind), bc_value=pin(pr.bc_value))
-    h_pts = pin(pr.points)
+    h_pts = pin(pts_np)
     h_sig = torch.empty(n, dtype=torch.float64).pin_memory()
     h_phi = torch.empty(m, dtype=torch.float64).pin_memory()
     h_E = torch.empty((3, m), dtype=torch.float64).pin_memory()
-    h2d = sum(v.numel() * v.element_size() for v in h.values()) + h_pts.numel() * 8
-    d2h = (h_sig.numel() + h_phi.numel() + h_E.numel()) * 8
 
-    def step_e2e():
-        nb.assemble(h["kind"], h["v0"], h["e1"], h["e2"], h["bc_kind"], h["bc_value"])
-        nb.solve(out=h_sig)
-        nb.eval(h_pts, phi=h_phi, E=h_E)
+    def assemble_from(a):
+        nb.assemble(a["kind"], a["v0"], a["e1"], a["e2"], a["bc_kind"], a["bc_value"], radius=a["radius"],
+                    eps_plus=a["eps_plus"], eps_minus=a["eps_minus"], img_shift=a["img_shift"])
+
+    if not is_c4:
+        def step_resident():
+            assemble_from(d)
+            nb.solve(out=d_sig)
+            nb.eval(d_pts, phi=d_phi, E=d_E)
+
+        def step_e2e():
+            assemble_from(h)
+            nb.solve(out=h_sig)
+            nb.eval(h_pts, phi=h_phi, E=h_E)
+
+        h2d = sum(v.numel() * v.element_size() for v in h.values() if v is not None) + h_pts.numel() * 8
+        d2h = (h_sig.numel() + h_phi.numel() + h_E.numel()) * 8
+    else:
+        # C4 (reading S22): geometry assembled and factorised ONCE, outside the timed steps; a step is one pass
+        # of the self-consistent loop with all charges
+        mu_dt = pr.meta["mu"] * pr.meta["dt"]
+        d_ch = t_dev(pr.charge_q, torch.float64)
+        h_ch = pin(pr.charge_q)
+        assemble_from(d)
+        nb.add_space_charge(d_pts, d_ch)
+        nb.solve(out=d_sig)
+
+        def step_resident():
+            nb.eval(d_pts, E=d_E, want_phi=False)
+            nb.push(d_pts, d_E, mu_dt)
+            nb.add_space_charge(d_pts, d_ch, replace=True)
+            nb.solve(out=d_sig)
+
+        def step_e2e():
+            nb.eval(h_pts, E=h_E, want_phi=False)
+            nb.push(h_pts, h_E, mu_dt)
+            nb.add_space_charge(h_pts, h_ch, replace=True)
+            nb.solve(out=h_sig)
+
+        h2d = (3 * m + 3 * m + 3 * m + 3 * m + m) * 8          # points for eval, pos+E for push, pos+q for the charges
+        d2h = (3 * m + 3 * m + n) * 8                          # E, pushed positions, sigma
 
     def barrier():
         if world > 1:
@@ -219,7 +304,7 @@ def main():
     nb.reset_stats()
     for _ in range(args.steps):
         flush.fill_(1)
-        nb.eval(d_pts, phi=d_phi, E=d_E)
+        nb.eval(d_pts, phi=None if is_c4 else d_phi, E=d_E, want_phi=not is_c4)
     st = nb.stage_ms()
     eval_ms = st["eval"][0] / max(1, st["eval"][1])
     nb.reset_stats()
@@ -237,8 +322,10 @@ def main():
     nb.set_option(P.binding.NEB_OPT_LU_LOOKAHEAD, 1)
     nb.set_option(P.binding.NEB_OPT_PROFILE, 0)
     dfma_peak, dmma_peak = nb.fp64_peak(0), nb.fp64_peak(1)
-    flop_eval = FLOP_PER_PAIR["rect"] * m * n
-    achieved = flop_eval / (eval_ms * 1e-3) * 1e-12
+    n_tri, n_wire = int(np.sum(pr.kind == 1)), int(np.sum(pr.kind == 2))
+    flop_pair = (FLOP_PER_PAIR["rect"] * (n - n_tri - n_wire) + FLOP_PER_PAIR["tri"] * n_tri + FLOP_PER_PAIR["wire"] * n_wire) / n
+    eval_pairs = copies * m * n
+    achieved = flop_pair * eval_pairs / (eval_ms * 1e-3) * 1e-12
     lu_flop = 2.0 / 3.0 * n ** 3
 
     if rank == 0:
@@ -246,7 +333,7 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": CONFIG,
+            "dtype": "f64", "data": "synthetic", "config": make_config(name, pr, m, q),
             "e2e": {"value": pairs_step * args.steps * world / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": launches, "clocks": _clocks_summary(samples),
@@ -254,9 +341,10 @@ def main():
                          "unit": "TFLOP/s", "frac": achieved / dfma_peak, "traffic": None,
                          "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process "
                                         "(nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2)",
-                         "flop_per_pair": FLOP_PER_PAIR["rect"], "kernel_ms": eval_ms,
-                         "fp64_pipe_slot_frac": FP64_INSTR_PER_PAIR["rect"] * m * n / (eval_ms * 1e-3) / (0.5e12 * dfma_peak),
-                         "pairs_per_s_kernel": m * n / (eval_ms * 1e-3),
+                         "flop_per_pair": flop_pair, "kernel_ms": eval_ms,
+                         "fp64_pipe_slot_frac": (FP64_INSTR_PER_PAIR["rect"] * eval_pairs / (eval_ms * 1e-3) / (0.5e12 * dfma_peak)
+                                                 if n_tri + n_wire == 0 else None),
+                         "pairs_per_s_kernel": eval_pairs / (eval_ms * 1e-3),
                          "field_map_points_per_s": m / (eval_ms * 1e-3)},
             "stages_ms": stages,
             "lu": {"tflops_whole_lu": lu_flop / (stages["lu"] * 1e-3) * 1e-12 if stages.get("lu") else None,
@@ -264,7 +352,10 @@ def main():
                    "dmma_peak_tflops": dmma_peak},
         }
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline_run(pr)
+            if name == "C1":
+                line["cpu_baseline"] = cpu_baseline_run(pr, with_lu=True)      # the whole C1 step, LU included
+            elif not is_c4:
+                line["cpu_baseline"] = cpu_baseline_run(pr, max(1, 8192 // copies), max(1, 160000 // copies))
         print(json.dumps(line), flush=True)
     nb.close()
     if world > 1:
