@@ -37,6 +37,10 @@ UNIT = "pairs/s"
 # 206 instructions); right triangle 232 flop; wire 139; point charge 30
 FLOP_PER_PAIR = {"rect": 279.0, "tri": 232.0, "wire": 139.0, "charge": 30.0}
 FP64_INSTR_PER_PAIR = {"rect": 167.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE eval_kernel launch on C1, from the ncu --set full capture
+# summarised in profiles/r1_ncu_full_eval_assemble.md (3.285504 MB + 84.992 kB); algorithmic bytes of that launch:
+# 2.4 MB of points in + 4 x 8 x 1e5 x n_split partial sums out, the 0.8 MB element table from L2
+EVAL_TRAFFIC_C1_BYTES = 3285504 + 84992
 L2_NOTE = "256 MiB buffer written between timed steps; the matrix exceeds L2"
 WORKLOADS = {
     "C1": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
@@ -338,7 +342,8 @@ def main():
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": launches, "clocks": _clocks_summary(samples),
             "roofline": {"bound": "alu", "kernel": "eval_kernel<MathFast> (a7)", "achieved": achieved, "peak": dfma_peak,
-                         "unit": "TFLOP/s", "frac": achieved / dfma_peak, "traffic": None,
+                         "unit": "TFLOP/s", "frac": achieved / dfma_peak,
+                         "traffic": EVAL_TRAFFIC_C1_BYTES if name == "C1" else None,
                          "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process "
                                         "(nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2)",
                          "flop_per_pair": flop_pair, "kernel_ms": eval_ms,
@@ -355,7 +360,8 @@ def main():
             if name == "C1":
                 line["cpu_baseline"] = cpu_baseline_run(pr, with_lu=True)      # the whole C1 step, LU included
             elif not is_c4:
-                line["cpu_baseline"] = cpu_baseline_run(pr, max(1, 8192 // copies), max(1, 160000 // copies))
+                per_unit = n * copies                                          # pairs per assembly row / per point
+                line["cpu_baseline"] = cpu_baseline_run(pr, max(1, int(2e8 // per_unit)), max(1, int(1.8e9 // per_unit)))
         print(json.dumps(line), flush=True)
     nb.close()
     if world > 1:
