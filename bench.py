@@ -34,8 +34,8 @@ UNIT = "pairs/s"
 # FP64 work of one (point, element copy) evaluation of (Phi', E') on the path that >99 % of the pairs of a field
 # map take (warp-uniform far branch), counted in the SASS of eval_kernel<MathFast> (FMA = 2 flop):
 # rectangle 113 DFMA + 38 DMUL + 15 DADD = 279 flop in 167 FP64-pipe instructions (the near branch: 323 flop,
-# 206 instructions); right triangle 232 flop; wire 139; point charge 30
-FLOP_PER_PAIR = {"rect": 279.0, "tri": 232.0, "wire": 139.0, "charge": 30.0}
+# 206 instructions); right triangle 230 flop in 139 instructions; wire 139; point charge 30
+FLOP_PER_PAIR = {"rect": 279.0, "tri": 230.0, "wire": 139.0, "charge": 30.0}
 FP64_INSTR_PER_PAIR = {"rect": 167.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE eval_kernel launch on C1, from the ncu --set full capture
 # summarised in profiles/r1_ncu_full_eval_assemble.md (3.285504 MB + 84.992 kB); algorithmic bytes of that launch:
