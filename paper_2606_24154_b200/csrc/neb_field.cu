@@ -20,51 +20,95 @@ constexpr int kTile = 64;       // elements per shared-memory tile
 constexpr int kChargeTile = 256;
 constexpr int kMaxImg = 32;     // periodic copies kept in shared memory
 
-struct TileSmem {
-  double rec[kRec][kTile];
+// Element tiles are staged by the TMA unit: one thread arms an mbarrier with the tile's byte count and issues one
+// 1-D bulk copy (cp.async.bulk, SASS UBLKCP) per record field (64 elements x 8 bytes, contiguous in the SoA table);
+// the copies land in shared memory asynchronously and complete the mbarrier's transaction count.  Two buffers: tile
+// i+1 is in flight while the CTA evaluates tile i, so the only CTA-wide barrier per tile is the one that hands a
+// fully read buffer back to the producer.
+struct __align__(128) TileSmem {
+  double rec[2][kRec][kTile];
   double img[3][kMaxImg];
+  unsigned long long mbar[2];
 };
+constexpr unsigned kTileBytes = kRec * kTile * sizeof(double);
 
-__device__ __forceinline__ void load_tile(TileSmem& sm, const GeoTables& g, int64_t base, int cnt) {
-  for (int idx = threadIdx.x; idx < kRec * kTile; idx += blockDim.x) {
-    int f = idx / kTile, e = idx % kTile;
-    if (e < cnt) sm.rec[f][e] = g.rec[f * g.stride + base + e];
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void tile_pipe_init(TileSmem& sm) {
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.mbar[0])));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.mbar[1])));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
 }
 
-__device__ __forceinline__ Frame frame_of(const TileSmem& sm, int e) {
+// Thread 0: start the copy of the 64-element window [tb, tb + 64) (tb a multiple of 64; the table's stride is a
+// multiple of 128 and its tail is zero-filled, so every window is in bounds and 16-byte aligned) into buffer seq & 1.
+__device__ __forceinline__ void tile_issue(TileSmem& sm, const GeoTables& g, int64_t tb, unsigned seq) {
+  const unsigned buf = seq & 1u, bar = smem_u32(&sm.mbar[buf]);
+  // the buffer was last READ through the generic proxy (ordered before this point by the CTA barrier): order
+  // those reads before the async-proxy writes
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(kTileBytes) : "memory");
+#pragma unroll
+  for (int f = 0; f < kRec; ++f) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(&sm.rec[buf][f][0])), "l"(g.rec + f * g.stride + tb), "r"((unsigned)(kTile * sizeof(double))), "r"(bar)
+                 : "memory");
+  }
+}
+
+// Every thread: wait until tile seq has landed.  The spin is bounded (each try_wait already blocks for a
+// hardware-defined interval), so that a lost copy ends in a trap instead of a hang.
+__device__ __forceinline__ void tile_wait(TileSmem& sm, unsigned seq) {
+  const unsigned bar = smem_u32(&sm.mbar[seq & 1u]), parity = (seq >> 1) & 1u;
+  unsigned done = 0;
+  int spin = 0;
+  do {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done && ++spin < (1 << 22));
+  if (!done) asm volatile("trap;");
+}
+
+__device__ __forceinline__ Frame frame_of(const TileSmem& sm, unsigned buf, int e) {
   Frame f;
-  f.v0x = sm.rec[0][e]; f.v0y = sm.rec[1][e]; f.v0z = sm.rec[2][e];
-  f.exx = sm.rec[3][e]; f.exy = sm.rec[4][e]; f.exz = sm.rec[5][e];
-  f.eyx = sm.rec[6][e]; f.eyy = sm.rec[7][e]; f.eyz = sm.rec[8][e];
-  f.ezx = sm.rec[9][e]; f.ezy = sm.rec[10][e]; f.ezz = sm.rec[11][e];
-  f.a = sm.rec[12][e]; f.b = sm.rec[13][e]; f.aux = sm.rec[14][e]; f.far2 = sm.rec[16][e];
+  f.v0x = sm.rec[buf][0][e]; f.v0y = sm.rec[buf][1][e]; f.v0z = sm.rec[buf][2][e];
+  f.exx = sm.rec[buf][3][e]; f.exy = sm.rec[buf][4][e]; f.exz = sm.rec[buf][5][e];
+  f.eyx = sm.rec[buf][6][e]; f.eyy = sm.rec[buf][7][e]; f.eyz = sm.rec[buf][8][e];
+  f.ezx = sm.rec[buf][9][e]; f.ezy = sm.rec[buf][10][e]; f.ezz = sm.rec[buf][11][e];
+  f.a = sm.rec[buf][12][e]; f.b = sm.rec[buf][13][e]; f.aux = sm.rec[buf][14][e]; f.far2 = sm.rec[buf][16][e];
   return f;
 }
 
 // All elements of one kind in [lo, hi): tile loop, image loop, sink(j, weight_j, sum over copies).
+// seq = number of tiles this CTA has consumed so far (buffer = seq & 1, mbarrier parity = (seq >> 1) & 1).
 template <class M, int KIND, class Sink>
 __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img,
-                                             double px, double py, double pz, Sink& sink) {
-  for (int64_t base = lo; base < hi; base += kTile) {
-    int cnt = (int)min((int64_t)kTile, hi - base);
-    __syncthreads();
-    load_tile(sm, g, base, cnt);
-    __syncthreads();
+                                             double px, double py, double pz, Sink& sink, unsigned& seq) {
+  const int64_t tb0 = lo & ~(int64_t)(kTile - 1);
+  if (threadIdx.x == 0) tile_issue(sm, g, tb0, seq);
+  for (int64_t tb = tb0; tb < hi; tb += kTile) {
+    if (threadIdx.x == 0 && tb + kTile < hi) tile_issue(sm, g, tb + kTile, seq + 1);
+    tile_wait(sm, seq);
+    const unsigned buf = seq & 1u;
+    const int e0 = (int)max(lo - tb, (int64_t)0), e1 = (int)min(hi - tb, (int64_t)kTile);
 #pragma unroll 1
-    for (int e = 0; e < cnt; ++e) {
-      Frame fr = frame_of(sm, e);
+    for (int e = e0; e < e1; ++e) {
+      Frame fr = frame_of(sm, buf, e);
       // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
       // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
       Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
-      if (sink.self_pv(base + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
+      if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
 #pragma unroll 1
       for (int s = 1; s < n_img; ++s) {
         Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
         acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
       }
-      sink(base + e, sm.rec[15][e], acc);
+      sink(tb + e, sm.rec[buf][15][e], acc);
     }
+    __syncthreads();                               // the buffer is free for the tile after next
+    ++seq;
   }
 }
 
@@ -73,12 +117,13 @@ __device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, in
                                               double px, double py, double pz, Sink& sink) {
   int64_t r1 = g.n_rect, t1 = r1 + g.n_tri, w1 = t1 + g.n_wire;
   int64_t lo, hi;
+  unsigned seq = 0;
   lo = max(j0, (int64_t)0); hi = min(j1, r1);
-  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, px, py, pz, sink);
+  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
   lo = max(j0, r1); hi = min(j1, t1);
-  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, px, py, pz, sink);
+  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
   lo = max(j0, t1); hi = min(j1, w1);
-  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, px, py, pz, sink);
+  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
 }
 
 __device__ __forceinline__ void load_images(TileSmem& sm, const double* img, int n_img) {
@@ -104,7 +149,9 @@ __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables
                                                         const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                         double* __restrict__ partial) {
   __shared__ TileSmem sm;
+  tile_pipe_init(sm);
   load_images(sm, img, n_img);
+  __syncthreads();
   int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   int64_t pc = min(p, m - 1);
   double px = pts[pc], py = pts[m + pc], pz = pts[2 * m + pc];
@@ -204,7 +251,9 @@ __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const d
                                                             const double* __restrict__ diag, double* __restrict__ K,
                                                             int64_t ld, unsigned long long* __restrict__ rowmax_bits) {
   __shared__ TileSmem sm;
+  tile_pipe_init(sm);
   load_images(sm, img, n_img);
+  __syncthreads();
   int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
   int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   int64_t ic = min(i, n - 1);
