@@ -93,7 +93,7 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
     tile_wait(sm, seq);
     const unsigned buf = seq & 1u;
     const int e0 = (int)max(lo - tb, (int64_t)0), e1 = (int)min(hi - tb, (int64_t)kTile);
-#pragma unroll 1
+#pragma unroll 2
     for (int e = e0; e < e1; ++e) {
       Frame fr = frame_of(sm, buf, e);
       // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
