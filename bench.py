@@ -32,11 +32,13 @@ sys.path.insert(0, ROOT)
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
 # FP64 work of one (point, element copy) evaluation of (Phi', E') on the path that >99 % of the pairs of a field
-# map take (warp-uniform far branch), counted in the SASS of eval_kernel<MathFast> (FMA = 2 flop):
-# rectangle 113 DFMA + 38 DMUL + 15 DADD = 279 flop in 167 FP64-pipe instructions (the near branch: 323 flop,
-# 206 instructions); right triangle 230 flop in 139 instructions; wire 139; point charge 30
-FLOP_PER_PAIR = {"rect": 279.0, "tri": 230.0, "wire": 139.0, "charge": 30.0}
-FP64_INSTR_PER_PAIR = {"rect": 167.0}
+# map take (uniform-axes window + warp-uniform far branch), counted in the SASS of
+# eval_kernel<MathFast> (FMA = 2 flop): rectangle 101 DFMA + 32 DMUL + 14 DADD = 248 flop in 148 FP64-pipe
+# instructions (general window: 279 flop / 167; near branch: +44 flop / +39); right triangle 199 flop (230 on a
+# general window, less the same 31 flop of frame work); wire 139; point charge 30.  Windows that are not uniform
+# do more work than counted here, so `achieved` is a lower bound on them.
+FLOP_PER_PAIR = {"rect": 248.0, "tri": 199.0, "wire": 139.0, "charge": 30.0}
+FP64_INSTR_PER_PAIR = {"rect": 148.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE eval_kernel launch on C1, from the ncu --set full capture
 # summarised in profiles/r1_ncu_full_eval_assemble.md (3.285504 MB + 84.992 kB); algorithmic bytes of that launch:
 # 2.4 MB of points in + 4 x 8 x 1e5 x n_split partial sums out, the 0.8 MB element table from L2

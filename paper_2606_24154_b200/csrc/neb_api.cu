@@ -207,6 +207,9 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
     double rf = 2.5 * lmax + diag;
     r[16 * stride] = rf * rf;
   }
+  r[17 * stride] = fma(p0[0], ex[0], fma(p0[1], ex[1], p0[2] * ex[2]));
+  r[18 * stride] = fma(p0[0], ey[0], fma(p0[1], ey[1], p0[2] * ey[2]));
+  r[19 * stride] = fma(p0[0], ez[0], fma(p0[1], ez[1], p0[2] * ez[2]));
   for (int c = 0; c < 3; ++c) { colloc[c * stride + s] = cp[c]; normal[c * stride + s] = ey[c]; }
   int bk = bc_kind_in[j];
   if (bk != NEB_BC_DIRICHLET && bk != NEB_BC_DIELECTRIC) { atomicOr(flag, 16); bk = NEB_BC_DIRICHLET; }
@@ -219,6 +222,20 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
   bc_kind[s] = bk;
   bc_value[s] = bc_value_in ? bc_value_in[j] : 0.0;
   diag[s] = dg;
+}
+
+// One 64-thread CTA per 64-element window of the sorted table: do all its elements have bit-identical unit axes?
+__global__ void __launch_bounds__(64) tile_uniform_kernel(int64_t n, int64_t stride, const double* __restrict__ rec,
+                                                          int32_t* __restrict__ uniform) {
+  const int64_t j0 = (int64_t)blockIdx.x * 64, j = j0 + threadIdx.x;
+  int same = 1;
+  if (j < n) {
+#pragma unroll
+    for (int f = 3; f < 12; ++f)
+      same &= __double_as_longlong(rec[f * stride + j]) == __double_as_longlong(rec[f * stride + j0]);
+  }
+  same = __syncthreads_and(same);
+  if (threadIdx.x == 0) uniform[blockIdx.x] = (j0 < n) ? same : 0;
 }
 
 __global__ void set_weights_kernel(int64_t n, int64_t stride, const int32_t* __restrict__ perm, const double* __restrict__ sigma_caller,
@@ -255,11 +272,11 @@ __global__ void push_kernel(int64_t n3, double* __restrict__ pos, const double* 
 }
 
 static void free_problem(neb_ctx* c) {
-  void* ptrs[] = {c->d_rec, c->d_perm, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_img,
+  void* ptrs[] = {c->d_rec, c->d_uniform, c->d_perm, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_img,
                   c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma, c->d_dinv};
   for (void* p : ptrs)
     if (p) cudaFree(p);
-  c->d_rec = nullptr; c->d_perm = nullptr; c->d_colloc = nullptr; c->d_normal = nullptr; c->d_bc_kind = nullptr;
+  c->d_rec = nullptr; c->d_uniform = nullptr; c->d_perm = nullptr; c->d_colloc = nullptr; c->d_normal = nullptr; c->d_bc_kind = nullptr;
   c->d_bc_value = nullptr; c->d_diag = nullptr; c->d_img = nullptr; c->d_K = nullptr; c->d_rscale = nullptr;
   c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr; c->d_dinv = nullptr;
   c->assembled = c->factored = c->have_sigma = false;
@@ -376,6 +393,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
   const int64_t st = c->stride, npad = c->npad;
   if (!reuse) {
     NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_uniform, sizeof(int32_t) * (st / 64)));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_perm, sizeof(int32_t) * st));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_colloc, sizeof(double) * 3 * st));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_normal, sizeof(double) * 3 * st));
@@ -432,6 +450,8 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
         n, st, c->d_perm, (const int32_t*)dk, (const double*)dv0, (const double*)de1, (const double*)de2,
         (const double*)drad, (const double*)dcol, (const int32_t*)dbk, (const double*)dbv, (const double*)dep,
         (const double*)dem, c->d_rec, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_flag);
+    c->launches++;
+    tile_uniform_kernel<<<(unsigned)(st / 64), 64, 0, c->stream>>>(n, st, c->d_rec, c->d_uniform);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }

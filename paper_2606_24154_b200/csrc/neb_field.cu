@@ -28,6 +28,7 @@ constexpr int kMaxImg = 32;     // periodic copies kept in shared memory
 struct __align__(128) TileSmem {
   double rec[2][kRec][kTile];
   double img[3][kMaxImg];
+  double limg[3][kMaxImg];    // the image shifts in the axes of the current uniform window
   unsigned long long mbar[2];
 };
 constexpr unsigned kTileBytes = kRec * kTile * sizeof(double);
@@ -93,19 +94,58 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
     tile_wait(sm, seq);
     const unsigned buf = seq & 1u;
     const int e0 = (int)max(lo - tb, (int64_t)0), e1 = (int)min(hi - tb, (int64_t)kTile);
-#pragma unroll 2
-    for (int e = e0; e < e1; ++e) {
-      Frame fr = frame_of(sm, buf, e);
-      // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
-      // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
-      Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
-      if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
-#pragma unroll 1
-      for (int s = 1; s < n_img; ++s) {
-        Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
-        acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
+    if (KIND != 2 && g.uniform[tb >> 6]) {
+      // Uniform window: all 64 elements share one set of unit axes (a face of a mesh).  The point's products with
+      // the axes are formed once per window, an element's local coordinates are three subtractions, and the field
+      // is accumulated in the LOCAL frame and rotated to global once per window instead of once per pair.
+      Axes ax;
+      ax.exx = sm.rec[buf][3][e0]; ax.exy = sm.rec[buf][4][e0]; ax.exz = sm.rec[buf][5][e0];
+      ax.eyx = sm.rec[buf][6][e0]; ax.eyy = sm.rec[buf][7][e0]; ax.eyz = sm.rec[buf][8][e0];
+      ax.ezx = sm.rec[buf][9][e0]; ax.ezy = sm.rec[buf][10][e0]; ax.ezz = sm.rec[buf][11][e0];
+      if (n_img > 1) {
+        if (threadIdx.x < n_img) {
+          const double sx = sm.img[0][threadIdx.x], sy = sm.img[1][threadIdx.x], sz = sm.img[2][threadIdx.x];
+          sm.limg[0][threadIdx.x] = fma(sx, ax.exx, fma(sy, ax.exy, sz * ax.exz));
+          sm.limg[1][threadIdx.x] = fma(sx, ax.eyx, fma(sy, ax.eyy, sz * ax.eyz));
+          sm.limg[2][threadIdx.x] = fma(sx, ax.ezx, fma(sy, ax.ezy, sz * ax.ezz));
+        }
+        __syncthreads();
       }
-      sink(tb + e, sm.rec[buf][15][e], acc);
+      const double PX = fma(px, ax.exx, fma(py, ax.exy, pz * ax.exz));
+      const double PY = fma(px, ax.eyx, fma(py, ax.eyy, pz * ax.eyz));
+      const double PZ = fma(px, ax.ezx, fma(py, ax.ezy, pz * ax.ezz));
+      sink.tile_begin(ax);
+#pragma unroll 2
+      for (int e = e0; e < e1; ++e) {
+        const double a = sm.rec[buf][12][e], b = sm.rec[buf][13][e], aux = sm.rec[buf][14][e], far2 = sm.rec[buf][16][e];
+        const double X0 = PX - sm.rec[buf][17][e], Y0 = PY - sm.rec[buf][18][e], Z0 = PZ - sm.rec[buf][19][e];
+        double phi, lx, ly, lz;
+        local_pair<M, KIND>(a, b, aux, far2, X0, Y0, Z0, phi, lx, ly, lz);
+        if (sink.self_pv(tb + e)) { lx = 0.0; ly = 0.0; lz = 0.0; }   // principal value (S5, S8)
+#pragma unroll 1
+        for (int s = 1; s < n_img; ++s) {
+          double p1, x1, y1, z1;
+          local_pair<M, KIND>(a, b, aux, far2, X0 - sm.limg[0][s], Y0 - sm.limg[1][s], Z0 - sm.limg[2][s], p1, x1, y1, z1);
+          phi += p1; lx += x1; ly += y1; lz += z1;
+        }
+        sink.local(tb + e, sm.rec[buf][15][e], phi, lx, ly, lz);
+      }
+      sink.tile_end(ax);
+    } else {
+#pragma unroll 2
+      for (int e = e0; e < e1; ++e) {
+        Frame fr = frame_of(sm, buf, e);
+        // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
+        // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
+        Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
+        if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
+#pragma unroll 1
+        for (int s = 1; s < n_img; ++s) {
+          Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
+          acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
+        }
+        sink(tb + e, sm.rec[buf][15][e], acc);
+      }
     }
     __syncthreads();                               // the buffer is free for the tile after next
     ++seq;
@@ -138,6 +178,17 @@ struct EvalSink {
   __device__ __forceinline__ bool self_pv(int64_t) const { return false; }
   __device__ __forceinline__ void operator()(int64_t, double w, const Infl& a) {
     phi = fma(w, a.phi, phi); ex = fma(w, a.ex, ex); ey = fma(w, a.ey, ey); ez = fma(w, a.ez, ez);
+  }
+  // uniform window: weighted sum of the LOCAL field components, rotated to global at its end
+  double lx = 0, ly = 0, lz = 0;
+  __device__ __forceinline__ void tile_begin(const Axes&) { lx = 0.0; ly = 0.0; lz = 0.0; }
+  __device__ __forceinline__ void local(int64_t, double w, double p, double fx, double fy, double fz) {
+    phi = fma(w, p, phi); lx = fma(w, fx, lx); ly = fma(w, fy, ly); lz = fma(w, fz, lz);
+  }
+  __device__ __forceinline__ void tile_end(const Axes& ax) {
+    ex = fma(lx, ax.exx, fma(ly, ax.eyx, fma(lz, ax.ezx, ex)));
+    ey = fma(lx, ax.exy, fma(ly, ax.eyy, fma(lz, ax.ezy, ey)));
+    ez = fma(lx, ax.exz, fma(ly, ax.eyz, fma(lz, ax.ezz, ez)));
   }
 };
 
@@ -241,6 +292,21 @@ struct AsmSink {
     rmax = fmax(rmax, fabs(v));
     if (active) K[i + j * ld] = v;
   }
+  // uniform window: the row's normal in the window's axes, so that n . E' needs no rotation per pair
+  double nlx = 0, nly = 0, nlz = 0;
+  __device__ __forceinline__ void tile_begin(const Axes& ax) {
+    nlx = fma(nx, ax.exx, fma(ny, ax.exy, nz * ax.exz));
+    nly = fma(nx, ax.eyx, fma(ny, ax.eyy, nz * ax.eyz));
+    nlz = fma(nx, ax.ezx, fma(ny, ax.ezy, nz * ax.ezz));
+  }
+  __device__ __forceinline__ void local(int64_t j, double, double p, double fx, double fy, double fz) {
+    double vd = fma(nlx, fx, fma(nly, fy, nlz * fz));
+    double v = kCoulomb * (dielectric ? vd : p);
+    v += (dielectric && j == i) ? diag : 0.0;
+    rmax = fmax(rmax, fabs(v));
+    if (active) K[i + j * ld] = v;
+  }
+  __device__ __forceinline__ void tile_end(const Axes&) {}
 };
 
 template <class M>
@@ -329,7 +395,7 @@ static int pick_splits(int64_t pt_blocks, int64_t units, int64_t unit_tile, int 
 
 static GeoTables tables(const neb_ctx* c) {
   GeoTables g;
-  g.rec = c->d_rec; g.stride = c->stride; g.n_rect = c->n_rect; g.n_tri = c->n_tri; g.n_wire = c->n_wire;
+  g.rec = c->d_rec; g.uniform = c->d_uniform; g.stride = c->stride; g.n_rect = c->n_rect; g.n_tri = c->n_tri; g.n_wire = c->n_wire;
   return g;
 }
 

@@ -11,7 +11,7 @@
 
 namespace neb {
 
-// Frame-table record (a1), 16 doubles per element, stored SoA in global memory (field-major):
+// Frame-table record (a1), 20 doubles per element, stored SoA in global memory (field-major):
 //   0..2  v0      corner / right-angle vertex / wire start
 //   3..5  ex      unit vector along e1 (local X)
 //   6..8  ey      unit normal e2 x e1 / |e2 x e1| (local Y)        [wire: unused]
@@ -22,7 +22,10 @@ namespace neb {
 //   15    w       weight: sigma_j / (4 pi eps0) for evaluation (set by neb_solve / neb_set_sigma)
 //   16    far2    (2.5 Lmax + diag)^2, Lmax = longest edge, diag = sqrt(a^2+b^2): a point at least that far
 //                 (squared) from v0 is >= 2.5 Lmax away from every point of the element      [wire: unused]
-#define NEB_REC 17
+//   17..19 c      (v0 . ex, v0 . ey, v0 . ez): the element's origin in its own axes.  With them the local coordinates of
+//                 a point are (P . ex, P . ey, P . ez) - c, and the products P . e are shared by every element that has
+//                 the same axes (a whole face of a mesh): the uniform-tile path of neb_field.cu   [wire: unused]
+#define NEB_REC 20
 
 struct Infl {
   double phi, ex, ey, ez;   // primed potential and GLOBAL primed field components
@@ -142,6 +145,19 @@ __device__ __forceinline__ void tri_local(double a, double b, double ih, double 
 struct Frame {
   double v0x, v0y, v0z, exx, exy, exz, eyx, eyy, eyz, ezx, ezy, ezz, a, b, aux, far2;
 };
+
+// Unit axes of a frame (rows of the local <- global rotation).
+struct Axes {
+  double exx, exy, exz, eyx, eyy, eyz, ezx, ezy, ezz;
+};
+
+// Rectangle or right triangle at local coordinates (X, Y, Z): phi' and the LOCAL field components.
+template <class M, int KIND>
+__device__ __forceinline__ void local_pair(double a, double b, double aux, double far2, double X, double Y, double Z,
+                                           double& phi, double& lx, double& ly, double& lz) {
+  if (KIND == 0) rect_local<M>(a, b, aux, far2, X, Y, Z, phi, lx, ly, lz);
+  else tri_local<M>(a, b, aux, far2, X, Y, Z, phi, lx, ly, lz);
+}
 
 template <class M, int KIND>
 __device__ __forceinline__ Infl influence(const Frame& f, double px, double py, double pz) {

@@ -10,13 +10,14 @@ namespace neb {
 
 constexpr double kEps0 = 8.8541878128e-12;                 // F/m (reading S3)
 constexpr double kCoulomb = 1.0 / (4.0 * 3.14159265358979323846 * kEps0);
-constexpr int kRec = 17;                                   // doubles per frame-table record
+constexpr int kRec = 20;                                   // doubles per frame-table record
 constexpr int kPad = 128;                                  // matrix dimension is padded to a multiple of this
 
 // Frame tables (a1), elements sorted by kind: [rect | tri | wire].  SoA, field-major:
 // rec[f * stride + j], f < kRec (fields listed in neb_influence.cuh).
 struct GeoTables {
   const double* rec;
+  const int32_t* uniform;   // per 64-element window: 1 if all its elements share one set of unit axes (bitwise)
   int64_t stride;
   int32_t n_rect, n_tri, n_wire;
 };
@@ -48,6 +49,7 @@ struct neb_ctx {
   int64_t n = 0, npad = 0, stride = 0;
   int32_t n_rect = 0, n_tri = 0, n_wire = 0, n_img = 0;
   double* d_rec = nullptr;        // kRec * stride
+  int32_t* d_uniform = nullptr;   // stride / 64 window flags (see GeoTables)
   int32_t* d_perm = nullptr;      // sorted position -> caller index
   double* d_colloc = nullptr;     // 3 * stride, sorted order
   double* d_normal = nullptr;     // 3 * stride, sorted order
