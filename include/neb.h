@@ -49,7 +49,8 @@ enum { NEB_BC_DIRICHLET = 0, NEB_BC_DIELECTRIC = 1 };   /* row kinds            
 /* Options for neb_set_option. */
 enum {
   NEB_OPT_MATH = 0,     /* 1 (default): hand-written log/atan2/sqrt/rcp sequences; 0: CUDA libm  */
-  NEB_OPT_LU_BLOCK = 1, /* LU panel width nb; this build supports 64 only                        */
+  NEB_OPT_LU_BLOCK = 1, /* LU outer block width (64, 128 or 256) once the trailing matrix is <= 8192 rows;
+                           default 64; larger trailing matrices always use 256 (panels are 64 wide) */
   NEB_OPT_PROFILE = 2,  /* 1: record per-stage CUDA-event timings (neb_stage_ms); default 0      */
   NEB_OPT_LU_PANEL = 3, /* 0 (default): cluster/DSMEM panel kernel where the panel fits (<= 8192 rows),
                            grid-wide cooperative kernel above; 1: grid-wide kernel only          */

@@ -364,7 +364,8 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
   switch (option) {
     case NEB_OPT_MATH: c->math_fast = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_LU_BLOCK:
-      if (value != 64) return fail(c, NEB_EINVAL, "this build supports LU panel width 64 only");
+      if (value != 64 && value != 128 && value != 256) return fail(c, NEB_EINVAL, "LU outer block width must be 64, 128 or 256");
+      c->lu_nb = (int)value;
       return NEB_OK;
     case NEB_OPT_PROFILE: c->profile = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_LU_PANEL: c->panel_mode = value ? 1 : 0; return NEB_OK;

@@ -244,16 +244,22 @@ __global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
-// Trailing update C -= L * U with C = A[r0.., r0..] (m x m), L = A[r0.., k..k+64), U = A[k..k+64, r0..].
-// CTA tile 128 (rows) x 64 (cols), 8 warps as 4 (rows) x 2 (cols), warp tile 32 x 32 = 4 x 4 DMMA tiles.
+// Trailing update C -= L * U on the FP64 tensor cores, any depth K (a multiple of 32):
+//   C = A[r0 .. r0+m, c_first ..],  L = A[r0 .. r0+m, k .. k+K),  U = A[k .. k+K, c_first ..].
+// CTA tile 128 (rows) x 64 (cols), 8 warps as 4 (rows) x 2 (cols), warp tile 32 x 32 = 4 x 4 DMMA tiles
+// (mma.sync.m8n8k4.f64).  The accumulators start from C and stay in registers over the whole K loop; L and U
+// arrive in chunks of 32 k through a two-stage cp.async pipeline (the next chunk loads while this one is
+// multiplied), so C is read and written ONCE per update whatever its depth: with K = 256 (two-level blocking,
+// lu_factor) the update does 32 flop per byte of C instead of 8.
 // The mma computes the transposed tile: mma row <-> C column, mma col <-> C row, so that each lane's
 // two accumulators are two consecutive rows of one column (16-byte global accesses).
 // ------------------------------------------------------------------------------------------------
-constexpr int GM = 128, GN = 64, GK = NB;
+constexpr int GM = 128, GN = 64, GKC = 32;     // tile and k-chunk
 constexpr int LDL = GM + 4;    // shared leading dimensions: stride mod 16 (in doubles) = 4 -> conflict-free
-constexpr int LDU = GK + 4;
+constexpr int LDU = GKC + 4;
 constexpr int GEMM_THREADS = 256;
-constexpr size_t GEMM_SMEM = (size_t)(GK * LDL + GN * LDU) * sizeof(double);
+constexpr int GEMM_STAGE = GKC * LDL + GN * LDU;               // doubles per stage
+constexpr size_t GEMM_SMEM = (size_t)2 * GEMM_STAGE * sizeof(double);
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -268,30 +274,32 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t r0,
+__global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int K, int64_t r0,
                                                                int64_t m, int64_t c_first) {
   extern __shared__ __align__(16) double smem[];
-  double* sL = smem;                 // sL[kk * LDL + i] = L[i][kk]
-  double* sU = smem + GK * LDL;      // sU[j * LDU + kk] = U[kk][j]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t i0 = r0 + (int64_t)blockIdx.x * GM;       // first row of the tile
   const int64_t j0 = c_first + (int64_t)blockIdx.y * GN;  // first column
   const int rows_here = (int)min((int64_t)GM, r0 + m - i0);   // 64 or 128
-  // stage operands: two k-halves as two cp.async groups
-#pragma unroll
-  for (int half = 0; half < 2; ++half) {
-    // L: 32 k-columns x 128 rows = 32 x 64 16-byte chunks
-    for (int idx = tid; idx < 32 * (GM / 2); idx += GEMM_THREADS) {
-      int kk = half * 32 + idx / (GM / 2), ch = idx % (GM / 2);
-      if (2 * ch < rows_here) cp_async16(sL + kk * LDL + 2 * ch, A + (i0 + 2 * ch) + (k + kk) * ld);
+  const int nchunks = K / GKC;
+  // stage st <- chunk ch: sL[kk * LDL + i] = L[i][ch*32 + kk], sU[j * LDU + kk] = U[ch*32 + kk][j]
+  auto issue = [&](int ch, int st) {
+    double* sL = smem + st * GEMM_STAGE;
+    double* sU = sL + GKC * LDL;
+    const int64_t kc = k + (int64_t)ch * GKC;
+    for (int idx = tid; idx < GKC * (GM / 2); idx += GEMM_THREADS) {     // 32 k-columns x 64 16-byte chunks
+      const int kk = idx / (GM / 2), c2 = idx % (GM / 2);
+      if (2 * c2 < rows_here) cp_async16(sL + kk * LDL + 2 * c2, A + (i0 + 2 * c2) + (kc + kk) * ld);
     }
-    // U: 64 columns x 32 k-rows = 64 x 16 chunks
-    for (int idx = tid; idx < GN * 16; idx += GEMM_THREADS) {
-      int j = idx / 16, ch = idx % 16;
-      cp_async16(sU + j * LDU + half * 32 + 2 * ch, A + (k + half * 32 + 2 * ch) + (j0 + j) * ld);
+    for (int idx = tid; idx < GN * (GKC / 2); idx += GEMM_THREADS) {     // 64 columns x 16 chunks
+      const int j = idx / (GKC / 2), c2 = idx % (GKC / 2);
+      cp_async16(sU + j * LDU + 2 * c2, A + (kc + 2 * c2) + (j0 + j) * ld);
     }
-    cp_async_commit();
-  }
+  };
+  issue(0, 0);
+  cp_async_commit();
+  if (nchunks > 1) issue(1, 1);
+  cp_async_commit();
   const int wr = warp & 3, wc = warp >> 2;                // warp tile origin: rows wr*32, cols wc*32
   const int g = lane >> 2, t = lane & 3;
   const bool active = wr * 32 < rows_here;
@@ -306,13 +314,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restric
         acc[ni][mi][0] = v.x; acc[ni][mi][1] = v.y;
       }
   }
-#pragma unroll
-  for (int half = 0; half < 2; ++half) {
-    if (half == 0) cp_async_wait<1>(); else cp_async_wait<0>();
+#pragma unroll 1
+  for (int ch = 0; ch < nchunks; ++ch) {
+    cp_async_wait<1>();                                   // chunk ch has landed (one younger group may be in flight)
     __syncthreads();
+    const double* sL = smem + (ch & 1) * GEMM_STAGE;
+    const double* sU = sL + GKC * LDL;
     if (active) {
 #pragma unroll 2
-      for (int k4 = half * 8; k4 < half * 8 + 8; ++k4) {
+      for (int k4 = 0; k4 < GKC / 4; ++k4) {
         double fa[4], fb[4];
         // mma A operand (row = C column n, col = k): U[k4*4 + t][n = g]
 #pragma unroll
@@ -326,6 +336,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restric
           for (int mi = 0; mi < 4; ++mi) dmma884(acc[ni][mi][0], acc[ni][mi][1], fa[ni], fb[mi]);
       }
     }
+    if (ch + 2 < nchunks) {
+      __syncthreads();                                    // everyone is done with this stage: refill it
+      issue(ch + 2, ch & 1);
+    }
+    cp_async_commit();                                    // (possibly empty) keeps the group count in step
   }
   if (active) {
 #pragma unroll
@@ -507,53 +522,85 @@ neb_status lu_factor(neb_ctx* c) {
     return NEB_OK;
   };
   // row exchanges of panel k on the columns [c_lo, c_hi) \ [skip_lo, skip_hi)
-  auto laswp = [&](int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
+  auto laswp = [&](cudaStream_t st, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
     const int64_t ncols = (c_hi - c_lo) - (skip_hi - skip_lo);
     if (ncols <= 0) return;
-    laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, S1>>>(c->d_K, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
+    laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, st>>>(c->d_K, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
     c->launches++;
   };
-  // U12 and the trailing update of panel k restricted to the columns [c_first, c_first + ncols)
-  auto update = [&](int64_t k, int64_t c_first, int64_t ncols, bool timed) {
-    if (ncols <= 0) return;
-    const int64_t r0 = k + NB, m = npad - r0;
-    trsm_kernel<<<(unsigned)(ncols / NB), TRSM_THREADS, TRSM_SMEM, S1>>>(c->d_K, ld, k, c_first);
-    c->launches++;
+  // C[r0 .. r0+m, c_first .. c_first+ncols) -= A[r0 .., k .. k+K) * A[k .. k+K, c_first ..) on the tensor cores
+  const bool timed = !c->lu_lookahead;
+  auto gemm = [&](cudaStream_t st, int64_t k, int K, int64_t r0, int64_t m, int64_t c_first, int64_t ncols) {
+    if (m <= 0 || ncols <= 0) return;
     dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
     if (timed) {
       StageTimer tg(c, NEB_STAGE_LU_GEMM);
-      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, S1>>>(c->d_K, ld, k, r0, m, c_first);
-      c->launches++;
+      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(c->d_K, ld, k, K, r0, m, c_first);
     } else {
-      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, S1>>>(c->d_K, ld, k, r0, m, c_first);
-      c->launches++;
+      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(c->d_K, ld, k, K, r0, m, c_first);
     }
+    c->launches++;
+  };
+  auto trsm = [&](cudaStream_t st, int64_t k, int64_t c_first, int64_t ncols) {
+    if (ncols <= 0) return;
+    trsm_kernel<<<(unsigned)(ncols / NB), TRSM_THREADS, TRSM_SMEM, st>>>(c->d_K, ld, k, c_first);
+    c->launches++;
   };
 
-  // Right-looking with a look-ahead of one panel: as soon as panel k is factored, ITS update is applied to the 64
-  // columns of panel k+1 first; panel k+1 is then factored on the side stream (one cluster: 16 SMs) while the main
-  // stream updates the rest of the trailing matrix on the other SMs.  Only where the next panel runs on a cluster
-  // (the grid-wide panel kernel needs every SM).  The trailing update is timed alone only without look-ahead.
-  NEB_TRY(launch_panel(0, S1));
-  for (int64_t k = 0; k < npad; k += NB) {
-    const int64_t r0 = k + NB, m = npad - r0;
-    const bool ahead = c->lu_lookahead && S2 && m > NB && m <= cluster_rows;
+  // Two-level right-looking factorisation.  Outer blocks of OB = 256 columns = 4 panels of 64:
+  //   chain   for each panel of the block: factor it, then apply its update (row exchanges, U12 = L11^-1 A12,
+  //           rank-64 tensor-core update) to the REST OF THE BLOCK only;
+  //   wide    the block's row exchanges on all other columns, the block row of U (4 x [TRSM + small update]), and
+  //           ONE rank-256 tensor-core update of the whole trailing matrix: C is read and written once per 256
+  //           columns instead of once per 64 (32 flop per byte of C: compute-bound on the DMMA pipe).
+  // Look-ahead: the rank-256 update is applied to the next block's columns first; that block's chain (latency-bound,
+  // one cluster = 16 SMs per panel) then runs on the side stream while the main stream finishes the update on the
+  // other SMs.  Only where the panels run on a cluster (the grid-wide panel kernel needs every SM).
+  // Block width: 256 while the trailing matrix is large (its update dominates and wants the depth); c->lu_nb (64 by
+  // default) once the remaining panels run on a cluster with look-ahead: there the chain of panels is the critical
+  // path and anything added to it (the in-block updates, a wider look-ahead slice) costs more than the deeper
+  // update saves.
+  auto block_width = [&](int64_t remaining) -> int64_t { return remaining > cluster_rows ? 4 * NB : (int64_t)c->lu_nb; };
+  bool chain_on_side = false;
+  for (int64_t kb = 0; kb < npad;) {
+    const int64_t w = min(block_width(npad - kb), npad - kb), nb = kb + w;
+    cudaStream_t SC = chain_on_side ? S2 : S1;
+    for (int64_t k = kb; k < nb; k += NB) {
+      NEB_TRY(launch_panel(k, SC));
+      const int64_t in_cols = nb - (k + NB);               // columns of this block right of the panel
+      laswp(SC, k, kb, nb, k, k + NB);                     // the block's other columns, left and right of the panel
+      trsm(SC, k, k + NB, in_cols);
+      gemm(SC, k, NB, k + NB, npad - (k + NB), k + NB, in_cols);
+    }
+    if (chain_on_side) {
+      NEB_CUDA(c, cudaEventRecord(c->ev_panel, S2));
+      NEB_CUDA(c, cudaStreamWaitEvent(S1, c->ev_panel, 0));
+    }
+    const int64_t right = npad - nb;                       // columns (and rows) of the trailing matrix
+    // everything the factored block does to the columns [c0, c0 + nc) right of it
+    auto wide = [&](int64_t c0, int64_t nc) {
+      if (nc <= 0) return;
+      for (int64_t k = kb; k < nb; k += NB) laswp(S1, k, c0, c0 + nc, c0 + nc, c0 + nc);
+      for (int64_t k = kb; k < nb; k += NB) {
+        trsm(S1, k, c0, nc);
+        gemm(S1, k, NB, k + NB, nb - (k + NB), c0, nc);    // rows of the block row still below this panel
+      }
+      gemm(S1, kb, (int)w, nb, right, c0, nc);
+    };
+    const int64_t w_next = right > 0 ? min(block_width(right), right) : 0;
+    const bool ahead = c->lu_lookahead && S2 && right > 0 && right <= cluster_rows && right > w_next;
     if (ahead) {
-      laswp(k, r0, r0 + NB, r0 + NB, r0 + NB);
-      update(k, r0, NB, false);
+      wide(nb, w_next);                                    // the next block's columns first ...
       NEB_CUDA(c, cudaEventRecord(c->ev_next, S1));
       NEB_CUDA(c, cudaStreamWaitEvent(S2, c->ev_next, 0));
-      NEB_TRY(launch_panel(r0, S2));
-      NEB_CUDA(c, cudaEventRecord(c->ev_panel, S2));
-      laswp(k, 0, npad, k, r0 + NB);
-      update(k, r0 + NB, m - NB, false);
-      NEB_CUDA(c, cudaStreamWaitEvent(S1, c->ev_panel, 0));
+      wide(nb + w_next, right - w_next);                   // ... the rest while its chain runs on the side stream
     } else {
-      laswp(k, 0, npad, k, r0);
-      update(k, r0, m, !c->lu_lookahead);
-      if (m > 0) NEB_TRY(launch_panel(r0, S1));
+      wide(nb, right);
     }
+    for (int64_t k = kb; k < nb; k += NB) laswp(S1, k, 0, kb, kb, kb);   // the factors to the left
+    chain_on_side = ahead;
     NEB_CUDA(c, cudaGetLastError());
+    kb = nb;
   }
   // composed permutation for the solves
   if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
