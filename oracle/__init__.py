@@ -173,3 +173,29 @@ def push(pos, E, mu, dt, mode="ld"):
     E = _d(E)
     _lib(mode).orc_push(C.c_int64(pos.shape[1]), _p(pos), _p(E), C.c_double(mu), C.c_double(dt))
     return pos
+
+
+def fastvol_nodes(nx, ny, nz, origin, spacing):
+    """Node coordinates (3, nx*ny*nz) of a uniform FastVolume grid, i fastest (reading S25)."""
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    return np.stack([origin[0] + i.ravel() * spacing[0], origin[1] + j.ravel() * spacing[1],
+                     origin[2] + k.ravel() * spacing[2]])
+
+
+def fastvol_eval(shape, origin, spacing, values, pts, mode="ld"):
+    """Trilinear interpolation of values (4, nx*ny*nz) = Phi, Ex, Ey, Ez at pts (3, m); NaN outside."""
+    nx, ny, nz = (int(v) for v in shape)
+    values, pts = _d(values), _d(pts)
+    origin, spacing = _d(np.asarray(origin, dtype=np.float64)), _d(np.asarray(spacing, dtype=np.float64))
+    m = pts.shape[1]
+    phi, E = np.zeros(m), np.zeros((3, m))
+    _lib(mode).orc_fastvol_eval(C.c_int32(nx), C.c_int32(ny), C.c_int32(nz), _p(origin), _p(spacing), _p(values),
+                                C.c_int64(m), _p(pts), _p(phi), _p(E))
+    return phi, E
+
+
+def weighting_rhs(g: Geometry, bc_value_w) -> np.ndarray:
+    """Right-hand side of a weighting-field solve (P:222 CreateWtFldFastVolPF; reading S26): the read-out
+    electrode's panels at their weighting potential (1), every other conductor at 0, no space charge;
+    dielectric rows stay homogeneous (0)."""
+    return np.where(g.bc_kind == 0, np.asarray(bc_value_w, dtype=np.float64), 0.0)

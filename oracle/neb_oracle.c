@@ -16,7 +16,9 @@
  * value): brute-force Gauss-Legendre / mpmath quadrature of the defining integrals P:121, P:125,
  * P:131; far-field limit Eq.(2); E = -grad(Phi) P:75 by central differences; closed forms
  * (centre of a rectangle, axis of a square); additivity; Gauss's law on a closed cube; textbook
- * image charge over a dielectric half-space; slab capacitor; numpy.linalg.solve for the LU.
+ * image charge over a dielectric half-space; slab capacitor; numpy.linalg.solve for the LU;
+ * FastVolume interpolation: exact reproduction of products of linear functions, node values, and
+ * scipy.interpolate.RegularGridInterpolator.
  * Parity unpinned: the paper's "<=1.67 % vs COMSOL" accuracy — geometry and COMSOL absent.
  *
  * Layout: all vectors are SoA, x[0..n) y[0..n) z[0..n).  SI units.  Physical values are
@@ -486,4 +488,54 @@ void orc_eval(int64_t n, const int32_t* kind, const double* v0, const double* e1
 /* a9. Charge push of the synthetic C4 loop (reading S23): x += mu * E * dt. */
 void orc_push(int64_t q, double* pos, const double* E, double mu, double dt) {
   for (int64_t k = 0; k < 3 * q; ++k) pos[k] = (double)((real)pos[k] + (real)mu * (real)E[k] * (real)dt);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * FastVolume ("Fast Volume", P:222 CreateFastVolPF): the potential and field are precomputed on a
+ * 3-D grid of nodal points and "rapidly estimated using a simple trilinear interpolation from the
+ * values stored at the nearest nodes".  Reading (S25): uniform grid, node (i,j,k) at
+ * origin + (i hx, j hy, k hz), i < nx fastest; values[c][(k*ny + j)*nx + i], c = 0..3 = Phi, Ex, Ey, Ez;
+ * each of the four quantities is interpolated on its own; a point outside the grid's box gets NaN.
+ * "Outside" is decided on the cell coordinate t = (x - origin)/h in DOUBLE (the precision of the CUDA
+ * path, so that both sides take this yes/no decision alike) with a slack of 1e-9 cells, because a node
+ * of the upper faces, computed as origin + i h, may round to t = n-1+1e-16; t is then clamped to [0, n-1].
+ * Trilinear interpolation written out as its definition: the sum over the 8 corners of the cell of
+ * the corner value times the product of the three 1-D hat weights.
+ * ------------------------------------------------------------------------------------------------ */
+void orc_fastvol_eval(int32_t nx, int32_t ny, int32_t nz, const double* origin, const double* spacing,
+                      const double* values, int64_t m, const double* pts, double* phi, double* E) {
+  const int64_t nn = (int64_t)nx * ny * nz;
+  const int32_t dim[3] = {nx, ny, nz};
+#pragma omp parallel for schedule(static)
+  for (int64_t p = 0; p < m; ++p) {
+    int32_t cell[3];
+    real f[3];
+    int inside = 1;
+    for (int a = 0; a < 3; ++a) {
+      const double td = (pts[a * m + p] - origin[a]) / spacing[a];
+      if (!(td >= -1e-9 && td <= (double)(dim[a] - 1) + 1e-9)) { inside = 0; break; }
+      real t = ((real)pts[a * m + p] - (real)origin[a]) / (real)spacing[a];
+      if (t < 0) t = 0;
+      if (t > (real)(dim[a] - 1)) t = (real)(dim[a] - 1);
+      int32_t i = (int32_t)floorl((long double)t);
+      if (i > dim[a] - 2) i = dim[a] - 2;      /* t == n-1: last cell, weight 1 on its far node */
+      cell[a] = i;
+      f[a] = t - (real)i;
+    }
+    double out[4];
+    for (int c = 0; c < 4; ++c) {
+      if (!inside) { out[c] = NAN; continue; }
+      long double acc = 0;
+      for (int dk = 0; dk < 2; ++dk)
+        for (int dj = 0; dj < 2; ++dj)
+          for (int di = 0; di < 2; ++di) {
+            real w = (di ? f[0] : 1 - f[0]) * (dj ? f[1] : 1 - f[1]) * (dk ? f[2] : 1 - f[2]);
+            int64_t node = ((int64_t)(cell[2] + dk) * ny + (cell[1] + dj)) * nx + (cell[0] + di);
+            acc += (long double)(w * (real)values[c * nn + node]);
+          }
+      out[c] = (double)acc;
+    }
+    phi[p] = out[0];
+    E[p] = out[1]; E[m + p] = out[2]; E[2 * m + p] = out[3];
+  }
 }

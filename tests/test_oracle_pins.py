@@ -473,3 +473,78 @@ def test_push_is_axpy(orc):
     E = np.array([[1e3, 0.0], [0.0, -2e3], [4e3, 0.0]])
     out = orc.push(pos, E, mu=1.5e-4, dt=1e-9)
     assert out[0, 0] == 1.0 + 1.5e-4 * 1e3 * 1e-9 and out[1, 1] == 4.0 - 1.5e-4 * 2e3 * 1e-9 and out[2, 1] == 6.0
+
+
+# ---------------------------------------------------------------------------------------------
+# FastVolume and weighting field: pins for the oracle's interpolation
+# ---------------------------------------------------------------------------------------------
+def test_fastvol_trilinear_reproduces_products_of_linear_functions(orc):
+    """Trilinear interpolation is exact for every function that is linear in each coordinate separately
+    (1, x, y, z, xy, yz, zx, xyz); it returns the node values at the nodes; outside the box it gives NaN."""
+    nx, ny, nz = 5, 4, 3
+    o, h = np.array([0.1, -0.2, 0.3]), np.array([0.5, 0.25, 1.0])
+    P = orc.fastvol_nodes(nx, ny, nz, o, h)
+    assert P.shape == (3, 60) and np.allclose(P[:, 1] - P[:, 0], [h[0], 0, 0]) and np.allclose(P[:, nx] - P[:, 0], [0, h[1], 0])
+    f = lambda x, y, z: (1 + 2 * x) * (3 - y) * (0.5 + z)
+    vals = np.stack([f(*P), P[0] - P[2], P[1] * P[2], P[0] * P[1] * P[2]])
+    rs = np.random.RandomState(0)
+    pts = o[:, None] + rs.rand(3, 500) * (h * np.array([nx - 1, ny - 1, nz - 1]))[:, None]
+    phi, E = orc.fastvol_eval((nx, ny, nz), o, h, vals, pts)
+    assert np.max(np.abs(phi - f(*pts))) < 1e-13 * np.max(np.abs(vals[0]))
+    assert np.max(np.abs(E[0] - (pts[0] - pts[2]))) < 1e-14 and np.max(np.abs(E[2] - pts[0] * pts[1] * pts[2])) < 1e-14
+    phi_n, E_n = orc.fastvol_eval((nx, ny, nz), o, h, vals, P)                  # at the nodes, upper faces included
+    assert np.max(np.abs(phi_n - vals[0])) < 1e-13 and np.max(np.abs(E_n - vals[1:])) < 1e-14
+    out = np.array([[o[0] - 1e-6, o[0] + 0.1], [o[1] + 0.1, o[1] + 0.1], [o[2] + 0.1, o[2] + (nz - 1) * h[2] + 1e-6]])
+    phi_o, E_o = orc.fastvol_eval((nx, ny, nz), o, h, vals, out)
+    assert np.all(np.isnan(phi_o)) and np.all(np.isnan(E_o))
+
+
+def test_fastvol_matches_scipy_regular_grid_interpolator(orc):
+    from scipy.interpolate import RegularGridInterpolator
+    nx, ny, nz = 7, 6, 5
+    o, h = np.array([-1.0, 0.0, 2.0]), np.array([0.3, 0.7, 0.45])
+    rs = np.random.RandomState(5)
+    vals = rs.normal(size=(4, nx * ny * nz))
+    pts = o[:, None] + rs.rand(3, 400) * (h * np.array([nx - 1, ny - 1, nz - 1]))[:, None]
+    phi, E = orc.fastvol_eval((nx, ny, nz), o, h, vals, pts)
+    axes = (o[2] + h[2] * np.arange(nz), o[1] + h[1] * np.arange(ny), o[0] + h[0] * np.arange(nx))
+    for c, got in enumerate([phi, E[0], E[1], E[2]]):
+        ref = RegularGridInterpolator(axes, vals[c].reshape(nz, ny, nx), method="linear")(pts[::-1].T)
+        assert np.max(np.abs(got - ref)) < 1e-12
+
+
+def test_fastvol_error_is_second_order_against_direct_evaluation(orc):
+    """A FastVolume of a charged plate's field: the interpolation error against direct evaluation falls by ~4
+    per halving of the grid spacing (the paper reports < 0.25 % for its map)."""
+    pr = W.plate(n_side=4, m_points=0)
+    g = orc.Geometry(pr)
+    sig = np.full(pr.n, 1e-8)
+    o = np.array([-4e-3, -4e-3, 2e-3])
+    rs = np.random.RandomState(2)
+    pts = o[:, None] + rs.rand(3, 200) * 8e-3
+    phi_d, E_d = orc.evaluate(g, sig, pts, mode="f64")
+    errs = []
+    for n in (5, 9, 17):
+        h = np.full(3, 8e-3 / (n - 1))
+        P = orc.fastvol_nodes(n, n, n, o, h)
+        ph, Ev = orc.evaluate(g, sig, P, mode="f64")
+        phi_i, E_i = orc.fastvol_eval((n, n, n), o, h, np.vstack([ph[None], Ev]), pts, mode="f64")
+        errs.append(np.max(np.abs(phi_i - phi_d)) / np.max(np.abs(phi_d)))
+    assert errs[0] > 3.0 * errs[1] > 9.0 * errs[2] and errs[2] < 2.5e-3
+
+
+def test_weighting_rhs_and_superposition(orc):
+    """Weighting potentials of all conductors add up to the potential of the whole system at 1 V (linearity of
+    Eq. 6): on the cube split into two read-out groups, sigma_w1 + sigma_w2 = sigma(all at 1 V)."""
+    pr = W.cube(n_side=4, m_points=0)
+    g = orc.Geometry(pr)
+    K = orc.assemble(g, mode="f64")
+    grp = (np.arange(pr.n) < pr.n // 2).astype(float)
+    b1, b2 = orc.weighting_rhs(g, grp), orc.weighting_rhs(g, 1.0 - grp)
+    assert np.array_equal(b1 + b2, np.ones(pr.n))
+    s1, s2 = orc.solve(K, b1, mode="f64"), orc.solve(K, b2, mode="f64")
+    s = orc.solve(K, orc.rhs(g, mode="f64"), mode="f64")
+    assert np.max(np.abs(s1 + s2 - s)) < 1e-12 * np.max(np.abs(s))
+    mixed = W.thgem(d=10, n_plane=6, n_grid=2)
+    bw = orc.weighting_rhs(orc.Geometry(mixed), np.ones(mixed.n))
+    assert np.all(bw[mixed.bc_kind == W.DIELECTRIC] == 0.0) and np.all(bw[mixed.bc_kind == W.DIRICHLET] == 1.0)
