@@ -71,8 +71,10 @@ enum {
   NEB_STAGE_EVAL = 7,     /* a7 fused element kernel alone                     */
   NEB_STAGE_CHARGES = 8,  /* a8 point-charge direct sum kernel                 */
   NEB_STAGE_REDUCE = 9,   /* fixed-order sum of the per-chunk partials of a7/a8 */
-  NEB_STAGE_COUNT = 10
+  NEB_STAGE_FASTVOL = 10, /* FastVolume: node packing and trilinear lookups    */
+  NEB_STAGE_COUNT = 11
 };
+#define NEB_FASTVOL_SLOTS 4
 
 /* Creates a context on `device`.  `cuda_stream` is a cudaStream_t (e.g. torch's current stream),
  * NULL = the legacy default stream.  NEB_ECUDA if the device is absent or not sm_100. */
@@ -118,8 +120,31 @@ neb_status neb_assemble(neb_ctx* ctx, int64_t n, const int32_t* kind, const doub
  * Errors: NEB_ESTATE before neb_assemble; NEB_ESINGULAR. */
 neb_status neb_solve(neb_ctx* ctx, double* sigma_out);
 
-/* Test hook: sets the charge densities directly (n values, caller's element order). */
+/* Sets the charge densities used by neb_eval / neb_fastvol_build directly (n values, caller's element
+ * order): a test hook, and the way to evaluate a weighting field (sigma from neb_solve_weighting). */
 neb_status neb_set_sigma(neb_ctx* ctx, const double* sigma);
+
+/* Weighting field (P:222 CreateWtFldFastVolPF; reading S26): solves K sigma_w = b_w on the RESIDENT LU
+ * factors, b_w = bc_value_w on Dirichlet rows (1 on the read-out electrode's panels, 0 on every other
+ * conductor), 0 on dielectric rows, no space charge.  bc_value_w and sigma_w_out hold n values in the
+ * caller's element order.  Leaves the context's own sigma and right-hand side untouched.
+ * Errors: NEB_ESTATE before the first neb_solve (no factors yet). */
+neb_status neb_solve_weighting(neb_ctx* ctx, const double* bc_value_w, double* sigma_w_out);
+
+/* FastVolume (P:179, P:222 CreateFastVolPF; reading S25).  neb_fastvol_build precomputes Phi and E, from
+ * the context's current sigma (all elements with their periodic copies) and, if with_charges != 0, the
+ * space charges, at the nx*ny*nz nodes origin + (i hx, j hy, k hz) of a uniform grid and keeps them on the
+ * device in slot `slot` (0 .. NEB_FASTVOL_SLOTS-1; e.g. 0 = field, 1.. = weighting fields); rebuilding a
+ * slot frees the old map.  origin and spacing are 3 HOST doubles each.
+ * neb_fastvol_eval: trilinear interpolation of each of Phi, Ex, Ey, Ez from the 8 nodes of the cell at m
+ * points (3*m SoA, host or device); a point outside the grid's box (beyond a slack of 1e-9 cells) gets NaN.
+ * neb_fastvol_get (test hook): the node values as 4 planes Phi, Ex, Ey, Ez of nx*ny*nz doubles, i fastest.
+ * Errors: NEB_EINVAL (slot, fewer than 2 nodes on an axis, spacing <= 0, more than 2^28 nodes),
+ * NEB_ESTATE (build before sigma exists; eval/get of an empty slot), NEB_ENOMEM. */
+neb_status neb_fastvol_build(neb_ctx* ctx, int32_t slot, int32_t nx, int32_t ny, int32_t nz, const double* origin,
+                             const double* spacing, int32_t with_charges);
+neb_status neb_fastvol_eval(neb_ctx* ctx, int32_t slot, int64_t m, const double* pts, double* phi, double* E);
+neb_status neb_fastvol_get(neb_ctx* ctx, int32_t slot, double* values);
 
 /* PFAtPoint: Phi (m) and E (3*m SoA) at m points pts (3*m SoA) from all elements (with
  * their periodic copies) and all space charges; a charge exactly at a point is skipped

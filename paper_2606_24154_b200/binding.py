@@ -10,7 +10,7 @@ from . import build as _build
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
 NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD = 0, 1, 2, 3, 4
-STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce"]
+STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -53,6 +53,10 @@ def lib():
         L.neb_set_sigma.argtypes = [vp, vp]
         L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
         L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
+        L.neb_solve_weighting.argtypes = [vp, vp, vp]
+        L.neb_fastvol_build.argtypes = [vp, i32, i32, i32, i32, vp, vp, i32]
+        L.neb_fastvol_eval.argtypes = [vp, i32, i64, vp, vp, vp]
+        L.neb_fastvol_get.argtypes = [vp, i32, vp]
         L.neb_push.argtypes = [vp, i64, vp, vp, dbl]
         L.neb_get_matrix.argtypes = [vp, vp]
         L.neb_get_rhs.argtypes = [vp, vp]
@@ -189,6 +193,47 @@ class Neb:
         pos = _check_arr(pos, np.float64, "float64", 3 * q, "pos")
         charge = _check_arr(charge, np.float64, "float64", q, "charge")
         self._ck(self._L.neb_add_space_charge(self._h, q, _ptr(pos), _ptr(charge), 1 if replace else 0))
+
+    def solve_weighting(self, bc_value_w, out=None):
+        """neb_solve_weighting: sigma_w (n) for the weighting potentials bc_value_w (n), on the resident factors."""
+        bc_value_w = _check_arr(bc_value_w, np.float64, "float64", self.n, "bc_value_w")
+        if out is None:
+            out = np.empty(self.n)
+        self._ck(self._L.neb_solve_weighting(self._h, _ptr(bc_value_w), _ptr(out)))
+        return out
+
+    def fastvol_build(self, slot: int, shape, origin, spacing, with_charges: bool = True):
+        """neb_fastvol_build: shape = (nx, ny, nz), origin and spacing 3 floats each (host)."""
+        nx, ny, nz = (int(v) for v in shape)
+        origin = np.ascontiguousarray(origin, dtype=np.float64)
+        spacing = np.ascontiguousarray(spacing, dtype=np.float64)
+        if origin.shape != (3,) or spacing.shape != (3,):
+            raise ValueError("origin and spacing must hold 3 values")
+        self._ck(self._L.neb_fastvol_build(self._h, slot, nx, ny, nz, _ptr(origin), _ptr(spacing), 1 if with_charges else 0))
+        self._fv_nodes = getattr(self, "_fv_nodes", {})
+        self._fv_nodes[slot] = nx * ny * nz
+
+    def fastvol_eval(self, slot: int, pts, phi=None, E=None):
+        m = int(pts.shape[1])
+        pts = _check_arr(pts, np.float64, "float64", 3 * m, "pts")
+        if isinstance(pts, np.ndarray):
+            phi = np.empty(m) if phi is None else phi
+            E = np.empty((3, m)) if E is None else E
+        else:
+            import torch
+            phi = torch.empty(m, dtype=torch.float64, device=pts.device) if phi is None else phi
+            E = torch.empty((3, m), dtype=torch.float64, device=pts.device) if E is None else E
+        self._ck(self._L.neb_fastvol_eval(self._h, slot, m, _ptr(pts), _ptr(phi), _ptr(E)))
+        return phi, E
+
+    def fastvol_get(self, slot: int):
+        """Node values (4, nx*ny*nz): Phi, Ex, Ey, Ez (test hook)."""
+        nn = getattr(self, "_fv_nodes", {}).get(slot)
+        if nn is None:
+            raise NebError(3, "fastvol_get: empty slot")
+        v = np.empty((4, nn))
+        self._ck(self._L.neb_fastvol_get(self._h, slot, _ptr(v)))
+        return v
 
     def push(self, pos, E, mu_dt: float):
         q = int(pos.shape[1])

@@ -346,6 +346,8 @@ void neb_destroy(neb_ctx* c) {
   if (c->d_panel_ws) cudaFree(c->d_panel_ws);
   if (c->d_charges) cudaFree(c->d_charges);
   if (c->d_scratch) cudaFree(c->d_scratch);
+  for (int s = 0; s < NEB_FASTVOL_SLOTS; ++s)
+    if (c->fastvol[s].nodes) cudaFree((void*)c->fastvol[s].nodes);
   if (c->pool) cudaMemPoolDestroy(c->pool);
   if (c->side_stream) { cudaStreamSynchronize(c->side_stream); cudaStreamDestroy(c->side_stream); }
   if (c->ev_next) cudaEventDestroy(c->ev_next);
@@ -538,6 +540,59 @@ neb_status neb_eval(neb_ctx* c, int64_t m, const double* pts, double* phi, doubl
   NEB_TRY(sg.out(phi, sizeof(double) * m, &dphi));
   NEB_TRY(sg.out(E, sizeof(double) * 3 * m, &dE));
   NEB_TRY(field_at_points(c, m, (const double*)dp, true, true, (double*)dphi, (double*)dE));
+  return sg.finish();
+}
+
+neb_status neb_solve_weighting(neb_ctx* c, const double* bc_value_w, double* sigma_w_out) {
+  if (!c || !bc_value_w || !sigma_w_out) return NEB_EINVAL;
+  if (!c->factored || !c->assembled) return fail(c, NEB_ESTATE, "neb_solve_weighting before the first neb_solve (no LU factors)");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  const void* dw;
+  void* dout;
+  NEB_TRY(sg.in(bc_value_w, sizeof(double) * c->n, &dw));
+  NEB_TRY(sg.out(sigma_w_out, sizeof(double) * c->n, &dout));
+  NEB_TRY(solve_weighting(c, (const double*)dw, (double*)dout));
+  return sg.finish();
+}
+
+neb_status neb_fastvol_build(neb_ctx* c, int32_t slot, int32_t nx, int32_t ny, int32_t nz, const double* origin,
+                             const double* spacing, int32_t with_charges) {
+  if (!c || !origin || !spacing) return NEB_EINVAL;
+  if (slot < 0 || slot >= NEB_FASTVOL_SLOTS || nx < 2 || ny < 2 || nz < 2 || (int64_t)nx * ny * nz > (1LL << 28))
+    return fail(c, NEB_EINVAL, "neb_fastvol_build: slot out of range, fewer than 2 nodes on an axis, or more than 2^28 nodes");
+  for (int a = 0; a < 3; ++a)
+    if (!(spacing[a] > 0.0) || !isfinite(origin[a]) || !isfinite(spacing[a]))
+      return fail(c, NEB_EINVAL, "neb_fastvol_build: spacing must be positive and finite");
+  if (!c->have_sigma) return fail(c, NEB_ESTATE, "neb_fastvol_build before neb_solve / neb_set_sigma");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  return fastvol_build(c, slot, nx, ny, nz, origin, spacing, with_charges != 0);
+}
+
+neb_status neb_fastvol_eval(neb_ctx* c, int32_t slot, int64_t m, const double* pts, double* phi, double* E) {
+  if (!c || m < 0 || (m > 0 && !pts) || slot < 0 || slot >= NEB_FASTVOL_SLOTS) return NEB_EINVAL;
+  if (!c->fastvol[slot].nodes) return fail(c, NEB_ESTATE, "neb_fastvol_eval: empty slot (call neb_fastvol_build)");
+  if (m == 0) return NEB_OK;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  const void* dp;
+  void *dphi, *dE;
+  NEB_TRY(sg.in(pts, sizeof(double) * 3 * m, &dp));
+  NEB_TRY(sg.out(phi, sizeof(double) * m, &dphi));
+  NEB_TRY(sg.out(E, sizeof(double) * 3 * m, &dE));
+  NEB_TRY(fastvol_eval(c, slot, m, (const double*)dp, (double*)dphi, (double*)dE));
+  return sg.finish();
+}
+
+neb_status neb_fastvol_get(neb_ctx* c, int32_t slot, double* values) {
+  if (!c || !values || slot < 0 || slot >= NEB_FASTVOL_SLOTS) return NEB_EINVAL;
+  const FastVol& fv = c->fastvol[slot];
+  if (!fv.nodes) return fail(c, NEB_ESTATE, "neb_fastvol_get: empty slot");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  void* dout;
+  NEB_TRY(sg.out(values, sizeof(double) * 4 * (size_t)fv.nx * fv.ny * fv.nz, &dout));
+  NEB_TRY(fastvol_get(c, slot, (double*)dout));
   return sg.finish();
 }
 

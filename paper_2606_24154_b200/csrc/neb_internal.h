@@ -22,6 +22,13 @@ struct GeoTables {
   int32_t n_rect, n_tri, n_wire;
 };
 
+// One FastVolume map (neb_fastvol.cu): a 32-byte record (Phi, Ex, Ey, Ez) per node, i fastest.
+struct FastVol {
+  const double4* nodes = nullptr;
+  int nx = 0, ny = 0, nz = 0;
+  double o[3] = {0, 0, 0}, h[3] = {1, 1, 1};
+};
+
 struct StageStat {
   double ms = 0.0;
   int64_t launches = 0;
@@ -74,6 +81,8 @@ struct neb_ctx {
   // space charges: SoA x,y,z,q (4 * q_cap)
   double* d_charges = nullptr;
   int64_t q = 0, q_cap = 0;
+
+  neb::FastVol fastvol[NEB_FASTVOL_SLOTS];
 
   // scratch for partial sums / staging
   double* d_scratch = nullptr;
@@ -128,6 +137,12 @@ size_t lu_panel_ws_bytes(int num_sms);
 // neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
 int64_t panel_cluster_max_rows(neb_ctx* c);
 neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream);
+
+// neb_fastvol.cu (device pointers only; the ABI wrappers in neb_api.cu stage host arrays) --------------
+neb_status fastvol_build(neb_ctx* c, int slot, int nx, int ny, int nz, const double* origin, const double* spacing, bool with_charges);
+neb_status fastvol_eval(neb_ctx* c, int slot, int64_t m, const double* d_pts, double* d_phi, double* d_E);
+neb_status fastvol_get(neb_ctx* c, int slot, double* d_values);
+neb_status solve_weighting(neb_ctx* c, const double* d_w_caller, double* d_sigma_out);
 
 // neb_peaks.cu ------------------------------------------------------------------------------------
 neb_status fp64_peak(neb_ctx* c, int kind, double* tflops);

@@ -473,6 +473,92 @@ def test_c4_dynamic_loop_reduced(nb, orc):
 
 
 # ---------------------------------------------------------------------------------------------
+# FastVolume and weighting field
+# ---------------------------------------------------------------------------------------------
+def test_fastvol_build_and_lookup(nb, orc, P):
+    """Node values of the map = direct evaluation (oracle) at the nodes; lookups = the oracle's trilinear
+    interpolation of ORACLE-computed node values; ragged sizes, points on the faces, outside -> NaN; host and
+    device pointers; space charges in or out."""
+    import torch
+    pr = W.thgem(d=10, n_plane=8, n_grid=4)
+    rs = np.random.RandomState(11)
+    pr.charge_pos = rs.normal(size=(3, 500)) * 1e-4 + np.array([[0.0], [0.0], [1e-3]])
+    pr.charge_q = np.full(500, W.Q_E * 1e4)
+    g = orc.Geometry(pr)
+    nb.assemble_problem(pr)
+    nb.add_space_charge(pr.charge_pos, pr.charge_q)
+    s = nb.solve()
+    shape, o, h = (9, 7, 13), np.array([-0.4e-3, -0.3e-3, 0.4e-3]), np.array([0.1e-3, 0.1e-3, 0.15e-3])
+    nodes = orc.fastvol_nodes(*shape, o, h)
+    for slot, with_q in ((0, True), (2, False)):
+        nb.fastvol_build(slot, shape, o, h, with_charges=with_q)
+        vals = nb.fastvol_get(slot)
+        ph_o, E_o = orc.evaluate(g, s, nodes, pr.charge_pos if with_q else None, pr.charge_q if with_q else None)
+        check_field(vals[0], vals[1:], ph_o, E_o, TOL_FAR, f"fastvol nodes slot {slot}")
+        ext = h * (np.array(shape) - 1)
+        pts = o[:, None] + rs.rand(3, 3001) * ext[:, None]
+        pts[:, :40] = nodes[:, rs.choice(nodes.shape[1], 40)]              # exactly on nodes (faces included)
+        pts[0, 40:60] = o[0] + ext[0]                                      # on the upper x face
+        pts[2, 60:70] = o[2] - 1e-6                                        # outside
+        pts[1, 70:80] = o[1] + ext[1] + 1e-6
+        phi, E = nb.fastvol_eval(slot, pts)
+        phi_i, E_i = orc.fastvol_eval(shape, o, h, np.vstack([ph_o[None], E_o]), pts)
+        out = np.zeros(pts.shape[1], dtype=bool)
+        out[60:80] = True
+        assert np.all(np.isnan(phi[out])) and np.all(np.isnan(E[:, out])) and np.all(np.isnan(phi_i[out]))
+        assert not np.any(np.isnan(phi[~out])) and not np.any(np.isnan(E[:, ~out]))
+        check_field(phi[~out], E[:, ~out], phi_i[~out], E_i[:, ~out], TOL_FAR, f"fastvol lookup slot {slot}")
+        d_phi, d_E = nb.fastvol_eval(slot, torch.from_numpy(pts).cuda())
+        assert np.array_equal(d_phi.cpu().numpy(), phi, equal_nan=True) and np.array_equal(d_E.cpu().numpy(), E, equal_nan=True)
+    # interpolation error against direct evaluation: small on this grid, and it is an approximation (not parity)
+    phi_d, E_d = nb.eval(pts[:, 100:600])
+    phi_f, _ = nb.fastvol_eval(0, pts[:, 100:600])
+    assert np.max(np.abs(phi_f - phi_d)) < 0.05 * np.max(np.abs(phi_d))
+    with pytest.raises(P.NebError) as e:
+        nb.fastvol_eval(1, pts)                                            # empty slot
+    assert e.value.status == 3
+    with pytest.raises(P.NebError) as e:
+        nb.fastvol_build(0, (1, 4, 4), o, h)
+    assert e.value.status == 1
+    with pytest.raises(P.NebError) as e:
+        nb.fastvol_build(7, (4, 4, 4), o, h)
+    assert e.value.status == 1
+
+
+def test_weighting_solve_and_map(nb, orc):
+    """Weighting potential of one read-out group: sigma_w against the oracle's solve of the oracle's weighting
+    right-hand side; the physical sigma and right-hand side stay untouched; the weighting solutions of a partition of
+    the conductors add up to the solution with every conductor at 1 V; weighting-field map through slot 1."""
+    pr = W.thgem(d=10, n_plane=8, n_grid=4)
+    g = orc.Geometry(pr)
+    K = orc.assemble(g)
+    nb.assemble_problem(pr)
+    s = nb.solve()
+    b = nb.get_rhs()
+    top = (pr.bc_kind == W.DIRICHLET) & (pr.centroids()[2] > 2.9e-3)       # the drift plane as read-out electrode
+    assert top.sum() == 64
+    w = top.astype(float)
+    sw = nb.solve_weighting(w)
+    so = orc.solve(K, orc.weighting_rhs(g, w))
+    assert np.max(np.abs(sw - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    rest = ((pr.bc_kind == W.DIRICHLET) & ~top).astype(float)
+    s_all = nb.solve_weighting(np.ones(pr.n))
+    assert np.max(np.abs(sw + nb.solve_weighting(rest) - s_all)) <= 1e-12 * np.max(np.abs(s_all))
+    assert np.array_equal(nb.get_rhs(), b)                                 # untouched by the weighting solves
+    phi0, _ = nb.eval(pr.points)
+    phi_o, _ = orc.evaluate(g, s, pr.points)
+    assert rel_err(phi0, phi_o).max() <= TOL_FAR                           # still the physical sigma
+    nb.set_sigma(sw)
+    shape, o, h = (5, 5, 9), np.array([-0.4e-3, -0.4e-3, 0.5e-3]), np.array([0.2e-3, 0.2e-3, 0.25e-3])
+    nb.fastvol_build(1, shape, o, h, with_charges=False)
+    vals = nb.fastvol_get(1)
+    ph_w, E_w = orc.evaluate(g, so, orc.fastvol_nodes(*shape, o, h))
+    check_field(vals[0], vals[1:], ph_w, E_w, TOL_FAR, "weighting map")
+    assert 0.0 < vals[0].min() and vals[0].max() < 1.0                     # a weighting potential lies in (0, 1)
+    nb.set_sigma(s)
+
+
+# ---------------------------------------------------------------------------------------------
 # edge cases and error behaviour of the ABI
 # ---------------------------------------------------------------------------------------------
 def test_edge_cases_and_errors(nb, P, orc):
