@@ -334,6 +334,51 @@ def main():
     achieved = flop_pair * eval_pairs / (eval_ms * 1e-3) * 1e-12
     lu_flop = 2.0 / 3.0 * n ** 3
 
+    fastvol = None
+    if name == "C2" and rank == 0:
+        # the 100^3 field map of C2 as a FastVolume (same nodes as the eval points), then 1e7
+        # trilinear lookups at seeded points inside it.  Bound by memory: 24 B of coordinates in, 32 B of results out
+        # and 8 node records of 32 B per point (the 32 MB map stays in L2), reported against the measured HBM copy rate.
+        from workloads import rng
+        ng = int(round(m ** (1.0 / 3.0)))
+        o = np.array([pr.points[0].min(), pr.points[1].min(), pr.points[2].min()])
+        hh = (np.array([pr.points[0].max(), pr.points[1].max(), pr.points[2].max()]) - o) / (ng - 1)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        nb.fastvol_build(0, (ng, ng, ng), o, hh)
+        ev1.record()
+        torch.cuda.synchronize()
+        build_ms = ev0.elapsed_time(ev1)
+        ml = 10_000_000
+        lp = torch.from_numpy(np.stack([o[k] + rng.uniform(7, ml, 0.0, 1.0, offset=k * ml) * hh[k] * (ng - 1) for k in range(3)])).to(dev)
+        l_phi = torch.empty(ml, dtype=torch.float64, device=dev)
+        l_E = torch.empty((3, ml), dtype=torch.float64, device=dev)
+        for _ in range(3):
+            nb.fastvol_eval(0, lp, phi=l_phi, E=l_E)
+        t_l = []
+        for _ in range(10):
+            flush.fill_(1)
+            ev0.record()
+            nb.fastvol_eval(0, lp, phi=l_phi, E=l_E)
+            ev1.record()
+            torch.cuda.synchronize()
+            t_l.append(ev0.elapsed_time(ev1))
+        look_ms = sum(t_l) / len(t_l)
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+            src = "MEASURED_PEAKS.json hbm_gbs (measured copy rate)"
+        except Exception:
+            hbm_peak, src = 6650.0, "fallback 6.65 TB/s of B200_PROFILING.md"
+        gbs = ml * (24 + 32 + 8 * 32) / (look_ms * 1e-3) * 1e-9
+        fastvol = {"grid": [ng, ng, ng], "build_ms": build_ms, "lookups": ml, "lookup_ms": look_ms,
+                   "lookup_points_per_s": ml / (look_ms * 1e-3),
+                   "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                                "bytes_per_point": 24 + 32 + 8 * 32, "peak_source": src,
+                                "hbm_only_gbs": ml * (24 + 32) / (look_ms * 1e-3) * 1e-9,
+                                "note": "algorithmic bytes incl. the 8 node records per point; the 32 MB map is served by "
+                                        "L2, so only the 56 B/point of coordinates and results (hbm_only_gbs) cross HBM"}}
+        del lp, l_phi, l_E
+
     if rank == 0:
         value = pairs_step * args.steps * world / (ms * 1e-3)
         line = {
@@ -358,6 +403,8 @@ def main():
                    "tflops_trailing_update": lu_flop / (stages["lu_gemm"] * 1e-3) * 1e-12 if stages.get("lu_gemm") else None,
                    "dmma_peak_tflops": dmma_peak},
         }
+        if fastvol:
+            line["fastvol"] = fastvol
         if not args.no_cpu_baseline and world == 1:
             if name == "C1":
                 line["cpu_baseline"] = cpu_baseline_run(pr, with_lu=True)      # the whole C1 step, LU included
