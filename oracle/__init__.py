@@ -199,3 +199,29 @@ def weighting_rhs(g: Geometry, bc_value_w) -> np.ndarray:
     electrode's panels at their weighting potential (1), every other conductor at 0, no space charge;
     dielectric rows stay homogeneous (0)."""
     return np.where(g.bc_kind == 0, np.asarray(bc_value_w, dtype=np.float64), 0.0)
+
+
+def voxelize(charge_pos, charge_q, origin, voxel, dims):
+    """Alg. 3 (reading S27): point charges -> line charges.  Returns lines (5, nl): x, y, z_start,
+    z_stop, lambda, in voxel-index order."""
+    pos, ch = _d(charge_pos), _d(charge_q)
+    origin, voxel = _d(np.asarray(origin, dtype=np.float64)), _d(np.asarray(voxel, dtype=np.float64))
+    dims = np.ascontiguousarray(dims, dtype=np.int32)
+    q = int(ch.shape[0])
+    cap = int(min(q, int(np.prod(dims.astype(np.int64))))) or 1
+    lines = np.zeros((5, cap))
+    L = _lib("f64")
+    L.orc_voxelize.restype = C.c_int64
+    nl = L.orc_voxelize(C.c_int64(q), _p(pos), _p(ch), _p(origin), _p(voxel), _p(dims, _ip), C.c_int64(cap), _p(lines))
+    if nl < 0:
+        raise RuntimeError("oracle voxelize: capacity")
+    return np.ascontiguousarray(lines[:, :nl])
+
+
+def line_charges(pts, lines, mode="ld"):
+    """Phi (m), E (3, m) of line charges (5, nl) parallel to z at pts (3, m)."""
+    pts, lines = _d(pts), _d(lines)
+    m, nl = pts.shape[1], lines.shape[1]
+    phi, E = np.zeros(m), np.zeros((3, m))
+    _lib(mode).orc_line_charges(C.c_int64(m), _p(pts), C.c_int64(nl), C.c_int64(nl), _p(lines), _p(phi), _p(E))
+    return phi, E

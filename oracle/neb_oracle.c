@@ -539,3 +539,77 @@ void orc_fastvol_eval(int32_t nx, int32_t ny, int32_t nz, const double* origin, 
     E[p] = out[1]; E[m + p] = out[2]; E[2 * m + p] = out[3];
   }
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Alg. 3 "Point to Line Charge Reduction (Voxelization)": dense clusters of point charges
+ * are mapped into representative line charges.  Reading (S27): the grid has dims[a] voxels of
+ * size voxel[a] from origin[a]; the voxel index of a point is floor((p - origin)/voxel) per axis, clamped
+ * to the grid (a point outside is counted in the nearest border voxel, so that the total charge is
+ * conserved); a voxel is occupied when at least one point fell in it (Alg. 3's isOccupied), even if its
+ * charges cancel; an occupied voxel becomes ONE line charge through the voxel's centre, parallel to z,
+ * spanning the voxel's z extent, of line density lambda = (total charge of the voxel) / voxel[2].  Lines
+ * are listed in voxel-index order (x fastest).  Kernel 1 = the scatter loop, Kernel 2 = the line loop.
+ * lines: 5*cap doubles SoA  x, y, z_start, z_stop, lambda.  Returns the number of lines (<= cap), or -1
+ * if cap is too small.
+ * ------------------------------------------------------------------------------------------------ */
+int64_t orc_voxelize(int64_t q, const double* pos, const double* charge, const double* origin, const double* voxel,
+                     const int32_t* dims, int64_t cap, double* lines) {
+  const int64_t nv = (int64_t)dims[0] * dims[1] * dims[2];
+  long double* total = (long double*)calloc((size_t)nv, sizeof(long double));
+  unsigned char* occupied = (unsigned char*)calloc((size_t)nv, 1);
+  for (int64_t c = 0; c < q; ++c) {                                /* Kernel 1: Voxelize (Scatter) */
+    int64_t idx[3];
+    for (int a = 0; a < 3; ++a) {
+      int64_t i = (int64_t)floor((pos[a * q + c] - origin[a]) / voxel[a]);   /* decided in double, like the GPU */
+      if (i < 0) i = 0;
+      if (i > dims[a] - 1) i = dims[a] - 1;
+      idx[a] = i;
+    }
+    const int64_t v = (idx[2] * dims[1] + idx[1]) * dims[0] + idx[0];
+    total[v] += (long double)charge[c];
+    occupied[v] = 1;
+  }
+  int64_t nl = 0;
+  for (int64_t v = 0; v < nv; ++v) {                               /* Kernel 2: Generate Lines (Reduce) */
+    if (!occupied[v]) continue;
+    if (nl >= cap) { nl = -1; break; }
+    const int64_t i = v % dims[0], j = (v / dims[0]) % dims[1], k = v / ((int64_t)dims[0] * dims[1]);
+    lines[0 * cap + nl] = origin[0] + ((double)i + 0.5) * voxel[0];
+    lines[1 * cap + nl] = origin[1] + ((double)j + 0.5) * voxel[1];
+    lines[2 * cap + nl] = origin[2] + (double)k * voxel[2];
+    lines[3 * cap + nl] = origin[2] + (double)(k + 1) * voxel[2];
+    lines[4 * cap + nl] = (double)(total[v] / (long double)voxel[2]);
+    ++nl;
+  }
+  free(total);
+  free(occupied);
+  return nl;
+}
+
+/* Potential and field of nl straight line charges parallel to z (uniform line density lambda, C/m) at m
+ * points: the defining integral  Phi = (1/4 pi eps0) Int lambda dz' / |r - r'|  (Eq. 2 P:68 integrated along
+ * the line; the wire integral P:131 without its radius) in closed form, with l1 = z_start - Z, l2 = z_stop - Z,
+ * rho^2 = dx^2 + dy^2, R_i = sqrt(rho^2 + l_i^2):
+ *   Phi = k lambda [asinh(l2/rho) - asinh(l1/rho)],  E_rho = k lambda (l2/R2 - l1/R1)/rho,  E_z = k lambda (1/R2 - 1/R1).
+ * A point exactly on a line's axis (rho = 0) is skipped, like r = 0 in Alg. 2 (reading S27). */
+void orc_line_charges(int64_t m, const double* pts, int64_t nl, int64_t cap, const double* lines, double* phi, double* E) {
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t p = 0; p < m; ++p) {
+    long double acc[4] = {0, 0, 0, 0};
+    for (int64_t c = 0; c < nl; ++c) {
+      real dx = (real)pts[p] - (real)lines[c], dy = (real)pts[m + p] - (real)lines[cap + c];
+      real l1 = (real)lines[2 * cap + c] - (real)pts[2 * m + p], l2 = (real)lines[3 * cap + c] - (real)pts[2 * m + p];
+      real rho2 = dx * dx + dy * dy;
+      if (!(rho2 > 0)) continue;
+      real rho = R_SQRT(rho2), R1 = R_SQRT(rho2 + l1 * l1), R2 = R_SQRT(rho2 + l2 * l2);
+      real lam = (real)lines[4 * cap + c];
+      real er = lam * (l2 / R2 - l1 / R1) / rho2;      /* E_rho / rho */
+      acc[0] += lam * (R_ASINH(l2 / rho) - R_ASINH(l1 / rho));
+      acc[1] += er * dx;
+      acc[2] += er * dy;
+      acc[3] += lam * (1 / R2 - 1 / R1);
+    }
+    if (phi) phi[p] = (double)(acc[0] * K_COULOMB);
+    if (E) { E[p] = (double)(acc[1] * K_COULOMB); E[m + p] = (double)(acc[2] * K_COULOMB); E[2 * m + p] = (double)(acc[3] * K_COULOMB); }
+  }
+}

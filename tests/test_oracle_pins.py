@@ -548,3 +548,73 @@ def test_weighting_rhs_and_superposition(orc):
     mixed = W.thgem(d=10, n_plane=6, n_grid=2)
     bw = orc.weighting_rhs(orc.Geometry(mixed), np.ones(mixed.n))
     assert np.all(bw[mixed.bc_kind == W.DIELECTRIC] == 0.0) and np.all(bw[mixed.bc_kind == W.DIRICHLET] == 1.0)
+
+
+# ---------------------------------------------------------------------------------------------
+# Alg. 3: voxelisation of point charges into line charges
+# ---------------------------------------------------------------------------------------------
+def test_line_charge_against_quadrature_and_limits(orc):
+    """The closed form of a line charge against Gauss-Legendre quadrature of Eq. (2) P:68 along the line, against
+    the (already pinned) thin-wire routine outside its radius, E = -grad Phi, and the point-charge limit."""
+    lines = np.array([[0.3e-3], [-0.2e-3], [0.1e-3], [0.5e-3], [2.0e-9]])        # x, y, z1, z2, lambda
+    rs = np.random.RandomState(3)
+    pts = rs.normal(size=(3, 12)) * 1e-3
+    phi, E = orc.line_charges(pts, lines)
+    xg, wg = np.polynomial.legendre.leggauss(200)
+    zc, hl = 0.5 * (lines[2, 0] + lines[3, 0]), 0.5 * (lines[3, 0] - lines[2, 0])
+    for p in range(pts.shape[1]):
+        zq = zc + hl * xg
+        d = np.stack([np.full_like(zq, pts[0, p] - lines[0, 0]), np.full_like(zq, pts[1, p] - lines[1, 0]), pts[2, p] - zq])
+        r = np.linalg.norm(d, axis=0)
+        if r.min() < 5e-5:
+            continue                                                              # quadrature needs distance
+        phi_q = orc.K_COULOMB * lines[4, 0] * hl * np.sum(wg / r)
+        E_q = orc.K_COULOMB * lines[4, 0] * hl * np.sum(wg * d / r ** 3, axis=1)
+        assert abs(phi[p] - phi_q) < 1e-11 * abs(phi_q) and np.max(np.abs(E[:, p] - E_q)) < 1e-10 * np.linalg.norm(E_q)
+    # the pinned wire formula (surface density sigma on radius r_w: lambda = 2 pi r_w sigma) outside the radius
+    rw = 1e-6
+    inf = np.array([orc.influence(W.WIRE, [lines[0, 0], lines[1, 0], lines[2, 0]], [0, 0, 2 * hl], [1, 0, 0], pts[:, p], radius=rw)
+                    for p in range(pts.shape[1])])
+    sig = lines[4, 0] / (2 * np.pi * rw)
+    assert np.max(np.abs(orc.K_COULOMB * sig * inf[:, 0] - phi)) < 1e-12 * np.max(np.abs(phi))
+    assert np.max(np.abs(orc.K_COULOMB * sig * inf[:, 1:].T - E)) < 1e-12 * np.max(np.abs(E))
+    h = 1e-8
+    for k in range(3):
+        dp = np.zeros((3, 1)); dp[k] = h
+        g = (orc.line_charges(pts + dp, lines)[0] - orc.line_charges(pts - dp, lines)[0]) / (2 * h)
+        assert np.max(np.abs(E[k] + g)) < 1e-6 * np.max(np.abs(E))
+    far = np.array([[0.2], [0.1], [-0.3]])
+    phi_f, _ = orc.line_charges(far, lines)
+    q = lines[4, 0] * 2 * hl
+    assert abs(phi_f[0] - orc.K_COULOMB * q / np.linalg.norm(far[:, 0] - [lines[0, 0], lines[1, 0], zc])) < 1e-5 * abs(phi_f[0])
+    on_axis = np.array([[lines[0, 0]], [lines[1, 0]], [1e-3]])                    # rho = 0: skipped
+    assert orc.line_charges(on_axis, lines)[0][0] == 0.0
+
+
+def test_voxelize_against_brute_force_histogram(orc):
+    rs = np.random.RandomState(8)
+    q = 5000
+    pos = rs.normal(size=(3, q)) * 1.2e-4
+    ch = rs.choice([1.0, -1.0, 2.0], size=q) * W.Q_E
+    o, d, dims = np.array([-3e-4, -2e-4, -2.5e-4]), np.array([1e-4, 0.8e-4, 0.5e-4]), np.array([6, 5, 10])
+    lines = orc.voxelize(pos, ch, o, d, dims)
+    idx = np.stack([np.clip(np.floor((pos[a] - o[a]) / d[a]).astype(int), 0, dims[a] - 1) for a in range(3)])
+    flat = (idx[2] * dims[1] + idx[1]) * dims[0] + idx[0]
+    tot = np.zeros(dims.prod()); np.add.at(tot, flat, ch)
+    occ = np.zeros(dims.prod(), dtype=bool); occ[flat] = True
+    v = np.nonzero(occ)[0]
+    assert lines.shape == (5, v.size) and v.size < q                              # N_voxels << N_points
+    assert np.allclose(lines[4] * d[2], tot[v], rtol=1e-12, atol=1e-30)
+    assert abs(np.sum(lines[4]) * d[2] - ch.sum()) < 1e-12 * np.abs(ch).sum()      # total charge conserved (clamped points too)
+    i, j, k = v % dims[0], (v // dims[0]) % dims[1], v // (dims[0] * dims[1])
+    assert np.allclose(lines[0], o[0] + (i + 0.5) * d[0], rtol=0, atol=1e-18) and np.allclose(lines[1], o[1] + (j + 0.5) * d[1], rtol=0, atol=1e-18)
+    assert np.allclose(lines[2], o[2] + k * d[2], rtol=0, atol=1e-18) and np.allclose(lines[3] - lines[2], d[2], rtol=1e-12)
+    assert np.any(idx[0] == 0) and (np.floor((pos[0] - o[0]) / d[0]) < 0).any()    # some points were clamped
+    # far from the cloud the lines reproduce the points' field (monopole exactly, dipole up to voxel size / distance)
+    pts = np.array([[3e-3, 6e-3], [1e-3, 2e-3], [-2e-3, -4e-3]])
+    same = np.full(q, W.Q_E)
+    l2 = orc.voxelize(pos, same, o, d, dims)
+    p_pt, _ = orc.point_charges(pts, pos, same)
+    p_ln, _ = orc.line_charges(pts, l2)
+    err = np.abs(p_ln - p_pt) / np.abs(p_pt)
+    assert np.all(err < 1e-3)
