@@ -155,6 +155,22 @@ neb_status neb_eval(neb_ctx* ctx, int64_t m, const double* pts, double* phi, dou
  * replace != 0 discards the charges held so far; q = 0 with replace clears them. */
 neb_status neb_add_space_charge(neb_ctx* ctx, int64_t q, const double* pos, const double* charge, int32_t replace);
 
+/* Alg. 3, Point to Line Charge Reduction (Voxelization; reading S27): replaces the point charges
+ * the context holds by line charges.  Grid of dims[a] voxels of size voxel[a] (m) from origin[a] (3 HOST values
+ * each); voxel index = floor((p - origin)/voxel), clamped to the grid (a point outside counts in the nearest border
+ * voxel: the total charge is conserved); every voxel that received at least one point becomes ONE line charge
+ * through its centre, parallel to z, spanning its z extent, lambda = (its total charge)/voxel[2]; lines are kept
+ * in voxel-index order (x fastest).  From then on neb_eval and the right-hand side of neb_solve sum over the lines
+ * (closed form of Eq. 2 integrated along the line; a point exactly on a line's axis is skipped) and over any point
+ * charges added LATER with replace = 0; neb_add_space_charge with replace != 0 discards lines and points.
+ * n_lines_out (host, may be NULL) receives the number of lines.  Voxel totals are accumulated with atomics
+ * (order-dependent rounding in the last bit unless all charges are equal).
+ * neb_get_line_charges (test hook): 5*n_lines doubles SoA x, y, z_start, z_stop, lambda.
+ * Errors: NEB_EINVAL (non-positive voxel size, dims < 1, more than 2^26 voxels), NEB_ESTATE (no point charges). */
+neb_status neb_voxelize_space_charge(neb_ctx* ctx, const double* origin, const double* voxel, const int32_t* dims,
+                                     int64_t* n_lines_out);
+neb_status neb_get_line_charges(neb_ctx* ctx, double* lines);
+
 /* Charge push of the synthetic dynamic loop (BASELINE configs[4], reading S23): pos += mu_dt * E,
  * 3*q values, in place.  Stateless; pos and E must both be device or both be host pointers. */
 neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, double mu_dt);

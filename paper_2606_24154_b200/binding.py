@@ -54,6 +54,8 @@ def lib():
         L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
         L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
         L.neb_solve_weighting.argtypes = [vp, vp, vp]
+        L.neb_voxelize_space_charge.argtypes = [vp, vp, vp, vp, C.POINTER(i64)]
+        L.neb_get_line_charges.argtypes = [vp, vp]
         L.neb_fastvol_build.argtypes = [vp, i32, i32, i32, i32, vp, vp, i32]
         L.neb_fastvol_eval.argtypes = [vp, i32, i64, vp, vp, vp]
         L.neb_fastvol_get.argtypes = [vp, i32, vp]
@@ -234,6 +236,24 @@ class Neb:
         v = np.empty((4, nn))
         self._ck(self._L.neb_fastvol_get(self._h, slot, _ptr(v)))
         return v
+
+    def voxelize_space_charge(self, origin, voxel, dims) -> int:
+        """neb_voxelize_space_charge (Alg. 3): the held point charges become line charges; returns their number."""
+        origin = np.ascontiguousarray(origin, dtype=np.float64)
+        voxel = np.ascontiguousarray(voxel, dtype=np.float64)
+        dims = np.ascontiguousarray(dims, dtype=np.int32)
+        if origin.shape != (3,) or voxel.shape != (3,) or dims.shape != (3,):
+            raise ValueError("origin, voxel and dims must hold 3 values")
+        nl = C.c_int64(0)
+        self._ck(self._L.neb_voxelize_space_charge(self._h, _ptr(origin), _ptr(voxel), _ptr(dims), C.byref(nl)))
+        self._n_lines = int(nl.value)
+        return self._n_lines
+
+    def get_line_charges(self):
+        """(5, n_lines): x, y, z_start, z_stop, lambda (test hook)."""
+        out = np.empty((5, getattr(self, "_n_lines", 0)))
+        self._ck(self._L.neb_get_line_charges(self._h, _ptr(out)))
+        return out
 
     def push(self, pos, E, mu_dt: float):
         q = int(pos.shape[1])

@@ -345,6 +345,7 @@ void neb_destroy(neb_ctx* c) {
   if (c->d_flag) cudaFree(c->d_flag);
   if (c->d_panel_ws) cudaFree(c->d_panel_ws);
   if (c->d_charges) cudaFree(c->d_charges);
+  if (c->d_lines) cudaFree(c->d_lines);
   if (c->d_scratch) cudaFree(c->d_scratch);
   for (int s = 0; s < NEB_FASTVOL_SLOTS; ++s)
     if (c->fastvol[s].nodes) cudaFree((void*)c->fastvol[s].nodes);
@@ -599,7 +600,7 @@ neb_status neb_fastvol_get(neb_ctx* c, int32_t slot, double* values) {
 neb_status neb_add_space_charge(neb_ctx* c, int64_t q, const double* pos, const double* charge, int32_t replace) {
   if (!c || q < 0 || (q > 0 && (!pos || !charge))) return NEB_EINVAL;
   NEB_CUDA(c, cudaSetDevice(c->device));
-  if (replace) c->q = 0;
+  if (replace) { c->q = 0; c->n_lines = 0; }
   if (q == 0) return NEB_OK;
   int64_t need = c->q + q;
   if (need > c->q_cap) {
@@ -622,6 +623,28 @@ neb_status neb_add_space_charge(neb_ctx* c, int64_t q, const double* pos, const 
     NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + f * c->q_cap + c->q, pos + f * q, sizeof(double) * q, kp, c->stream));
   NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + 3 * c->q_cap + c->q, charge, sizeof(double) * q, kq, c->stream));
   c->q = need;
+  return NEB_OK;
+}
+
+neb_status neb_voxelize_space_charge(neb_ctx* c, const double* origin, const double* voxel, const int32_t* dims, int64_t* n_lines_out) {
+  if (!c || !origin || !voxel || !dims) return NEB_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if (!(voxel[a] > 0.0) || !isfinite(voxel[a]) || !isfinite(origin[a]) || dims[a] < 1)
+      return fail(c, NEB_EINVAL, "neb_voxelize_space_charge: voxel sizes must be positive and finite, dims >= 1");
+  if ((int64_t)dims[0] * dims[1] * dims[2] > (1LL << 26)) return fail(c, NEB_EINVAL, "neb_voxelize_space_charge: more than 2^26 voxels");
+  if (c->q == 0) return fail(c, NEB_ESTATE, "neb_voxelize_space_charge: no point charges (neb_add_space_charge first)");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  return voxelize_charges(c, origin, voxel, dims, n_lines_out);
+}
+
+neb_status neb_get_line_charges(neb_ctx* c, double* lines) {
+  if (!c || !lines) return NEB_EINVAL;
+  if (c->n_lines == 0) return NEB_OK;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  cudaMemcpyKind kind = is_device_ptr(lines) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  for (int f = 0; f < 5; ++f)
+    NEB_CUDA(c, cudaMemcpyAsync(lines + f * c->n_lines, c->d_lines + f * c->line_cap, sizeof(double) * c->n_lines, kind, c->stream));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
   return NEB_OK;
 }
 

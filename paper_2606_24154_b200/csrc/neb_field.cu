@@ -402,6 +402,7 @@ static GeoTables tables(const neb_ctx* c) {
 neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_elements, bool use_charges,
                            double* d_phi, double* d_E) {
   if (m <= 0) return NEB_OK;
+  const bool use_lines = use_charges && c->n_lines > 0;
   use_charges = use_charges && c->q > 0;
   int64_t pt_blocks = (m + kThreads - 1) / kThreads;
   int se = use_elements ? pick_splits(pt_blocks, c->n, kTile, c->num_sms) : 0;
@@ -417,7 +418,14 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
     per_q = (per_q + kChargeTile - 1) / kChargeTile * kChargeTile;
     sq = (int)((c->q + per_q - 1) / per_q);
   }
-  size_t need = (size_t)(se + sq) * 4 * (size_t)m * sizeof(double);
+  int sl = use_lines ? pick_splits(pt_blocks, c->n_lines, 256, c->num_sms) : 0;
+  int64_t per_l = 0;
+  if (sl) {
+    per_l = (c->n_lines + sl - 1) / sl;
+    per_l = (per_l + 255) / 256 * 256;
+    sl = (int)((c->n_lines + per_l - 1) / per_l);
+  }
+  size_t need = (size_t)(se + sq + sl) * 4 * (size_t)m * sizeof(double);
   NEB_TRY(ensure_scratch(c, need));
   double* partial = c->d_scratch;
   if (se) {
@@ -438,9 +446,15 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }
+  if (sl) {
+    // line charges of the voxelised cloud (Alg. 3): their partials follow the point charges' (same Coulomb factor)
+    StageTimer t(c, NEB_STAGE_CHARGES);
+    launch_line_kernel(c, m, d_pts, sl, per_l, partial + (size_t)(se + sq) * 4 * m);
+    NEB_CUDA(c, cudaGetLastError());
+  }
   {
     StageTimer t(c, NEB_STAGE_REDUCE);
-    reduce_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(partial, se, sq, m, d_phi, d_E);
+    reduce_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(partial, se, sq + sl, m, d_phi, d_E);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }
@@ -493,7 +507,7 @@ neb_status scale_matrix_rows(neb_ctx* c) {
 neb_status form_rhs(neb_ctx* c) {
   int64_t n = c->n;
   double *phi = nullptr, *E = nullptr;
-  if (c->q > 0) {
+  if (c->q > 0 || c->n_lines > 0) {
     // Phi_sc, E_sc at the collocation points: reuse d_x (npad >= n) for phi and a scratch tail for E.
     // field_at_points uses d_scratch for its partials, so E lives in a dedicated allocation.
     phi = c->d_x;

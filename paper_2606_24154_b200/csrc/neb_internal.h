@@ -81,6 +81,9 @@ struct neb_ctx {
   // space charges: SoA x,y,z,q (4 * q_cap)
   double* d_charges = nullptr;
   int64_t q = 0, q_cap = 0;
+  // line charges from the voxelisation (Alg. 3): SoA x, y, z_start, z_stop, lambda (5 * line_cap)
+  double* d_lines = nullptr;
+  int64_t n_lines = 0, line_cap = 0;
 
   neb::FastVol fastvol[NEB_FASTVOL_SLOTS];
 
@@ -143,6 +146,10 @@ neb_status fastvol_build(neb_ctx* c, int slot, int nx, int ny, int nz, const dou
 neb_status fastvol_eval(neb_ctx* c, int slot, int64_t m, const double* d_pts, double* d_phi, double* d_E);
 neb_status fastvol_get(neb_ctx* c, int slot, double* d_values);
 neb_status solve_weighting(neb_ctx* c, const double* d_w_caller, double* d_sigma_out);
+
+// neb_voxel.cu -----------------------------------------------------------------------------------
+neb_status voxelize_charges(neb_ctx* c, const double* origin, const double* voxel, const int32_t* dims, int64_t* n_lines_out);
+void launch_line_kernel(neb_ctx* c, int64_t m, const double* d_pts, int splits, int64_t per_split, double* partial);
 
 // neb_peaks.cu ------------------------------------------------------------------------------------
 neb_status fp64_peak(neb_ctx* c, int kind, double* tflops);

@@ -559,6 +559,60 @@ def test_weighting_solve_and_map(nb, orc):
 
 
 # ---------------------------------------------------------------------------------------------
+# Alg. 3, voxelisation of the point charges into line charges
+# ---------------------------------------------------------------------------------------------
+def test_voxelize_space_charge(nb, orc, P):
+    """Line list (voxel order, positions exact, lambda to rounding) against the oracle's Alg. 3; field of the lines
+    (+ elements, + point charges added afterwards) and the right-hand side against the oracle; points on a
+    line's axis; the reduction N_voxels << N_points."""
+    pr = W.thgem(d=10, n_plane=8, n_grid=4)
+    g = orc.Geometry(pr)
+    rs = np.random.RandomState(12)
+    q = 20011                                                 # ragged
+    pos = rs.normal(size=(3, q)) * 1e-4 + np.array([[0.0], [0.0], [1e-3]])
+    ch = np.full(q, W.Q_E * 1e3)
+    ch[::7] *= -0.5                                           # unequal charges: voxel totals to rounding only
+    o, d, dims = np.array([-2.5e-4, -2.5e-4, 0.75e-3]), np.array([0.5e-4, 0.5e-4, 0.25e-4]), np.array([10, 10, 20])
+    nb.assemble_problem(pr)
+    nb.add_space_charge(pos, ch)
+    nl = nb.voxelize_space_charge(o, d, dims)
+    lines_o = orc.voxelize(pos, ch, o, d, dims)
+    assert nl == lines_o.shape[1] and nl < q // 10
+    lines = nb.get_line_charges()
+    assert np.array_equal(lines[:4], lines_o[:4])
+    assert np.max(np.abs(lines[4] - lines_o[4])) <= 1e-12 * np.max(np.abs(lines_o[4]))
+    s = nb.solve()                                            # right-hand side from the lines
+    b = nb.get_rhs()
+    pc, _ = orc.line_charges(g.colloc, lines_o)
+    _, Ec = orc.line_charges(g.colloc, lines_o)
+    nrm = np.cross(pr.e2.T, pr.e1.T).T
+    nrm = nrm / np.linalg.norm(nrm, axis=0)
+    bo = np.where(pr.bc_kind == W.DIRICHLET, pr.bc_value - pc, -np.sum(nrm * Ec, axis=0))
+    assert np.max(np.abs(b - bo) / np.maximum(np.abs(bo), 1e-6 * np.abs(bo).max())) <= TOL_FAR
+    pts = rs.normal(size=(3, 700)) * 4e-4 + np.array([[0.0], [0.0], [1e-3]])
+    pts[:2, :5] = lines_o[:2, :5]                             # exactly on the axis of a line: that line is skipped
+    phi, E = nb.eval(pts)
+    phi_e, E_e = orc.evaluate(g, s, pts)
+    phi_l, E_l = orc.line_charges(pts, lines_o)
+    check_field(phi, E, phi_e + phi_l, E_e + E_l, TOL_FAR, "elements + lines")
+    extra_pos, extra_q = rs.normal(size=(3, 50)) * 1e-4 + np.array([[0.0], [0.0], [1.5e-3]]), np.full(50, W.Q_E * 1e4)
+    nb.add_space_charge(extra_pos, extra_q, replace=False)    # points added after the voxelisation stay points
+    phi2, E2 = nb.eval(pts)
+    phi_p, E_p = orc.point_charges(pts, extra_pos, extra_q)
+    check_field(phi2, E2, phi_e + phi_l + phi_p, E_e + E_l + E_p, TOL_FAR, "elements + lines + points")
+    nb.add_space_charge(None, None, replace=True)             # clears lines and points
+    phi3, E3 = nb.eval(pts)
+    check_field(phi3, E3, phi_e, E_e, TOL_FAR, "elements only")
+    with pytest.raises(P.NebError) as e:
+        nb.voxelize_space_charge(o, d, dims)                  # nothing to voxelise
+    assert e.value.status == 3
+    nb.add_space_charge(pos, ch)
+    with pytest.raises(P.NebError) as e:
+        nb.voxelize_space_charge(o, np.array([1e-4, 0.0, 1e-4]), dims)
+    assert e.value.status == 1
+
+
+# ---------------------------------------------------------------------------------------------
 # edge cases and error behaviour of the ABI
 # ---------------------------------------------------------------------------------------------
 def test_edge_cases_and_errors(nb, P, orc):
