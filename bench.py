@@ -376,7 +376,9 @@ def main():
                                 "bytes_per_point": 24 + 32 + 8 * 32, "peak_source": src,
                                 "hbm_only_gbs": ml * (24 + 32) / (look_ms * 1e-3) * 1e-9,
                                 "note": "algorithmic bytes incl. the 8 node records per point; the 32 MB map is served by "
-                                        "L2, so only the 56 B/point of coordinates and results (hbm_only_gbs) cross HBM"}}
+                                        "L2, so only the 56 B/point of coordinates and results (hbm_only_gbs) cross HBM; "
+                                        "ncu: the gather runs the L1/TEX pipe at 95 % of its peak "
+                                        "(profiles/r1_ncu_full_lu_kernels.md)"}}
         del lp, l_phi, l_E
 
     if rank == 0:
