@@ -225,3 +225,15 @@ def line_charges(pts, lines, mode="ld"):
     phi, E = np.zeros(m), np.zeros((3, m))
     _lib(mode).orc_line_charges(C.c_int64(m), _p(pts), C.c_int64(nl), C.c_int64(nl), _p(lines), _p(phi), _p(E))
     return phi, E
+
+
+def evaluate_adaptive(g: Geometry, sigma, pts, far_distance, charge_pos=None, charge_q=None, mode="ld"):
+    """evaluate() with Adaptive Modelling (reading S28): image copies whose shift is at least far_distance
+    long are replaced by the element's total charge at the copy's centroid."""
+    sigma, pts, pos, ch = _d(sigma), _d(pts), _d(charge_pos), _d(charge_q)
+    m = pts.shape[1]
+    q = 0 if ch is None else int(ch.shape[0])
+    phi, E = np.zeros(m), np.zeros((3, m))
+    _lib(mode).orc_eval_adaptive(*g._geo(), _p(sigma), C.c_int32(g.n_img), _p(g.img), C.c_double(float(far_distance)),
+                                 C.c_int64(q), _p(pos), _p(ch), C.c_int64(m), _p(pts), _p(phi), _p(E))
+    return phi, E

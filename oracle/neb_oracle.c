@@ -613,3 +613,69 @@ void orc_line_charges(int64_t m, const double* pts, int64_t nl, int64_t cap, con
     if (E) { E[p] = (double)(acc[1] * K_COULOMB); E[m + p] = (double)(acc[2] * K_COULOMB); E[2 * m + p] = (double)(acc[3] * K_COULOMB); }
   }
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Adaptive Modelling (Table 2): "the solver is permitted to use a simplified
+ * representation ... for parts of the geometry that are far away from the point of evaluation".
+ * Reading (S28): the inputs here are elements, not Garfield++ primitives, so the simplified
+ * representation of a FAR periodic copy of element j is its total charge sigma_j A_j as a point charge
+ * at the copy's centroid (rectangle: A = |e1 x e2|, v0 + (e1+e2)/2; right triangle: A = |e1 x e2|/2,
+ * v0 + (e1+e2)/3; wire: A = 2 pi r_w |e1|, v0 + e1/2); a copy is far when the length of its shift vector
+ * is >= far_distance (so the unshifted element is never simplified; far_distance <= 0 means no
+ * simplification).  Everything else is orc_eval.  An approximation: the error of a far copy's
+ * contribution is O((element size / distance)^2) — its quadrupole term.
+ * ------------------------------------------------------------------------------------------------ */
+void orc_eval_adaptive(int64_t n, const int32_t* kind, const double* v0, const double* e1, const double* e2,
+                       const double* radius, const double* sigma, int32_t n_img, const double* img, double far_distance,
+                       int64_t q, const double* pos, const double* charge, int64_t m, const double* pts, double* phi,
+                       double* E) {
+  elems_t g = {n, kind, v0, e1, e2, radius};
+  const int32_t copies = (n_img <= 0 || !img) ? 1 : n_img;
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t p = 0; p < m; ++p) {
+    real P[3] = {pts[p], pts[m + p], pts[2 * m + p]};
+    long double tot[4] = {0, 0, 0, 0};
+    for (int64_t j = 0; j < n; ++j) {
+      real a1[3] = {e1[j], e1[n + j], e1[2 * n + j]}, a2[3] = {e2[j], e2[n + j], e2[2 * n + j]};
+      real cr[3] = {a1[1] * a2[2] - a1[2] * a2[1], a1[2] * a2[0] - a1[0] * a2[2], a1[0] * a2[1] - a1[1] * a2[0]};
+      real area, cen[3];
+      if (kind[j] == ORC_WIRE) {
+        area = 2 * PI_L * (real)radius[j] * R_SQRT(a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2]);
+        for (int k = 0; k < 3; ++k) cen[k] = (real)v0[k * n + j] + a1[k] / 2;
+      } else {
+        real w = (kind[j] == ORC_RECT) ? (real)0.5 : (real)1 / 3;
+        area = R_SQRT(cr[0] * cr[0] + cr[1] * cr[1] + cr[2] * cr[2]) * ((kind[j] == ORC_RECT) ? 1 : (real)0.5);
+        for (int k = 0; k < 3; ++k) cen[k] = (real)v0[k * n + j] + w * (a1[k] + a2[k]);
+      }
+      long double acc[4] = {0, 0, 0, 0};
+      for (int32_t s = 0; s < copies; ++s) {
+        real sh[3] = {0, 0, 0};
+        if (n_img > 0 && img) { sh[0] = (real)img[s]; sh[1] = (real)img[n_img + s]; sh[2] = (real)img[2 * n_img + s]; }
+        real len = R_SQRT(sh[0] * sh[0] + sh[1] * sh[1] + sh[2] * sh[2]);
+        if (far_distance > 0 && len >= (real)far_distance) {
+          real d[3] = {P[0] - sh[0] - cen[0], P[1] - sh[1] - cen[1], P[2] - sh[2] - cen[2]};
+          real r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+          if (r2 > 0) {
+            real r = R_SQRT(r2);
+            acc[0] += area / r;
+            for (int k = 0; k < 3; ++k) acc[k + 1] += area * d[k] / (r2 * r);
+          }
+        } else {
+          real Ps[3] = {P[0] - sh[0], P[1] - sh[1], P[2] - sh[2]};
+          real o[4];
+          elem_influence(&g, j, Ps, o);
+          for (int k = 0; k < 4; ++k) acc[k] += o[k];
+        }
+      }
+      for (int k = 0; k < 4; ++k) tot[k] += (long double)sigma[j] * acc[k];
+    }
+    for (int k = 0; k < 4; ++k) tot[k] *= K_COULOMB;
+    if (q > 0) {
+      long double sc[4];
+      point_charge_sum(q, pos, charge, P, sc);
+      for (int k = 0; k < 4; ++k) tot[k] += sc[k];
+    }
+    if (phi) phi[p] = (double)tot[0];
+    if (E) { E[p] = (double)tot[1]; E[m + p] = (double)tot[2]; E[2 * m + p] = (double)tot[3]; }
+  }
+}

@@ -618,3 +618,40 @@ def test_voxelize_against_brute_force_histogram(orc):
     p_ln, _ = orc.line_charges(pts, l2)
     err = np.abs(p_ln - p_pt) / np.abs(p_pt)
     assert np.all(err < 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------
+# Adaptive Modelling (Table 2): far image copies as point charges
+# ---------------------------------------------------------------------------------------------
+def test_adaptive_modelling_limits_and_error_order(orc):
+    """far_distance <= 0 or beyond every shift = the exact sum; with every shifted copy simplified the result equals
+    the exact unshifted elements plus explicit point charges sigma A at the shifted centroids (written out here with
+    numpy); the error against the exact sum falls as (element size / pitch)^2."""
+    pr = W.random_elements(9, seed=4, kinds=(RECT, TRI, W.WIRE), size_mm=(0.02, 0.05), box_mm=0.2, m_points=40)
+    sig = np.linspace(0.5, 1.5, pr.n) * 1e-6
+    errs = []
+    for pitch in (1.0, 2.0):
+        pr.img_shift = W.image_shifts(1, pitch_mm=pitch)
+        g = orc.Geometry(pr)
+        phi_x, E_x = orc.evaluate(g, sig, pr.points)
+        for fd in (0.0, -1.0, 10.0):
+            phi0, E0 = orc.evaluate_adaptive(g, sig, pr.points, fd)
+            assert np.array_equal(phi0, phi_x) and np.array_equal(E0, E_x)
+        phi_a, E_a = orc.evaluate_adaptive(g, sig, pr.points, 0.5 * pitch * 1e-3)
+        # by hand: unshifted elements exactly + monopoles of the 8 shifted copies
+        g0 = orc.Geometry(pr); g0.img, g0.n_img = None, 0
+        phi_h, E_h = orc.evaluate(g0, sig, pr.points)
+        area = np.where(pr.kind == W.WIRE, 2 * np.pi * pr.radius * np.linalg.norm(pr.e1, axis=0),
+                        np.linalg.norm(np.cross(pr.e1.T, pr.e2.T), axis=1) * np.where(pr.kind == RECT, 1.0, 0.5))
+        cen = np.where(pr.kind == W.WIRE, pr.v0 + pr.e1 / 2, pr.v0 + (pr.e1 + pr.e2) * np.where(pr.kind == RECT, 0.5, 1 / 3))
+        for s in range(pr.img_shift.shape[1]):
+            sh = pr.img_shift[:, s]
+            if np.linalg.norm(sh) == 0:
+                continue
+            d = pr.points[:, None, :] - (cen + sh[:, None])[:, :, None]            # (3, n, m)
+            r = np.linalg.norm(d, axis=0)
+            phi_h = phi_h + orc.K_COULOMB * np.sum((sig * area)[:, None] / r, axis=0)
+            E_h = E_h + orc.K_COULOMB * np.sum((sig * area)[None, :, None] * d / r ** 3, axis=1)
+        assert np.max(np.abs(phi_a - phi_h)) < 1e-12 * np.max(np.abs(phi_h)) and np.max(np.abs(E_a - E_h)) < 1e-12 * np.max(np.abs(E_h))
+        errs.append(np.max(np.abs(phi_a - phi_x)) / np.max(np.abs(phi_x)))
+    assert 0 < errs[1] < 0.35 * errs[0] and errs[0] < 1e-3        # (L / pitch)^2: a factor 4 per doubling (with the 1/r of the copy, 8)
