@@ -381,6 +381,30 @@ def main():
                                         "(profiles/r1_ncu_full_lu_kernels.md)"}}
         del lp, l_phi, l_E
 
+    adaptive = None
+    if name == "C3" and rank == 0:
+        # SURVEY 8(f).3, Adaptive Modelling (Table 2): the same field map with the periodic copies beyond
+        # far_distance as point charges; time of the element kernel and the largest deviation from the exact map
+        ex_phi, ex_E = d_phi.clone(), d_E.clone()
+        adaptive = []
+        for far_mm in (1.5, 0.9):
+            nb.set_adaptive(far_mm * 1e-3)
+            nb.set_option(P.binding.NEB_OPT_PROFILE, 1)
+            nb.reset_stats()
+            flush.fill_(1)
+            nb.eval(d_pts, phi=d_phi, E=d_E)
+            am_ms = nb.stage_ms()["eval"][0]
+            nb.set_option(P.binding.NEB_OPT_PROFILE, 0)
+            en = torch.linalg.vector_norm(ex_E, dim=0)
+            adaptive.append({"far_distance_mm": far_mm,
+                             "copies_simplified": int(np.sum(np.linalg.norm(pr.img_shift, axis=0) >= far_mm * 1e-3)),
+                             "eval_kernel_ms": am_ms, "speedup_vs_exact": eval_ms / am_ms,
+                             "max_err_phi_rel_to_max": float((d_phi - ex_phi).abs().max() / ex_phi.abs().max()),
+                             "max_err_E_rel_to_max": float(torch.linalg.vector_norm(d_E - ex_E, dim=0).max() / en.max()),
+                             "median_err_E_pointwise": float((torch.linalg.vector_norm(d_E - ex_E, dim=0) / en).median())})
+        nb.set_adaptive(0.0)
+        del ex_phi, ex_E
+
     if rank == 0:
         value = pairs_step * args.steps * world / (ms * 1e-3)
         line = {
@@ -407,6 +431,8 @@ def main():
         }
         if fastvol:
             line["fastvol"] = fastvol
+        if adaptive:
+            line["adaptive_modelling"] = adaptive
         if not args.no_cpu_baseline and world == 1:
             if name == "C1":
                 line["cpu_baseline"] = cpu_baseline_run(pr, with_lu=True)      # the whole C1 step, LU included

@@ -124,6 +124,13 @@ neb_status neb_solve(neb_ctx* ctx, double* sigma_out);
  * order): a test hook, and the way to evaluate a weighting field (sigma from neb_solve_weighting). */
 neb_status neb_set_sigma(neb_ctx* ctx, const double* sigma);
 
+/* Adaptive Modelling (Table 2; reading S28): in neb_eval and neb_fastvol_build, a periodic copy of
+ * an element whose shift vector is at least far_distance (m) long is represented by the element's total charge
+ * sigma_j A_j at the copy's centroid instead of its exact closed form; nearer copies and the element itself stay
+ * exact.  An approximation (error of a far copy's contribution ~ (element size / distance)^2), off by default
+ * (far_distance = 0); the matrix assembly is never simplified.  Takes effect from the next neb_eval. */
+neb_status neb_set_adaptive(neb_ctx* ctx, double far_distance);
+
 /* Weighting field (P:222 CreateWtFldFastVolPF; reading S26): solves K sigma_w = b_w on the RESIDENT LU
  * factors, b_w = bc_value_w on Dirichlet rows (1 on the read-out electrode's panels, 0 on every other
  * conductor), 0 on dielectric rows, no space charge.  bc_value_w and sigma_w_out hold n values in the

@@ -54,6 +54,7 @@ def lib():
         L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
         L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
         L.neb_solve_weighting.argtypes = [vp, vp, vp]
+        L.neb_set_adaptive.argtypes = [vp, dbl]
         L.neb_voxelize_space_charge.argtypes = [vp, vp, vp, vp, C.POINTER(i64)]
         L.neb_get_line_charges.argtypes = [vp, vp]
         L.neb_fastvol_build.argtypes = [vp, i32, i32, i32, i32, vp, vp, i32]
@@ -195,6 +196,10 @@ class Neb:
         pos = _check_arr(pos, np.float64, "float64", 3 * q, "pos")
         charge = _check_arr(charge, np.float64, "float64", q, "charge")
         self._ck(self._L.neb_add_space_charge(self._h, q, _ptr(pos), _ptr(charge), 1 if replace else 0))
+
+    def set_adaptive(self, far_distance: float):
+        """neb_set_adaptive: image copies at least far_distance (m) away become point charges in eval (0 = off)."""
+        self._ck(self._L.neb_set_adaptive(self._h, float(far_distance)))
 
     def solve_weighting(self, bc_value_w, out=None):
         """neb_solve_weighting: sigma_w (n) for the weighting potentials bc_value_w (n), on the resident factors."""

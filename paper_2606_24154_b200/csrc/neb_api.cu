@@ -381,8 +381,10 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
                         const double* radius, const double* colloc, const int32_t* bc_kind, const double* bc_value,
                         const double* eps_plus, const double* eps_minus, int32_t n_img, const double* img_shift) {
   if (!c) return NEB_EINVAL;
-  if (n <= 0 || n > 65000 || !kind || !v0 || !e1 || !e2 || !bc_kind)
-    return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1..65000 and kind, v0, e1, e2, bc_kind non-NULL");
+  // the grid-wide LU panel keeps a slab of at most 384 rows per SM in shared memory: 148 x 384 = 56832 rows on a B200
+  const int64_t n_max = (int64_t)c->num_sms * 384 - kPad;
+  if (n <= 0 || n > n_max || !kind || !v0 || !e1 || !e2 || !bc_kind)
+    return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1.." + std::to_string(n_max) + " and kind, v0, e1, e2, bc_kind non-NULL");
   if (n_img < 0 || n_img > 32 || (n_img > 0 && !img_shift)) return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= 32");
   NEB_CUDA(c, cudaSetDevice(c->device));
   const bool reuse = (c->n == n && c->d_K != nullptr);   // same size as the last problem: keep the buffers
@@ -415,6 +417,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * 32));
   }
   c->n_img = n_img > 0 ? n_img : 1;
+  c->h_img_len[0] = 0.0;
   NEB_CUDA(c, cudaMemsetAsync(c->d_img, 0, sizeof(double) * 3 * c->n_img, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_rec, 0, sizeof(double) * kRec * st, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int32_t), c->stream));
@@ -439,7 +442,22 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     for (int s = 0; s < n_img && zero < 0; ++s)
       if (h_img[s] == 0.0 && h_img[n_img + s] == 0.0 && h_img[2 * n_img + s] == 0.0) zero = s;
     if (zero < 0) { free_problem(c); return fail(c, NEB_EINVAL, "neb_assemble: img_shift must include (0,0,0)"); }
-    for (int k = 0; k < 3; ++k) { double t = h_img[k * n_img]; h_img[k * n_img] = h_img[k * n_img + zero]; h_img[k * n_img + zero] = t; }
+    // copies sorted by the length of their shift (stable insertion sort): the zero shift lands in slot 0, and the
+    // far copies of Adaptive Modelling (neb_set_adaptive) form the tail
+    double len[32];
+    int order[32];
+    for (int s = 0; s < n_img; ++s) {
+      len[s] = sqrt(h_img[s] * h_img[s] + h_img[n_img + s] * h_img[n_img + s] + h_img[2 * n_img + s] * h_img[2 * n_img + s]);
+      order[s] = s;
+    }
+    for (int s = 1; s < n_img; ++s)
+      for (int t = s; t > 0 && len[order[t]] < len[order[t - 1]]; --t) { int tmp = order[t]; order[t] = order[t - 1]; order[t - 1] = tmp; }
+    double sorted[3 * 32];
+    for (int s = 0; s < n_img; ++s) {
+      for (int k = 0; k < 3; ++k) sorted[k * n_img + s] = h_img[k * n_img + order[s]];
+      c->h_img_len[s] = len[order[s]];
+    }
+    for (int k = 0; k < 3 * n_img; ++k) h_img[k] = sorted[k];
     NEB_CUDA(c, cudaMemcpyAsync(c->d_img, h_img, sizeof(double) * 3 * n_img, cudaMemcpyHostToDevice, c->stream));
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_img is a stack buffer
   }
@@ -542,6 +560,12 @@ neb_status neb_eval(neb_ctx* c, int64_t m, const double* pts, double* phi, doubl
   NEB_TRY(sg.out(E, sizeof(double) * 3 * m, &dE));
   NEB_TRY(field_at_points(c, m, (const double*)dp, true, true, (double*)dphi, (double*)dE));
   return sg.finish();
+}
+
+neb_status neb_set_adaptive(neb_ctx* c, double far_distance) {
+  if (!c || !(far_distance >= 0.0)) return NEB_EINVAL;
+  c->adaptive_far = far_distance;
+  return NEB_OK;
 }
 
 neb_status neb_solve_weighting(neb_ctx* c, const double* bc_value_w, double* sigma_w_out) {

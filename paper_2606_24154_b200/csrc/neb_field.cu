@@ -82,10 +82,25 @@ __device__ __forceinline__ Frame frame_of(const TileSmem& sm, unsigned buf, int 
   return f;
 }
 
+// Adaptive Modelling (reading S28): a FAR periodic copy of an element is represented by its total charge at
+// the copy's centroid.  d = (point - shift - centroid) in any orthonormal frame; adds area/r and area d/r^3.
+__device__ __forceinline__ void far_copy(double area, double dx, double dy, double dz, double& phi, double& fx, double& fy,
+                                         double& fz) {
+  const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+  double y = mufu_rsqrt(clamp_tiny(r2));            // 1/r: seed + two Newton steps, as in the point-charge kernel
+  const double h = 0.5 * r2;
+  y = fma(y, fma(-h * y, y, 0.5), y);
+  y = fma(y, fma(-h * y, y, 0.5), y);
+  y = (r2 > 0.0) ? y : 0.0;
+  const double ar = area * y, ar3 = ar * y * y;
+  phi += ar;
+  fx = fma(ar3, dx, fx); fy = fma(ar3, dy, fy); fz = fma(ar3, dz, fz);
+}
+
 // All elements of one kind in [lo, hi): tile loop, image loop, sink(j, weight_j, sum over copies).
 // seq = number of tiles this CTA has consumed so far (buffer = seq & 1, mbarrier parity = (seq >> 1) & 1).
 template <class M, int KIND, class Sink>
-__device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img,
+__device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img, int n_near,
                                              double px, double py, double pz, Sink& sink, unsigned& seq) {
   const int64_t tb0 = lo & ~(int64_t)(kTile - 1);
   if (threadIdx.x == 0) tile_issue(sm, g, tb0, seq);
@@ -123,10 +138,17 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
         local_pair<M, KIND>(a, b, aux, far2, X0, Y0, Z0, phi, lx, ly, lz);
         if (sink.self_pv(tb + e)) { lx = 0.0; ly = 0.0; lz = 0.0; }   // principal value (S5, S8)
 #pragma unroll 1
-        for (int s = 1; s < n_img; ++s) {
+        for (int s = 1; s < n_near; ++s) {
           double p1, x1, y1, z1;
           local_pair<M, KIND>(a, b, aux, far2, X0 - sm.limg[0][s], Y0 - sm.limg[1][s], Z0 - sm.limg[2][s], p1, x1, y1, z1);
           phi += p1; lx += x1; ly += y1; lz += z1;
+        }
+        if (n_near < n_img) {
+          // far copies (Adaptive Modelling): total charge at the copy's centroid, in the window's axes
+          const double area = (KIND == 0) ? aux : 0.5 * a * b;
+          const double cxl = X0 - ((KIND == 0) ? 0.5 : (1.0 / 3.0)) * a, czl = Z0 - ((KIND == 0) ? 0.5 : (1.0 / 3.0)) * b;
+#pragma unroll 1
+          for (int s = n_near; s < n_img; ++s) far_copy(area, cxl - sm.limg[0][s], Y0 - sm.limg[1][s], czl - sm.limg[2][s], phi, lx, ly, lz);
         }
         sink.local(tb + e, sm.rec[buf][15][e], phi, lx, ly, lz);
       }
@@ -140,9 +162,19 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
         Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
         if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
 #pragma unroll 1
-        for (int s = 1; s < n_img; ++s) {
+        for (int s = 1; s < n_near; ++s) {
           Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
           acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
+        }
+        if (n_near < n_img) {
+          // far copies (Adaptive Modelling): total charge at the copy's centroid, in global coordinates
+          const double wc = (KIND == 0) ? 0.5 : ((KIND == 1) ? (1.0 / 3.0) : 0.5), wz = (KIND == 2) ? 0.0 : wc;
+          const double area = (KIND == 0) ? fr.aux : ((KIND == 1) ? 0.5 * fr.a * fr.b : fr.aux * fr.a);
+          const double gx = px - fma(wc * fr.a, fr.exx, fma(wz * fr.b, fr.ezx, fr.v0x));
+          const double gy = py - fma(wc * fr.a, fr.exy, fma(wz * fr.b, fr.ezy, fr.v0y));
+          const double gz = pz - fma(wc * fr.a, fr.exz, fma(wz * fr.b, fr.ezz, fr.v0z));
+#pragma unroll 1
+          for (int s = n_near; s < n_img; ++s) far_copy(area, gx - sm.img[0][s], gy - sm.img[1][s], gz - sm.img[2][s], acc.phi, acc.ex, acc.ey, acc.ez);
         }
         sink(tb + e, sm.rec[buf][15][e], acc);
       }
@@ -153,17 +185,17 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
 }
 
 template <class M, class Sink>
-__device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, int64_t j1, TileSmem& sm, int n_img,
+__device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, int64_t j1, TileSmem& sm, int n_img, int n_near,
                                               double px, double py, double pz, Sink& sink) {
   int64_t r1 = g.n_rect, t1 = r1 + g.n_tri, w1 = t1 + g.n_wire;
   int64_t lo, hi;
   unsigned seq = 0;
   lo = max(j0, (int64_t)0); hi = min(j1, r1);
-  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, r1); hi = min(j1, t1);
-  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, t1); hi = min(j1, w1);
-  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
 }
 
 __device__ __forceinline__ void load_images(TileSmem& sm, const double* img, int n_img) {
@@ -196,7 +228,7 @@ struct EvalSink {
 #define NEB_EVAL_MINB 4
 #endif
 template <class M>
-__global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img,
+__global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img, int n_near,
                                                         const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                         double* __restrict__ partial) {
   __shared__ TileSmem sm;
@@ -209,7 +241,7 @@ __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables
   int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
   int64_t j0 = (int64_t)blockIdx.y * per_split, j1 = min(n, j0 + per_split);
   EvalSink sink;
-  process_range<M>(g, j0, j1, sm, n_img, px, py, pz, sink);
+  process_range<M>(g, j0, j1, sm, n_img, n_near, px, py, pz, sink);
   if (p < m) {
     double* o = partial + (int64_t)blockIdx.y * 4 * m;
     o[p] = sink.phi; o[m + p] = sink.ex; o[2 * m + p] = sink.ey; o[3 * m + p] = sink.ez;
@@ -330,7 +362,7 @@ __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const d
   sink.diag = diag[ic];
   double px = colloc[ic], py = colloc[stride + ic], pz = colloc[2 * stride + ic];
   int64_t j0 = (int64_t)blockIdx.y * kTile, j1 = min(n, j0 + kTile);
-  process_range<M>(g, j0, j1, sm, n_img, px, py, pz, sink);
+  process_range<M>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
   if (i < n) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
 }
 
@@ -428,13 +460,19 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
   size_t need = (size_t)(se + sq + sl) * 4 * (size_t)m * sizeof(double);
   NEB_TRY(ensure_scratch(c, need));
   double* partial = c->d_scratch;
+  // Adaptive Modelling: the copies are sorted by shift length (neb_assemble), the first n_near are evaluated exactly
+  int n_near = c->n_img;
+  if (c->adaptive_far > 0.0) {
+    n_near = 1;
+    while (n_near < c->n_img && c->h_img_len[n_near] < c->adaptive_far) ++n_near;
+  }
   if (se) {
     StageTimer t(c, NEB_STAGE_EVAL);
     dim3 grid((unsigned)pt_blocks, (unsigned)se);
     if (c->math_fast)
-      eval_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, d_pts, m, per_e, partial);
+      eval_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, n_near, d_pts, m, per_e, partial);
     else
-      eval_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, d_pts, m, per_e, partial);
+      eval_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, n_near, d_pts, m, per_e, partial);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }

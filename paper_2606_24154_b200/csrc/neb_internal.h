@@ -63,7 +63,9 @@ struct neb_ctx {
   int32_t* d_bc_kind = nullptr;   // sorted
   double* d_bc_value = nullptr;   // sorted
   double* d_diag = nullptr;       // sorted: 1/(2 eps0 lambda) on dielectric rows, else 0
-  double* d_img = nullptr;        // 3 * n_img
+  double* d_img = nullptr;        // 3 * n_img, sorted by length (slot 0 = the zero shift)
+  double h_img_len[32] = {0};     // their lengths (host)
+  double adaptive_far = 0.0;      // Adaptive Modelling: copies at least this far are simplified in neb_eval (0 = off)
   int32_t* d_flag = nullptr;      // device error flags (validation, singular pivot)
 
   // matrix / factors
