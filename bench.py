@@ -405,6 +405,36 @@ def main():
         nb.set_adaptive(0.0)
         del ex_phi, ex_E
 
+    voxelised = None
+    if is_c4 and rank == 0:
+        # SURVEY 8(f).2, Alg. 3: the same cloud as line charges (10 um voxels): time of the space-charge sums at the
+        # charges' own positions and the deviation of E there from the point-charge sum (the paper leaves the accuracy
+        # of the representation open; a charge sees its own voxel's line, so the near field differs)
+        nb.set_option(P.binding.NEB_OPT_PROFILE, 1)
+        nb.reset_stats()
+        nb.add_space_charge(d_pts, d_ch, replace=True)
+        nb.eval(d_pts, E=d_E, want_phi=False)
+        pt_ms = nb.stage_ms()["charges"][0]
+        E_pt = d_E.clone()
+        # a 2 mm box of 200^3 voxels about the cloud's median (charges that were pushed far away count in border voxels)
+        vox = np.full(3, 1e-5)
+        dims = np.full(3, 200, dtype=np.int32)
+        lo = d_pts.median(dim=1).values.cpu().numpy() - 0.5 * vox * dims
+        nb.reset_stats()
+        n_lines = nb.voxelize_space_charge(lo, vox, dims)
+        vox_ms = nb.stage_ms()["charges"][0]
+        nb.reset_stats()
+        nb.eval(d_pts, E=d_E, want_phi=False)
+        ln_ms = nb.stage_ms()["charges"][0]
+        nb.set_option(P.binding.NEB_OPT_PROFILE, 0)
+        en = torch.linalg.vector_norm(E_pt, dim=0)
+        dev = torch.linalg.vector_norm(d_E - E_pt, dim=0) / en
+        voxelised = {"voxel_um": 10.0, "grid": [int(v) for v in dims], "points": int(m), "lines": int(n_lines),
+                     "voxelise_ms": vox_ms, "point_charge_sum_ms": pt_ms, "line_charge_sum_ms": ln_ms,
+                     "median_dev_E_at_charges": float(dev.median()), "p99_dev_E_at_charges": float(dev.quantile(0.99))}
+        nb.add_space_charge(d_pts, d_ch, replace=True)
+        del E_pt
+
     if rank == 0:
         value = pairs_step * args.steps * world / (ms * 1e-3)
         line = {
@@ -433,6 +463,8 @@ def main():
             line["fastvol"] = fastvol
         if adaptive:
             line["adaptive_modelling"] = adaptive
+        if voxelised:
+            line["voxelised_space_charge"] = voxelised
         if not args.no_cpu_baseline and world == 1:
             if name == "C1":
                 line["cpu_baseline"] = cpu_baseline_run(pr, with_lu=True)      # the whole C1 step, LU included
