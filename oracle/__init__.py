@@ -168,6 +168,28 @@ def evaluate(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="ld")
     return phi, E
 
 
+def evaluate_abs(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="f64"):
+    """S_Phi (m), S_E (m): sums of the magnitudes of the terms evaluate() adds at pts (3, m) — the scale of the
+    rounding error of a cancelled sum; a tolerance scale for the parity tests, not a result."""
+    sigma, pts, pos, ch = _d(sigma), _d(pts), _d(charge_pos), _d(charge_q)
+    m = pts.shape[1]
+    q = 0 if ch is None else int(ch.shape[0])
+    s_phi, s_E = np.zeros(m), np.zeros(m)
+    _lib(mode).orc_eval_abs(*g._geo(), _p(sigma), C.c_int32(g.n_img), _p(g.img), C.c_int64(q), _p(pos), _p(ch),
+                            C.c_int64(m), _p(pts), _p(s_phi), _p(s_E))
+    return s_phi, s_E
+
+
+def solve_library(K: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """The solution of K sigma = b (Eq. 6-7) with a LIBRARY routine as the step: rows equilibrated by
+    1/max_j|K_ij| (reading S15), then numpy.linalg.solve (LAPACK dgesv: LU with partial pivoting, the same
+    algorithm as orc_solve).  For sizes the plain C loop of orc_lu_factor cannot finish in test time (C2: N = 19400);
+    tests/test_oracle_pins.py checks the two against each other on small systems."""
+    K, b = _d(K), _d(b)
+    r = 1.0 / np.abs(K).max(axis=1)
+    return np.linalg.solve(K * r[:, None], b * r)
+
+
 def push(pos, E, mu, dt, mode="ld"):
     pos = np.array(pos, dtype=np.float64, order="C")
     E = _d(E)

@@ -485,6 +485,48 @@ void orc_eval(int64_t n, const int32_t* kind, const double* v0, const double* e1
   }
 }
 
+/* Condition of the sums Eq.(3),(4) at a point: the sum of the MAGNITUDES of the terms orc_eval adds,
+ *   S_Phi(P) = (1/4 pi eps0) [ sum_j |sigma_j| sum_img |Phi'_j(P)| + sum_k |q_k| / r_k ],
+ *   S_E(P)   = (1/4 pi eps0) [ sum_j |sigma_j| sum_img |E'_j(P)|   + sum_k |q_k| / r_k^2 ]   (|.| = vector norm).
+ * Not a result of the method: the parity tests use it as the scale of the rounding error of a cancelled sum
+ * (a sum of n terms of both signs evaluated in precision eps carries an error ~ eps x S wherever it happens to
+ * cancel, whatever the implementation), so that no global floor on |Phi| is needed. */
+void orc_eval_abs(int64_t n, const int32_t* kind, const double* v0, const double* e1, const double* e2,
+                  const double* radius, const double* sigma, int32_t n_img, const double* img, int64_t q,
+                  const double* pos, const double* charge, int64_t m, const double* pts, double* s_phi, double* s_E) {
+  elems_t g = {n, kind, v0, e1, e2, radius};
+  const int32_t copies = (n_img <= 0 || !img) ? 1 : n_img;
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t p = 0; p < m; ++p) {
+    real P[3] = {pts[p], pts[m + p], pts[2 * m + p]};
+    long double tp = 0, te = 0;
+    for (int64_t j = 0; j < n; ++j) {
+      long double ap = 0, ae = 0;
+      for (int32_t s = 0; s < copies; ++s) {
+        real sh[3] = {0, 0, 0};
+        if (n_img > 0 && img) { sh[0] = (real)img[s]; sh[1] = (real)img[n_img + s]; sh[2] = (real)img[2 * n_img + s]; }
+        real Ps[3] = {P[0] - sh[0], P[1] - sh[1], P[2] - sh[2]};
+        real o[4];
+        elem_influence(&g, j, Ps, o);
+        ap += R_FABS(o[0]);
+        ae += R_SQRT(o[1] * o[1] + o[2] * o[2] + o[3] * o[3]);
+      }
+      tp += R_FABS((real)sigma[j]) * ap;
+      te += R_FABS((real)sigma[j]) * ae;
+    }
+    for (int64_t c = 0; c < q; ++c) {
+      real dx = P[0] - (real)pos[c], dy = P[1] - (real)pos[q + c], dz = P[2] - (real)pos[2 * q + c];
+      real r2 = dx * dx + dy * dy + dz * dz;
+      if (r2 > 0) {
+        tp += R_FABS((real)charge[c]) / R_SQRT(r2);
+        te += R_FABS((real)charge[c]) / r2;
+      }
+    }
+    if (s_phi) s_phi[p] = (double)(tp * K_COULOMB);
+    if (s_E) s_E[p] = (double)(te * K_COULOMB);
+  }
+}
+
 /* a9. Charge push of the synthetic C4 loop (reading S23): x += mu * E * dt. */
 void orc_push(int64_t q, double* pos, const double* E, double mu, double dt) {
   for (int64_t k = 0; k < 3 * q; ++k) pos[k] = (double)((real)pos[k] + (real)mu * (real)E[k] * (real)dt);

@@ -32,7 +32,10 @@ CASES = [
     ("tri", 0.5, 2.0, (1.5, 0.0, 0.7)),           # in plane, outside
     ("tri", 1.0, 1.0, (-12.0, 9.0, 20.0)),        # far
     ("tri", 2.0, 0.3, (1.0, 0.04, 0.1)),          # low height above a thin triangle
-    ("wire", 1.0, 0.0, (0.2, 0.0, 0.85)),         # SURVEY pin: h=0.5, rho=0.2, Z(from centre)=0.35; wire on local X axis here
+    ("wire", 1.0, 0.0, (0.2, 0.0, 0.85)),         # beside the first fifth of the wire, rho = 0.85
+    ("wire", 1.0, 0.0, (0.85, 0.0, 0.2)),         # SURVEY 8(c) pin: h=0.5, rho=0.2, 0.35 from the centre ALONG the axis; wire on
+                                                  # the local X axis here: X = 0.5+0.35, rho along Z.  Survey values: Phi' =
+                                                  # 2.84677535102197, E'_rho (here E'z) = 7.86708584166788, E'_axis (E'x) = 2.85480333137226
     ("wire", 1.0, 0.0, (1.6, 0.3, 0.4)),          # beyond the end
     ("wire", 0.3, 0.0, (-4.0, 2.0, 1.0)),         # far
 ]
