@@ -89,7 +89,7 @@ neb_status neb_set_option(neb_ctx* ctx, int32_t option, int64_t value);
  * Elements, in GLOBAL coordinates (length n each; vectors 3*n SoA):
  *   kind      NEB_RECT / NEB_TRI / NEB_WIRE
  *   v0        corner (rect), right-angle vertex (tri), start point (wire)
- *   e1, e2    the two perpendicular edge vectors from v0 (rect: sides; tri: legs, hypotenuse from
+ *   e1, e2    the two PERPENDICULAR edge vectors from v0 (|cos| <= 1e-9, else NEB_EINVAL; rect: sides; tri: legs, hypotenuse from
  *             v0+e1 to v0+e2, P:123-127 with reading S2; wire: e1 = axis vector, e2 ignored).
  *             The unit normal is n = e2 x e1 / |e2 x e1|, so that (e1^, n, e2^) is the paper's
  *             local (X, Y, Z) of P:119.
@@ -170,10 +170,14 @@ neb_status neb_add_space_charge(neb_ctx* ctx, int64_t q, const double* pos, cons
  * in voxel-index order (x fastest).  From then on neb_eval and the right-hand side of neb_solve sum over the lines
  * (closed form of Eq. 2 integrated along the line; a point exactly on a line's axis is skipped) and over any point
  * charges added LATER with replace = 0; neb_add_space_charge with replace != 0 discards lines and points.
- * n_lines_out (host, may be NULL) receives the number of lines.  Voxel totals are accumulated with atomics
- * (order-dependent rounding in the last bit unless all charges are equal).
+ * A second call voxelises the points added since TOGETHER WITH the lines of the earlier call, each old line entering
+ * as its total charge lambda (z_stop - z_start) at its centre, so that the total charge is conserved (the call needs
+ * at least one point or line).  n_lines_out (host, may be NULL) receives the number of lines.  Voxel totals are
+ * accumulated in fixed point with integer atomics: lambda is bit-reproducible from run to run (exact sum of the
+ * charges, each taken with an absolute error below 2^-72 max|q|).  At most 2^26 charges.
  * neb_get_line_charges (test hook): 5*n_lines doubles SoA x, y, z_start, z_stop, lambda.
- * Errors: NEB_EINVAL (non-positive voxel size, dims < 1, more than 2^26 voxels), NEB_ESTATE (no point charges). */
+ * Errors: NEB_EINVAL (non-positive voxel size, dims < 1, more than 2^26 voxels or charges), NEB_ESTATE (no point
+ * charges and no lines). */
 neb_status neb_voxelize_space_charge(neb_ctx* ctx, const double* origin, const double* voxel, const int32_t* dims,
                                      int64_t* n_lines_out);
 neb_status neb_get_line_charges(neb_ctx* ctx, double* lines);
@@ -187,6 +191,11 @@ neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, doubl
  * neb_solve (NEB_ESTATE afterwards: the factors overwrite it).  neb_get_rhs: the RHS the last
  * neb_solve used (unscaled, caller's order). */
 neb_status neb_get_matrix(neb_ctx* ctx, double* K_out);
+/* neb_get_matrix_rows (test hook for sizes whose whole matrix does not fit the host, C3: 20 GB): the UNSCALED rows
+ * rows[0..n_rows) (caller's element indices, int32, host or device), as n_rows*n doubles ROW-major in the caller's
+ * column order: K_out[r*n + j] = K(rows[r], j).  Same state rule as neb_get_matrix.  NEB_EINVAL for an index
+ * outside [0, n). */
+neb_status neb_get_matrix_rows(neb_ctx* ctx, int64_t n_rows, const int32_t* rows, double* K_out);
 neb_status neb_get_rhs(neb_ctx* ctx, double* b_out);
 
 /* Measurement aids: register-only FP64 microbenchmarks on all SMs.

@@ -168,16 +168,18 @@ def evaluate(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="ld")
     return phi, E
 
 
-def evaluate_abs(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="f64"):
+def evaluate_abs(g: Geometry, sigma, pts, charge_pos=None, charge_q=None, mode="f64", with_field=False):
     """S_Phi (m), S_E (m): sums of the magnitudes of the terms evaluate() adds at pts (3, m) — the scale of the
-    rounding error of a cancelled sum; a tolerance scale for the parity tests, not a result."""
+    rounding error of a cancelled sum; a tolerance scale for the parity tests, not a result.
+    with_field=True also returns Phi, E formed in the same pass (bit-identical to evaluate()): (S_Phi, S_E, Phi, E)."""
     sigma, pts, pos, ch = _d(sigma), _d(pts), _d(charge_pos), _d(charge_q)
     m = pts.shape[1]
     q = 0 if ch is None else int(ch.shape[0])
     s_phi, s_E = np.zeros(m), np.zeros(m)
+    phi, E = (np.zeros(m), np.zeros((3, m))) if with_field else (None, None)
     _lib(mode).orc_eval_abs(*g._geo(), _p(sigma), C.c_int32(g.n_img), _p(g.img), C.c_int64(q), _p(pos), _p(ch),
-                            C.c_int64(m), _p(pts), _p(s_phi), _p(s_E))
-    return s_phi, s_E
+                            C.c_int64(m), _p(pts), _p(s_phi), _p(s_E), _p(phi), _p(E))
+    return (s_phi, s_E, phi, E) if with_field else (s_phi, s_E)
 
 
 def solve_library(K: np.ndarray, b: np.ndarray) -> np.ndarray:

@@ -490,18 +490,22 @@ void orc_eval(int64_t n, const int32_t* kind, const double* v0, const double* e1
  *   S_E(P)   = (1/4 pi eps0) [ sum_j |sigma_j| sum_img |E'_j(P)|   + sum_k |q_k| / r_k^2 ]   (|.| = vector norm).
  * Not a result of the method: the parity tests use it as the scale of the rounding error of a cancelled sum
  * (a sum of n terms of both signs evaluated in precision eps carries an error ~ eps x S wherever it happens to
- * cancel, whatever the implementation), so that no global floor on |Phi| is needed. */
+ * cancel, whatever the implementation), so that no global floor on |Phi| is needed.
+ * phi / E (may be NULL): the sums of orc_eval themselves, formed in the same pass from the same terms in the same
+ * order (bit-identical to orc_eval, checked in tests/test_oracle_pins.py), so that a sampled full-size parity check
+ * walks the 1e6 element copies once instead of twice. */
 void orc_eval_abs(int64_t n, const int32_t* kind, const double* v0, const double* e1, const double* e2,
                   const double* radius, const double* sigma, int32_t n_img, const double* img, int64_t q,
-                  const double* pos, const double* charge, int64_t m, const double* pts, double* s_phi, double* s_E) {
+                  const double* pos, const double* charge, int64_t m, const double* pts, double* s_phi, double* s_E,
+                  double* phi, double* E) {
   elems_t g = {n, kind, v0, e1, e2, radius};
   const int32_t copies = (n_img <= 0 || !img) ? 1 : n_img;
 #pragma omp parallel for schedule(dynamic, 4)
   for (int64_t p = 0; p < m; ++p) {
     real P[3] = {pts[p], pts[m + p], pts[2 * m + p]};
-    long double tp = 0, te = 0;
+    long double tp = 0, te = 0, tot[4] = {0, 0, 0, 0};
     for (int64_t j = 0; j < n; ++j) {
-      long double ap = 0, ae = 0;
+      long double ap = 0, ae = 0, acc[4] = {0, 0, 0, 0};
       for (int32_t s = 0; s < copies; ++s) {
         real sh[3] = {0, 0, 0};
         if (n_img > 0 && img) { sh[0] = (real)img[s]; sh[1] = (real)img[n_img + s]; sh[2] = (real)img[2 * n_img + s]; }
@@ -510,20 +514,35 @@ void orc_eval_abs(int64_t n, const int32_t* kind, const double* v0, const double
         elem_influence(&g, j, Ps, o);
         ap += R_FABS(o[0]);
         ae += R_SQRT(o[1] * o[1] + o[2] * o[2] + o[3] * o[3]);
+        for (int k = 0; k < 4; ++k) acc[k] += o[k];
       }
       tp += R_FABS((real)sigma[j]) * ap;
       te += R_FABS((real)sigma[j]) * ae;
+      for (int k = 0; k < 4; ++k) tot[k] += (long double)sigma[j] * acc[k];
     }
-    for (int64_t c = 0; c < q; ++c) {
-      real dx = P[0] - (real)pos[c], dy = P[1] - (real)pos[q + c], dz = P[2] - (real)pos[2 * q + c];
-      real r2 = dx * dx + dy * dy + dz * dz;
-      if (r2 > 0) {
-        tp += R_FABS((real)charge[c]) / R_SQRT(r2);
-        te += R_FABS((real)charge[c]) / r2;
+    for (int k = 0; k < 4; ++k) tot[k] *= K_COULOMB;
+    tp *= K_COULOMB;
+    te *= K_COULOMB;
+    if (q > 0) {
+      long double sc[4];
+      point_charge_sum(q, pos, charge, P, sc);
+      for (int k = 0; k < 4; ++k) tot[k] += sc[k];
+      long double cp = 0, ce = 0;
+      for (int64_t c = 0; c < q; ++c) {
+        real dx = P[0] - (real)pos[c], dy = P[1] - (real)pos[q + c], dz = P[2] - (real)pos[2 * q + c];
+        real r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 > 0) {
+          cp += R_FABS((real)charge[c]) / R_SQRT(r2);
+          ce += R_FABS((real)charge[c]) / r2;
+        }
       }
+      tp += cp * K_COULOMB;
+      te += ce * K_COULOMB;
     }
-    if (s_phi) s_phi[p] = (double)(tp * K_COULOMB);
-    if (s_E) s_E[p] = (double)(te * K_COULOMB);
+    if (s_phi) s_phi[p] = (double)tp;
+    if (s_E) s_E[p] = (double)te;
+    if (phi) phi[p] = (double)tot[0];
+    if (E) { E[p] = (double)tot[1]; E[m + p] = (double)tot[2]; E[2 * m + p] = (double)tot[3]; }
   }
 }
 

@@ -62,6 +62,7 @@ def lib():
         L.neb_fastvol_get.argtypes = [vp, i32, vp]
         L.neb_push.argtypes = [vp, i64, vp, vp, dbl]
         L.neb_get_matrix.argtypes = [vp, vp]
+        L.neb_get_matrix_rows.argtypes = [vp, i64, vp, vp]
         L.neb_get_rhs.argtypes = [vp, vp]
         L.neb_fp64_peak.argtypes = [vp, i32, C.POINTER(dbl)]
         L.neb_stage_ms.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(i64)]
@@ -269,6 +270,13 @@ class Neb:
         K = np.empty((self.n, self.n))
         self._ck(self._L.neb_get_matrix(self._h, _ptr(K)))
         return K.T            # column-major n*n -> K[i, j]
+
+    def get_matrix_rows(self, rows):
+        """K[rows, :] (len(rows), n), unscaled, caller's order (test hook; before the first solve)."""
+        rows = np.ascontiguousarray(rows, dtype=np.int32)
+        out = np.empty((rows.shape[0], self.n))
+        self._ck(self._L.neb_get_matrix_rows(self._h, rows.shape[0], _ptr(rows), _ptr(out)))
+        return out
 
     def get_rhs(self):
         b = np.empty(self.n)

@@ -2,6 +2,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "neb_internal.h"
@@ -54,8 +55,12 @@ static bool is_device_ptr(const void* p) {
 struct Staging {   // temporaries of one ABI call
   neb_ctx* c;
   std::vector<void*> temps;
+  bool host_in = false;   // an input was copied from host memory and the stream has not been synchronised since
   explicit Staging(neb_ctx* c_) : c(c_) {}
   ~Staging() {
+    // inputs are borrowed for the duration of the call (neb.h): a copy from PINNED host memory is truly
+    // asynchronous, so the call may not return before it has been read
+    if (host_in) cudaStreamSynchronize(c->stream);
     for (void* p : temps) cudaFreeAsync(p, c->stream);
   }
   // device view of an input array (copied if it lives on the host)
@@ -67,6 +72,7 @@ struct Staging {   // temporaries of one ABI call
     NEB_CUDA(c, cudaMallocFromPoolAsync(&d, bytes, c->pool, c->stream));
     temps.push_back(d);
     NEB_CUDA(c, cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, c->stream));
+    host_in = true;
     *out = d;
     return NEB_OK;
   }
@@ -88,6 +94,7 @@ struct Staging {   // temporaries of one ABI call
     if (outs.empty()) return NEB_OK;
     for (auto& o : outs) NEB_CUDA(c, cudaMemcpyAsync(o.host, o.dev, o.bytes, cudaMemcpyDeviceToHost, c->stream));
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+    host_in = false;
     outs.clear();
     return NEB_OK;
   }
@@ -182,7 +189,9 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
     // n = e2 x e1 / |e2 x e1| (local Y); then local Z = X x Y so the frame is orthonormal
     double c0 = z0[1] * ex[2] - z0[2] * ex[1], c1 = z0[2] * ex[0] - z0[0] * ex[2], c2 = z0[0] * ex[1] - z0[1] * ex[0];
     double lc = sqrt(c0 * c0 + c1 * c1 + c2 * c2);
-    if (!(lc > 0.5)) { atomicOr(flag, 4); lc = 1.0; }   // edges must be (nearly) perpendicular
+    // the edges must be perpendicular (the closed forms are those of a rectangle / RIGHT triangle): |cos| <= 1e-9
+    const double cs = z0[0] * ex[0] + z0[1] * ex[1] + z0[2] * ex[2];
+    if (!(fabs(cs) <= 1e-9) || !(lc > 0.5)) { atomicOr(flag, 4); lc = 1.0; }
     ey[0] = c0 / lc; ey[1] = c1 / lc; ey[2] = c2 / lc;
     ez[0] = ex[1] * ey[2] - ex[2] * ey[1];
     ez[1] = ex[2] * ey[0] - ex[0] * ey[2];
@@ -261,6 +270,22 @@ __global__ void unpermute_matrix_kernel(int64_t n, int64_t ld, const int32_t* __
   if (si < n) out[(int64_t)perm[si] + (int64_t)perm[sj] * n] = K[si + sj * ld];
 }
 
+__global__ void inverse_perm_kernel(int64_t n, const int32_t* __restrict__ perm, int32_t* __restrict__ inv) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) inv[perm[s]] = (int32_t)s;
+}
+
+// out[r * n + perm[sj]] = K[inv[rows[r]] + sj * ld]; grid = (ceil(n/256), n_rows)
+__global__ void gather_rows_kernel(int64_t n, int64_t ld, const int32_t* __restrict__ perm, const int32_t* __restrict__ inv,
+                                   const int32_t* __restrict__ rows, const double* __restrict__ K, double* __restrict__ out,
+                                   int32_t* __restrict__ flag) {
+  int64_t sj = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t r = blockIdx.y;
+  const int32_t i = rows[r];
+  if (i < 0 || i >= n) { if (sj == 0) atomicOr(flag, 64); return; }
+  if (sj < n) out[r * n + perm[sj]] = K[(int64_t)inv[i] + sj * ld];
+}
+
 __global__ void unpermute_vector_kernel(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ v, double* __restrict__ out) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s < n) out[perm[s]] = v[s];
@@ -329,6 +354,7 @@ neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
   }
   for (int s = 0; ok && s < NEB_STAGE_COUNT; ++s)
     ok = cudaEventCreate(&c->ev0[s]) == cudaSuccess && cudaEventCreate(&c->ev1[s]) == cudaSuccess;
+  ok = ok && lu_init_device(c) == NEB_OK;
   if (!ok) {
     neb_destroy(c);
     return NEB_ECUDA;
@@ -381,8 +407,9 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
                         const double* radius, const double* colloc, const int32_t* bc_kind, const double* bc_value,
                         const double* eps_plus, const double* eps_minus, int32_t n_img, const double* img_shift) {
   if (!c) return NEB_EINVAL;
-  // the grid-wide LU panel keeps a slab of at most 384 rows per SM in shared memory: 148 x 384 = 56832 rows on a B200
-  const int64_t n_max = (int64_t)c->num_sms * 384 - kPad;
+  // the LU panel runs on one cluster of cluster_max_ctas x 256 threads with at most 32 rows per thread: 131072 rows on
+  // a B200 (the matrix itself, 8 n^2 bytes, reaches the 180 GB of HBM at n ~ 1.4e5)
+  const int64_t n_max = std::max<int64_t>(panel_cluster_max_rows(c), (int64_t)c->num_sms * 384) - kPad;
   if (n <= 0 || n > n_max || !kind || !v0 || !e1 || !e2 || !bc_kind)
     return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1.." + std::to_string(n_max) + " and kind, v0, e1, e2, bc_kind non-NULL");
   if (n_img < 0 || n_img > 32 || (n_img > 0 && !img_shift)) return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= 32");
@@ -646,6 +673,8 @@ neb_status neb_add_space_charge(neb_ctx* c, int64_t q, const double* pos, const 
   for (int f = 0; f < 3; ++f)
     NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + f * c->q_cap + c->q, pos + f * q, sizeof(double) * q, kp, c->stream));
   NEB_CUDA(c, cudaMemcpyAsync(c->d_charges + 3 * c->q_cap + c->q, charge, sizeof(double) * q, kq, c->stream));
+  // borrowed host buffers (pinned memory copies asynchronously) must have been read before the call returns
+  if (kp == cudaMemcpyHostToDevice || kq == cudaMemcpyHostToDevice) NEB_CUDA(c, cudaStreamSynchronize(c->stream));
   c->q = need;
   return NEB_OK;
 }
@@ -656,7 +685,7 @@ neb_status neb_voxelize_space_charge(neb_ctx* c, const double* origin, const dou
     if (!(voxel[a] > 0.0) || !isfinite(voxel[a]) || !isfinite(origin[a]) || dims[a] < 1)
       return fail(c, NEB_EINVAL, "neb_voxelize_space_charge: voxel sizes must be positive and finite, dims >= 1");
   if ((int64_t)dims[0] * dims[1] * dims[2] > (1LL << 26)) return fail(c, NEB_EINVAL, "neb_voxelize_space_charge: more than 2^26 voxels");
-  if (c->q == 0) return fail(c, NEB_ESTATE, "neb_voxelize_space_charge: no point charges (neb_add_space_charge first)");
+  if (c->q == 0 && c->n_lines == 0) return fail(c, NEB_ESTATE, "neb_voxelize_space_charge: no point charges (neb_add_space_charge first)");
   NEB_CUDA(c, cudaSetDevice(c->device));
   return voxelize_charges(c, origin, voxel, dims, n_lines_out);
 }
@@ -706,6 +735,33 @@ neb_status neb_get_matrix(neb_ctx* c, double* K_out) {
   unpermute_matrix_kernel<<<grid, 256, 0, c->stream>>>(c->n, c->npad, c->d_perm, c->d_K, (double*)dout);
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());
+  return sg.finish();
+}
+
+neb_status neb_get_matrix_rows(neb_ctx* c, int64_t n_rows, const int32_t* rows, double* K_out) {
+  if (!c || n_rows < 0 || (n_rows > 0 && (!rows || !K_out))) return NEB_EINVAL;
+  if (!c->assembled || c->factored) return fail(c, NEB_ESTATE, "neb_get_matrix_rows: only between neb_assemble and the first neb_solve");
+  if (n_rows == 0) return NEB_OK;
+  if (n_rows > 65535) return fail(c, NEB_EINVAL, "neb_get_matrix_rows: at most 65535 rows per call");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  Staging sg(c);
+  const void* drows;
+  void* dout;
+  int32_t* inv = nullptr;
+  NEB_TRY(sg.in(rows, sizeof(int32_t) * n_rows, &drows));
+  NEB_TRY(sg.out(K_out, sizeof(double) * (size_t)n_rows * (size_t)c->n, &dout));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&inv, sizeof(int32_t) * c->n, c->pool, c->stream));
+  sg.temps.push_back(inv);
+  NEB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int32_t), c->stream));
+  inverse_perm_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->d_perm, inv);
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)n_rows);
+  gather_rows_kernel<<<grid, 256, 0, c->stream>>>(c->n, c->npad, c->d_perm, inv, (const int32_t*)drows, c->d_K, (double*)dout, c->d_flag);
+  c->launches += 2;
+  NEB_CUDA(c, cudaGetLastError());
+  int32_t h_flag = 0;
+  NEB_CUDA(c, cudaMemcpyAsync(&h_flag, c->d_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (h_flag & 64) return fail(c, NEB_EINVAL, "neb_get_matrix_rows: row index outside [0, n)");
   return sg.finish();
 }
 

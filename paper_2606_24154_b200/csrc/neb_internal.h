@@ -43,6 +43,7 @@ struct neb_ctx {
   cudaEvent_t ev_next = nullptr, ev_panel = nullptr;
   cudaMemPool_t pool = nullptr;   // staging temporaries (stream-ordered, memory kept across syncs)
   int num_sms = 0;
+  int cluster_max_ctas = 0;   // largest cluster the device schedules for the LU panel kernel (set by lu_init_device)
   std::string err;
 
   // options
@@ -135,11 +136,13 @@ neb_status scale_matrix_rows(neb_ctx* c); // applies the row scales in place
 neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
 
 // neb_lu.cu ---------------------------------------------------------------------------------------
+neb_status lu_init_device(neb_ctx* c);    // per-device kernel attributes (dynamic shared memory, cluster size); from neb_create
 neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-scaled)
 neb_status lu_solve(neb_ctx* c);          // a6: d_x <- solution of (scaled) system for RHS d_b
 size_t lu_panel_ws_bytes(int num_sms);
 
 // neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
+int panel_cluster_probe();
 int64_t panel_cluster_max_rows(neb_ctx* c);
 neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream);
 

@@ -485,19 +485,25 @@ __global__ void tri_finish_kernel(int64_t npad, double* x) {
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
+// cudaFuncSetAttribute applies to the CURRENT device only: done once per context, right after cudaSetDevice.
+neb_status lu_init_device(neb_ctx* c) {
+  NEB_CUDA(c, cudaFuncSetAttribute(panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  NEB_CUDA(c, cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
+  NEB_CUDA(c, cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM));
+  NEB_CUDA(c, cudaFuncSetAttribute(diag_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * NB * (NB + 1) * sizeof(double))));
+  NEB_CUDA(c, cudaFuncSetAttribute(compose_perm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  c->cluster_max_ctas = panel_cluster_probe();
+  return NEB_OK;
+}
+
 neb_status lu_factor(neb_ctx* c) {
   const int64_t npad = c->npad, ld = c->npad;
   StageTimer tt(c, NEB_STAGE_LU);
-  static bool attr_set = false;
-  if (!attr_set) {
-    NEB_CUDA(c, cudaFuncSetAttribute(panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    NEB_CUDA(c, cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
-    NEB_CUDA(c, cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM));
-    NEB_CUDA(c, cudaFuncSetAttribute(diag_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * NB * (NB + 1) * sizeof(double))));
-    attr_set = true;
-  }
   PanelWs* ws = (PanelWs*)c->d_panel_ws;
+  // panels run on one cluster (neb_lu_panel.cu) whatever their height; NEB_OPT_LU_PANEL = 1 selects the grid-wide
+  // cooperative kernel of round 1 instead (all SMs, no look-ahead, n <= 148 x 384 - 128): kept as a cross-check
   const int64_t cluster_rows = c->panel_mode == 0 ? panel_cluster_max_rows(c) : 0;
+  constexpr int64_t kChainRows = 8192;     // below this the panel chain, not the update, is the critical path
   cudaStream_t S1 = c->stream, S2 = c->side_stream;
 
   // panel k on stream st: the cluster kernel where the panel fits, else the grid-wide cooperative kernel
@@ -560,7 +566,7 @@ neb_status lu_factor(neb_ctx* c) {
   // default) once the remaining panels run on a cluster with look-ahead: there the chain of panels is the critical
   // path and anything added to it (the in-block updates, a wider look-ahead slice) costs more than the deeper
   // update saves.
-  auto block_width = [&](int64_t remaining) -> int64_t { return remaining > cluster_rows ? 4 * NB : (int64_t)c->lu_nb; };
+  auto block_width = [&](int64_t remaining) -> int64_t { return remaining > kChainRows ? 4 * NB : (int64_t)c->lu_nb; };
   bool chain_on_side = false;
   for (int64_t kb = 0; kb < npad;) {
     const int64_t w = min(block_width(npad - kb), npad - kb), nb = kb + w;
@@ -604,11 +610,6 @@ neb_status lu_factor(neb_ctx* c) {
   }
   // composed permutation for the solves
   if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
-    static bool attr2 = false;
-    if (!attr2) {
-      NEB_CUDA(c, cudaFuncSetAttribute(compose_perm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-      attr2 = true;
-    }
     compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * sizeof(unsigned), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
   } else {
     compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);

@@ -4,8 +4,8 @@
 // floor((p - origin)/voxel) clamped to the grid; an occupied voxel (at least one point, Alg. 3's isOccupied)
 // becomes one line through its centre, parallel to z, spanning its z extent, lambda = total charge / voxel_z.
 //
-//   Kernel 1 (scatter)  one thread per point: atomicAdd of the charge into the voxel's total, atomicOr of its
-//                       occupancy flag.
+//   Kernel 1 (scatter)  one thread per point: the charge is added to the voxel's total in 128-bit fixed point by
+//                       integer atomics (order-independent: lambda is bit-reproducible), atomicOr of its occupancy flag.
 //   Kernel 2 (reduce)   instead of Alg. 3's atomicAdd on a global line counter (arbitrary order), the occupied
 //                       voxels are compacted by a scan, so that the line list is in voxel-index order on every run:
 //                       count per 1024-voxel block -> exclusive scan of the block counts -> ballot/popc ranks.
@@ -26,19 +26,62 @@ struct VoxGrid {
   int n[3];
 };
 
-__global__ void voxel_scatter_kernel(int64_t q, int64_t q_stride, const double* __restrict__ ch, VoxGrid g,
-                                     double* __restrict__ total, unsigned* __restrict__ occupied) {
+// Voxel totals are accumulated in 128-bit FIXED POINT with integer atomics, so that they do not depend on the order in
+// which the threads arrive (an fp64 atomicAdd would make lambda order-dependent in its last bits): with
+// e = 35 - exponent(max |q|) every charge becomes x = q 2^e, |x| < 2^36, split exactly into an integer part and a
+// fraction kept to 2^-36; the two parts are summed in two 64-bit integers per voxel (no overflow below 2^26 charges),
+// i.e. each charge enters with an absolute error below 2^-72 max|q| and the sum itself is exact.
+constexpr int kFixFrac = 36;
+
+// max |charge| as an integer max on the bit pattern (non-negative doubles order like their bits); sources c >= q are
+// the line charges of an earlier voxelisation, folded back in as their total charge lambda (z_stop - z_start)
+__device__ __forceinline__ double voxel_source_charge(int64_t c, int64_t q, int64_t q_stride, const double* __restrict__ ch,
+                                                      int64_t line_cap, const double* __restrict__ lines) {
+  if (c < q) return ch[3 * q_stride + c];
+  const int64_t l = c - q;
+  return lines[4 * line_cap + l] * (lines[3 * line_cap + l] - lines[2 * line_cap + l]);
+}
+
+__global__ void voxel_maxabs_kernel(int64_t q, int64_t q_stride, const double* __restrict__ ch, int64_t nl, int64_t line_cap,
+                                    const double* __restrict__ lines, unsigned long long* __restrict__ maxbits) {
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= q) return;
+  unsigned long long b = 0ull;
+  if (c < q + nl) {
+    double v = fabs(voxel_source_charge(c, q, q_stride, ch, line_cap, lines));
+    if (v == v && v < 1.0e300) b = (unsigned long long)__double_as_longlong(v);
+  }
+  b = __reduce_max_sync(0xffffffffu, (unsigned)(b >> 32)) == (unsigned)(b >> 32) ? b : 0ull;   // cheap pre-filter per warp
+  if (b) atomicMax(maxbits, b);
+}
+
+__global__ void voxel_scatter_kernel(int64_t q, int64_t q_stride, const double* __restrict__ ch, int64_t nl, int64_t line_cap,
+                                     const double* __restrict__ lines, VoxGrid g, const unsigned long long* __restrict__ maxbits,
+                                     unsigned long long* __restrict__ tot_hi, unsigned long long* __restrict__ tot_lo,
+                                     unsigned* __restrict__ occupied) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= q + nl) return;
+  double p[3];
+  if (c < q) { p[0] = ch[c]; p[1] = ch[q_stride + c]; p[2] = ch[2 * q_stride + c]; }
+  else {
+    const int64_t l = c - q;          // an earlier line: its total charge at its centre
+    p[0] = lines[l]; p[1] = lines[line_cap + l]; p[2] = 0.5 * (lines[2 * line_cap + l] + lines[3 * line_cap + l]);
+  }
   int64_t idx[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    double t = floor((ch[a * q_stride + c] - g.o[a]) / g.d[a]);
+    double t = floor((p[a] - g.o[a]) / g.d[a]);
     t = fmin(fmax(t, 0.0), (double)(g.n[a] - 1));         // points outside count in the nearest border voxel
     idx[a] = (int64_t)t;
   }
   const int64_t v = (idx[2] * g.n[1] + idx[1]) * g.n[0] + idx[0];
-  atomicAdd(total + v, ch[3 * q_stride + c]);
+  const double mx = __longlong_as_double((long long)*maxbits);
+  const int e = (mx > 0.0) ? (kFixFrac - 1) - ilogb(mx) : 0;
+  const double x = scalbn(voxel_source_charge(c, q, q_stride, ch, line_cap, lines), e);    // exact; |x| < 2^36
+  const double fl = floor(x);
+  const long long hi = (long long)fl;
+  const long long lo = (long long)scalbn(x - fl, kFixFrac);       // fraction in [0, 1), truncated at 2^-36
+  atomicAdd(tot_hi + v, (unsigned long long)hi);
+  atomicAdd(tot_lo + v, (unsigned long long)lo);
   atomicOr(occupied + (v >> 5), 1u << (v & 31));
 }
 
@@ -87,7 +130,9 @@ __global__ void __launch_bounds__(1024) voxel_scan_kernel(int32_t nblocks, const
 }
 
 // one CTA of 1024 threads per block of 1024 voxels: rank of each occupied voxel, then its line
-__global__ void __launch_bounds__(kVoxBlock) voxel_lines_kernel(int64_t nv, VoxGrid g, const double* __restrict__ total,
+__global__ void __launch_bounds__(kVoxBlock) voxel_lines_kernel(int64_t nv, VoxGrid g, const unsigned long long* __restrict__ maxbits,
+                                                                const unsigned long long* __restrict__ tot_hi,
+                                                                const unsigned long long* __restrict__ tot_lo,
                                                                 const unsigned* __restrict__ occupied, const int32_t* __restrict__ block_off,
                                                                 int64_t cap, double* __restrict__ lines) {
   __shared__ int s_pre[32];
@@ -114,7 +159,10 @@ __global__ void __launch_bounds__(kVoxBlock) voxel_lines_kernel(int64_t nv, VoxG
   lines[1 * cap + L] = __dadd_rn(g.o[1], __dmul_rn((double)j + 0.5, g.d[1]));
   lines[2 * cap + L] = __dadd_rn(g.o[2], __dmul_rn((double)k, g.d[2]));
   lines[3 * cap + L] = __dadd_rn(g.o[2], __dmul_rn((double)(k + 1), g.d[2]));
-  lines[4 * cap + L] = total[v] / g.d[2];
+  const double mx = __longlong_as_double((long long)*maxbits);
+  const int e = (mx > 0.0) ? (kFixFrac - 1) - ilogb(mx) : 0;
+  const double total = scalbn((double)(long long)tot_hi[v] + scalbn((double)(long long)tot_lo[v], -kFixFrac), -e);
+  lines[4 * cap + L] = total / g.d[2];
 }
 
 // Direct sum over line charges parallel to z.  grid = (ceil(m/128), n_split); partial[(split*4 + c) * m + p],
@@ -170,28 +218,40 @@ neb_status voxelize_charges(neb_ctx* c, const double* origin, const double* voxe
   for (int a = 0; a < 3; ++a) { g.o[a] = origin[a]; g.d[a] = voxel[a]; g.n[a] = dims[a]; }
   const int64_t nv = (int64_t)dims[0] * dims[1] * dims[2];
   const int64_t nwords = (nv + 31) / 32, nblocks = (nv + kVoxBlock - 1) / kVoxBlock;
-  double* total = nullptr;
+  // sources: the point charges held now, and the lines of an earlier voxelisation (each as its total charge at its
+  // centre), so that charge is conserved over repeated calls
+  const int64_t nsrc = c->q + c->n_lines;
+  if (nsrc > (1LL << 26)) return fail(c, NEB_EINVAL, "neb_voxelize_space_charge: more than 2^26 charges");
+  unsigned long long *tot_hi = nullptr, *tot_lo = nullptr, *maxbits = nullptr;
   unsigned* occ = nullptr;
   int32_t *bcount = nullptr, *boff = nullptr;
   int64_t* d_nl = nullptr;
+  double* old_lines = c->d_lines;
+  const int64_t old_cap = c->line_cap, old_nl = c->n_lines;
   // the flag words are padded to whole blocks so that voxel_count_kernel's last CTA reads initialised memory
-  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&total, sizeof(double) * (size_t)nv, c->pool, c->stream));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tot_hi, sizeof(unsigned long long) * (size_t)nv, c->pool, c->stream));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tot_lo, sizeof(unsigned long long) * (size_t)nv, c->pool, c->stream));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&maxbits, sizeof(unsigned long long), c->pool, c->stream));
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&occ, sizeof(unsigned) * (size_t)(nblocks * 32), c->pool, c->stream));
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&bcount, sizeof(int32_t) * (size_t)nblocks, c->pool, c->stream));
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&boff, sizeof(int32_t) * (size_t)nblocks, c->pool, c->stream));
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&d_nl, sizeof(int64_t), c->pool, c->stream));
-  NEB_CUDA(c, cudaMemsetAsync(total, 0, sizeof(double) * (size_t)nv, c->stream));
+  NEB_CUDA(c, cudaMemsetAsync(tot_hi, 0, sizeof(unsigned long long) * (size_t)nv, c->stream));
+  NEB_CUDA(c, cudaMemsetAsync(tot_lo, 0, sizeof(unsigned long long) * (size_t)nv, c->stream));
+  NEB_CUDA(c, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long), c->stream));
   NEB_CUDA(c, cudaMemsetAsync(occ, 0, sizeof(unsigned) * (size_t)(nblocks * 32), c->stream));
   int64_t nl = 0;
   {
     StageTimer t(c, NEB_STAGE_CHARGES);
-    voxel_scatter_kernel<<<(unsigned)((c->q + 255) / 256), 256, 0, c->stream>>>(c->q, c->q_cap, c->d_charges, g, total, occ);
+    const unsigned sb = (unsigned)((nsrc + 255) / 256);
+    voxel_maxabs_kernel<<<sb, 256, 0, c->stream>>>(c->q, c->q_cap, c->d_charges, old_nl, old_cap, old_lines, maxbits);
+    voxel_scatter_kernel<<<sb, 256, 0, c->stream>>>(c->q, c->q_cap, c->d_charges, old_nl, old_cap, old_lines, g, maxbits, tot_hi, tot_lo, occ);
     voxel_count_kernel<<<(unsigned)nblocks, 32, 0, c->stream>>>(nwords, occ, bcount);
     voxel_scan_kernel<<<1, 1024, 0, c->stream>>>((int32_t)nblocks, bcount, boff, d_nl);
-    c->launches += 3;
+    c->launches += 4;
   }
   NEB_CUDA(c, cudaMemcpyAsync(&nl, d_nl, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
-  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));            // the old lines have been read by now
   if (nl > c->line_cap) {
     if (c->d_lines) NEB_CUDA(c, cudaFree(c->d_lines));
     c->d_lines = nullptr;
@@ -200,11 +260,13 @@ neb_status voxelize_charges(neb_ctx* c, const double* origin, const double* voxe
   }
   {
     StageTimer t(c, NEB_STAGE_CHARGES);
-    voxel_lines_kernel<<<(unsigned)nblocks, kVoxBlock, 0, c->stream>>>(nv, g, total, occ, boff, c->line_cap, c->d_lines);
+    voxel_lines_kernel<<<(unsigned)nblocks, kVoxBlock, 0, c->stream>>>(nv, g, maxbits, tot_hi, tot_lo, occ, boff, c->line_cap, c->d_lines);
     c->launches++;
   }
   NEB_CUDA(c, cudaGetLastError());
-  cudaFreeAsync(total, c->stream);
+  cudaFreeAsync(tot_hi, c->stream);
+  cudaFreeAsync(tot_lo, c->stream);
+  cudaFreeAsync(maxbits, c->stream);
   cudaFreeAsync(occ, c->stream);
   cudaFreeAsync(bcount, c->stream);
   cudaFreeAsync(boff, c->stream);

@@ -1,11 +1,15 @@
 """Parity of the CUDA path (through the C ABI of include/neb.h) against the CPU oracle, element by
 element on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
   * Phi and |E|: max relative error 1e-10 for points farther than 1e-3 element sizes from every
-    element, 1e-7 otherwise (reading S18); denominators are floored at 1e-6 x the median magnitude so
-    that points where the field cancels to zero do not divide by zero;
+    element, 1e-7 otherwise (reading S18).  A field value is a sum of 1e2..1e6 terms of both signs; where it
+    cancels its rounding error is still eps x (sum of the terms' magnitudes) in ANY implementation, so the
+    allowance is PER POINT  tol x |value| + C_SUM x eps x S(point),  S = the oracle's sum of term magnitudes
+    (orc_eval_abs), eps = 2^-53, C_SUM = 32 (derivation and the measured worst ratio).  There is
+    no global floor on |Phi|;
   * solved charge densities: 1e-9 relative, norm-wise (reading S14); LU residual 1e-13 (S16).
-The oracle runs in its long-double build ("ld") as the truth.
+The oracle runs in its long-double build ("ld") as the truth unless a test says otherwise.
 """
+import json
 import os
 
 import numpy as np
@@ -16,6 +20,11 @@ from workloads import configs as W
 pytestmark = pytest.mark.gpu
 
 TOL_FAR, TOL_NEAR, TOL_SIGMA, TOL_K = 1e-10, 1e-7, 1e-9, 1e-10
+EPS = 2.0 ** -53
+C_SUM = 32.0            # allowance for a cancelled sum: C_SUM x eps x sum|terms|
+C_SUM_F64 = 256.0       # the same against the oracle's fp64 build, which itself carries up to ~105 eps S (measured against
+                        # its long-double build on C1: the 4-corner form cancels in the far field); used for C4's 10 steps
+_STATS = {}             # worst observed |error| / (eps x S) per check, dumped to $NEB_PARITY_STATS if set
 
 
 @pytest.fixture(scope="module")
@@ -31,12 +40,19 @@ def nb(P):
     h.close()
 
 
+@pytest.fixture(scope="module", autouse=True)
+def _dump_stats():
+    yield
+    path = os.environ.get("NEB_PARITY_STATS")
+    if path:
+        with open(path, "w") as fh:
+            json.dump(_STATS, fh, indent=1, sort_keys=True)
+
+
 def rel_err(got, want):
-    # A potential is a sum over ~1e4-1e6 terms of both signs (electrodes at 0 and -2000 V): where it happens to cancel
-    # to ~0 its error is still eps x (sum of the terms' magnitudes), so the denominator is floored at 1e-4 of the typical
-    # magnitude; even the oracle's own fp64 and long-double builds differ by 6e-10 "relative" at such a
-    # zero crossing.
-    floor = 1e-4 * np.median(np.abs(want)) if want.size else 0.0
+    """Relative error with the denominator floored at 1e-6 x the median magnitude: only for quantities that have no
+    per-point scale from the oracle (interpolated FastVolume values, line-charge sums)."""
+    floor = 1e-6 * np.median(np.abs(want)) if want.size else 0.0
     return np.abs(got - want) / np.maximum(np.abs(want), floor)
 
 
@@ -47,10 +63,45 @@ def vec_rel_err(got, want, floor=None):
     return np.linalg.norm(got - want, axis=0) / np.maximum(mag, floor)
 
 
-def check_field(phi, E, phi_o, E_o, tol, what="", floor_E=None):
-    e1, e2 = rel_err(phi, phi_o).max(), vec_rel_err(E, E_o, floor_E).max()
-    assert e1 <= tol, f"{what} Phi rel err {e1:.3e} > {tol}"
-    assert e2 <= tol, f"{what} |E| rel err {e2:.3e} > {tol}"
+def truth(orc, g, sig, pts, pos=None, q=None, mode="ld"):
+    """Oracle Phi, E at pts and the per-point scales (S_Phi, S_E) of their rounding error."""
+    s_phi, s_E, phi_o, E_o = orc.evaluate_abs(g, sig, pts, pos, q, mode=mode, with_field=True)
+    return phi_o, E_o, (s_phi, s_E)
+
+
+def check_field(phi, E, phi_o, E_o, tol, what="", scale=None, c_sum=C_SUM):
+    """|dPhi| <= tol |Phi| + C_SUM eps S_Phi and |dE| <= tol |E| + C_SUM eps S_E at every point (scale = (S_Phi, S_E)
+    from truth()); without a scale: the floored relative error of rel_err / vec_rel_err."""
+    if scale is None:
+        e1 = rel_err(phi, phi_o).max(initial=0.0) if phi is not None else 0.0
+        e2 = vec_rel_err(E, E_o).max(initial=0.0)
+        assert e1 <= tol, f"{what} Phi rel err {e1:.3e} > {tol}"
+        assert e2 <= tol, f"{what} |E| rel err {e2:.3e} > {tol}"
+        return
+    s_phi, s_E = scale
+    dE, mE = np.linalg.norm(E - E_o, axis=0), np.linalg.norm(E_o, axis=0)
+    ratio_E = dE / (tol * mE + c_sum * EPS * s_E)
+    stat = {"E_err_over_eps_S": float(np.max(dE / (EPS * s_E), initial=0.0)), "E_rel": float(np.max(dE / mE, initial=0.0))}
+    ratio_phi = np.zeros(1)
+    if phi is not None:
+        dP = np.abs(phi - phi_o)
+        ratio_phi = dP / (tol * np.abs(phi_o) + c_sum * EPS * s_phi)
+        stat.update({"Phi_err_over_eps_S": float(np.max(dP / (EPS * s_phi), initial=0.0)),
+                     "Phi_rel": float(np.max(dP / np.abs(phi_o), initial=0.0))})
+    _STATS[what] = stat
+    assert ratio_phi.max(initial=0.0) <= 1.0, f"{what} Phi: {ratio_phi.max():.3f} x the allowance; {stat}"
+    assert ratio_E.max(initial=0.0) <= 1.0, f"{what} |E|: {ratio_E.max():.3f} x the allowance; {stat}"
+
+
+def near_surface_points(pr, rs, count, rel_height=(1e-6, 5e-4)):
+    """Points hovering over the interior of `count` random flat elements at rel_height x (longer side) from the
+    surface: closer than 1e-3 element sizes, the 1e-7 tolerance class of reading S18."""
+    flat = np.flatnonzero(pr.kind != W.WIRE)
+    j = rs.choice(flat, count, replace=flat.size < count)
+    s, t = rs.uniform(0.2, 0.4, size=count), rs.uniform(0.2, 0.4, size=count)
+    L = np.maximum(np.linalg.norm(pr.e1[:, j], axis=0), np.linalg.norm(pr.e2[:, j], axis=0))
+    h = L * 10.0 ** rs.uniform(np.log10(rel_height[0]), np.log10(rel_height[1]), size=count) * rs.choice([-1.0, 1.0], size=count)
+    return pr.v0[:, j] + pr.e1[:, j] * s + pr.e2[:, j] * t + pr.normals()[:, j] * h
 
 
 def test_native_library_is_in_tree(P):
@@ -180,8 +231,8 @@ def test_assembly_and_eval_random_mixed(nb, orc, math):
     sig = np.linspace(1e-6, 2e-6, pr.n)
     nb.set_sigma(sig)
     phi, E = nb.eval(pr.points)
-    phi_o, E_o = orc.evaluate(g, sig, pr.points)
-    check_field(phi, E, phi_o, E_o, TOL_FAR, "random mixed")
+    phi_o, E_o, S = truth(orc, g, sig, pr.points)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, f"random mixed math={math}", S)
 
 
 def test_explicit_collocation_points(nb, orc):
@@ -212,9 +263,11 @@ def _pipeline(nb, orc, pr, pts=None, orc_mode="ld"):
     res = np.max(np.abs(K @ s - b)) / (np.abs(K).sum(axis=1).max() * np.abs(s).max())
     assert res <= 1e-13
     if pts is not None:
+        # a7 parity on the SAME sigma (the GPU's; sigma itself is compared above): where the field cancels (inside a
+        # conductor) a 1e-13 difference between two solves would otherwise show up as a field "error"
         phi, E = nb.eval(pts)
-        phi_o, E_o = orc.evaluate(g, so, pts, pr.charge_pos, pr.charge_q, mode=orc_mode)
-        check_field(phi, E, phi_o, E_o, TOL_FAR, pr.name)
+        phi_o, E_o, S = truth(orc, g, s, pts, pr.charge_pos, pr.charge_q, mode=orc_mode)
+        check_field(phi, E, phi_o, E_o, TOL_FAR, pr.name, S)
     return g, s, so
 
 
@@ -256,8 +309,9 @@ def test_c1_cube_reduced_and_capacitance_sequence(nb, orc):
 
 
 def test_c1_cube_full_size(nb, orc):
-    """BASELINE configs[1] in the launch configuration bench.py times: 6144 panels, 1e5 points.
-    sigma against the (fp64, OpenMP) oracle LU; Phi/E on sampled points; properties at every point."""
+    """BASELINE configs[1] at full size: 6144 panels, 1e5 points.  sigma against the (fp64, OpenMP) oracle LU; Phi/E on
+    2000 sampled points (per-point allowance: inside the conductor the 6144 contributions cancel to E = 0) and on
+    near-surface points (1e-7 class of reading S18); properties at every point."""
     import torch
     pr = W.cube()
     g = orc.Geometry(pr)
@@ -277,15 +331,14 @@ def test_c1_cube_full_size(nb, orc):
     pts = torch.from_numpy(pr.points).cuda()
     phi, E = nb.eval(pts)
     phi, E = phi.cpu().numpy(), E.cpu().numpy()
-    idx = rs.choice(pr.points.shape[1], 300, replace=False)
-    phi_o, E_o = orc.evaluate(g, so, pr.points[:, idx])
-    inside = np.all(np.abs(pr.points) < 0.005, axis=0)      # inside the conductor: Phi = 1 V, E = 0
-    # inside the conductor the 6144 contributions cancel to E = 0 (up to the mesh error): a relative error of
-    # that remainder measures the cancellation, not the kernel, so there the error is taken relative to the
-    # field just outside (median exterior magnitude)
-    e_out = np.median(np.linalg.norm(E_o[:, ~inside[idx]], axis=0))
-    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C1 sampled", floor_E=np.where(inside[idx], e_out, 0.0))
-    inside = np.all(np.abs(pr.points) < 0.0045, axis=0)
+    idx = rs.choice(pr.points.shape[1], 2000, replace=False)
+    phi_o, E_o, S = truth(orc, g, s, pr.points[:, idx])       # same sigma on both sides (sigma is compared above)
+    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C1 sampled", S)
+    near = near_surface_points(pr, rs, 300)
+    phi_n, E_n = nb.eval(near)
+    phi_o, E_o, S = truth(orc, g, s, near)
+    check_field(phi_n, E_n, phi_o, E_o, TOL_NEAR, "C1 near surface", S)
+    inside = np.all(np.abs(pr.points) < 0.0045, axis=0)     # inside the conductor: Phi = 1 V up to the mesh error
     assert inside.sum() > 1000
     assert np.max(np.abs(phi[inside] - 1.0)) < 2e-3
     assert np.all(phi < 1.05) and np.all(phi > 0)            # maximum principle up to the mesh's collocation error
@@ -305,27 +358,42 @@ def test_c3_double_thgem_reduced_with_images(nb, orc):
     _pipeline(nb, orc, pr, pr.points, orc_mode="f64")
 
 
-def test_c2_thgem_full_size_sampled(nb, orc):
-    """BASELINE configs[2] at full size (N = 19400, 100^3 grid): sampled matrix entries, residual of the
-    GPU sigma against ORACLE-computed rows, sampled grid nodes; mirror symmetry of the whole map."""
+def test_c2_thgem_full_size(nb, orc):
+    """BASELINE configs[2] at full size (N = 19400: rectangles + right triangles, 4608 dielectric rows; 100^3 grid):
+    the WHOLE matrix against the oracle's, sigma against the oracle's full solve (oracle.solve_library on the
+    oracle's matrix), 2000 sampled grid nodes and 300 near-surface points against the long-double oracle; mirror
+    symmetry of the whole map."""
     import torch
     pr = W.thgem()
+    assert pr.n == 19400
     g = orc.Geometry(pr)
+    Ko = orc.assemble(g, mode="f64")                          # 3.8e8 pair evaluations on the host cores
+    so = orc.solve_library(Ko, orc.rhs(g, mode="f64"))
     nb.assemble_problem(pr)
+    K = nb.get_matrix()
+    rowmax = np.abs(Ko).max(axis=1)
+    worst = 0.0
+    for r0 in range(0, pr.n, 2048):                           # in slabs: no 3 GB temporaries
+        worst = max(worst, float(np.max(np.abs(K[r0:r0 + 2048] - Ko[r0:r0 + 2048]) / rowmax[r0:r0 + 2048, None])))
+    assert worst <= TOL_K, worst
     s = nb.solve()
-    rs = np.random.RandomState(2)
-    rows = rs.choice(pr.n, 48, replace=False)
-    R, Cc = np.repeat(rows, pr.n), np.tile(np.arange(pr.n), rows.size)
-    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)
-    b = orc.rhs(g, mode="f64")[rows]
-    res = np.abs(Krows @ s - b) / (np.abs(Krows).sum(axis=1) * np.abs(s).max())
-    assert res.max() <= 1e-12
+    assert np.max(np.abs(s - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    b = nb.get_rhs()
+    # S16's 1e-13 is relative to ||K||_inf ||sigma||_inf of the ROW-SCALED system (rows of 1e5 and 1e11 here)
+    res = np.abs(K @ s - b) / (np.abs(K).sum(axis=1) * np.abs(s).max())
+    assert res.max() <= 1e-13, res.max()
+    del K, Ko
     pts = torch.from_numpy(pr.points).cuda()
     phi, E = nb.eval(pts)
     phi, E = phi.cpu().numpy(), E.cpu().numpy()
-    idx = rs.choice(pr.points.shape[1], 64, replace=False)
-    phi_o, E_o = orc.evaluate(g, s, pr.points[:, idx], mode="ld")
-    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C2 sampled")
+    rs = np.random.RandomState(2)
+    idx = rs.choice(pr.points.shape[1], 2000, replace=False)
+    phi_o, E_o, S = truth(orc, g, s, pr.points[:, idx])
+    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C2 sampled nodes", S)
+    near = near_surface_points(pr, rs, 300)
+    phi_n, E_n = nb.eval(near)
+    phi_o, E_o, S = truth(orc, g, s, near)
+    check_field(phi_n, E_n, phi_o, E_o, TOL_NEAR, "C2 near surface", S)
     # the cell is mirror symmetric in x and in y: Phi(x,y,z) = Phi(-x,y,z) = Phi(x,-y,z), E_x odd in x
     G = phi.reshape(100, 100, 100)                          # [z, y, x]
     scale = np.abs(G).max()
@@ -347,13 +415,17 @@ def _rows_geometry(orc, g, rows):
     return gs
 
 
-def test_c3_c4_full_size_sampled(nb, orc):
-    """BASELINE configs[3] and [4] at FULL size on one GPU: N = 49928 panels with 5x5 image copies (fp64 matrix
-    of 20 GB, 6.2e10 pair evaluations), LU, then (C3) a 2e5-point slab of the 1e7 seeded points and (C4) one
-    step of the space-charge loop with all 1e6 charges: E at the charges from the panels and from all other
-    charges, push, RHS update, re-solve on the resident factors.  The oracle cannot factor 50k x 50k in test
-    time, so parity is (a) the residual of the GPU sigma against ORACLE-computed matrix rows and right-hand
-    sides on sampled rows and (b) Phi/E on sampled points / charges."""
+def test_c3_c4_full_size(nb, orc):
+    """BASELINE configs[3] and [4] at FULL size on one GPU, in the launch configuration bench.py times.
+    C3: N = 49928 panels x 25 image copies (20 GB fp64 matrix, 6.2e10 pair evaluations), LU, Phi/E at ALL 1e7 seeded
+    points.  The oracle cannot factor 50k x 50k in test time, so: 1024 matrix rows, entry by entry,
+    against the oracle; the residual of the GPU sigma on those oracle rows; 1024 points sampled over all 1e7 and 128
+    near-surface points against the long-double oracle.
+    C4: all 10 self-consistent steps with all 1e6 charges (per step 1.25e12 element pairs + 1e12 charge pairs, push,
+    RHS update, re-solve on the resident factors); per step 1024 sampled charges: E from the panels and all other
+    charges against the oracle (fp64 build: 1.3e9 + 1e9 pair evaluations per step), the push, and the re-solved
+    sigma through the residual on the oracle rows with the oracle's right-hand side; first and last step also
+    against the long-double build on 64 charges."""
     import torch
     if torch.cuda.get_device_properties(0).total_memory < 60e9:
         pytest.skip("needs ~25 GB of device memory")
@@ -361,46 +433,68 @@ def test_c3_c4_full_size_sampled(nb, orc):
     assert pr.n > 45000 and pr.n_img == 25 and pr.points.shape[1] == 10_000_000 and pr.charge_q.shape[0] == 1_000_000
     g = orc.Geometry(pr)
     rs = np.random.RandomState(34)
-    rows = rs.choice(pr.n, 16, replace=False)
+    n_rows = 1024
+    rows = np.sort(rs.choice(pr.n, n_rows, replace=False))
+    assert np.sum(pr.bc_kind[rows] == W.DIELECTRIC) > 100 and np.sum(pr.kind[rows] == W.TRI) > 5
     R, Cc = np.repeat(rows, pr.n), np.tile(np.arange(pr.n), rows.size)
-    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)
+    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)      # 1.3e9 pair evaluations
     gs = _rows_geometry(orc, g, rows)
-    # ---- C3: assemble, factor, solve, evaluate
+    rowsum = np.abs(Krows).sum(axis=1)
+    # ---- C3: assemble, matrix rows, factor, solve, evaluate at all 1e7 points
     nb.assemble_problem(pr)
+    Kg = nb.get_matrix_rows(rows)
+    assert np.max(np.abs(Kg - Krows) / np.abs(Krows).max(axis=1, keepdims=True)) <= TOL_K
+    del Kg
     s = nb.solve()
-    res = np.abs(Krows @ s - orc.rhs(gs, mode="f64")) / (np.abs(Krows).sum(axis=1) * np.abs(s).max())
-    assert res.max() <= 1e-12
-    m = 200_000
-    pts = torch.from_numpy(np.ascontiguousarray(pr.points[:, :m])).cuda()
+    res = np.abs(Krows @ s - orc.rhs(gs, mode="f64")) / (rowsum * np.abs(s).max())
+    assert res.max() <= 1e-12, res.max()            # oracle rows in fp64: their own rounding is ~1e-13 of the row sum
+    pts = torch.from_numpy(pr.points).cuda()
     phi, E = nb.eval(pts)
-    phi, E = phi.cpu().numpy(), E.cpu().numpy()
-    idx = rs.choice(m, 32, replace=False)
-    phi_o, E_o = orc.evaluate(g, s, pr.points[:, idx], mode="ld")
-    check_field(phi[idx], E[:, idx], phi_o, E_o, TOL_FAR, "C3 sampled")
-    assert phi.min() > -2000.0 - 40.0 and phi.max() < 40.0       # maximum principle up to the mesh error
-    # ---- C4: one full-size step on the resident factors
+    del pts
+    idx = np.sort(rs.choice(pr.points.shape[1], 1024, replace=False))
+    assert idx[0] < 100_000 and idx[-1] > 9_900_000                        # spread over all 1e7
+    tidx = torch.from_numpy(idx).cuda()
+    phi_s, E_s = phi[tidx].cpu().numpy(), E[:, tidx].cpu().numpy()
+    assert float(phi.min()) > -2000.0 - 40.0 and float(phi.max()) < 40.0  # maximum principle up to the mesh error
+    del phi, E
+    phi_o, E_o, S = truth(orc, g, s, pr.points[:, idx])
+    check_field(phi_s, E_s, phi_o, E_o, TOL_FAR, "C3 sampled over 1e7", S)
+    near = near_surface_points(pr, rs, 128)
+    phi_n, E_n = nb.eval(near)
+    phi_o, E_o, S = truth(orc, g, s, near)
+    check_field(phi_n, E_n, phi_o, E_o, TOL_NEAR, "C3 near surface", S)
+    # ---- C4: 10 full-size steps on the resident factors
     pos = torch.from_numpy(pr.charge_pos.copy()).cuda()
     ch = torch.from_numpy(pr.charge_q).cuda()
-    nb.add_space_charge(pos, ch)
-    s1 = nb.solve()
-    b1 = orc.rhs(gs, pr.charge_pos, pr.charge_q, mode="f64")
-    assert np.max(np.abs(nb.get_rhs()[rows] - b1) / np.maximum(np.abs(b1), 1e-6 * np.abs(b1).max())) <= TOL_FAR
-    res = np.abs(Krows @ s1 - b1) / (np.abs(Krows).sum(axis=1) * np.abs(s1).max())
-    assert res.max() <= 1e-12
-    assert np.max(np.abs(s1 - s)) > 0.0                          # the charges changed the right-hand side
-    _, Eq = nb.eval(pos, want_phi=False)                         # 1.25e12 element pairs + 1e12 charge pairs
-    cidx = rs.choice(pr.charge_q.shape[0], 16, replace=False)
-    _, Eq_o = orc.evaluate(g, s1, pr.charge_pos[:, cidx], pr.charge_pos, pr.charge_q, mode="ld")
-    assert vec_rel_err(Eq.cpu().numpy()[:, cidx], Eq_o).max() <= TOL_FAR
     mu_dt = pr.meta["mu"] * pr.meta["dt"]
-    nb.push(pos, Eq, mu_dt)
-    pos_o = orc.push(pr.charge_pos[:, cidx], Eq_o, pr.meta["mu"], pr.meta["dt"])
-    assert np.max(np.abs(pos.cpu().numpy()[:, cidx] - pos_o)) <= 1e-12 * np.max(np.abs(pos_o))
-    nb.add_space_charge(pos, ch, replace=True)
-    s2 = nb.solve()
-    b2 = orc.rhs(gs, pos.cpu().numpy(), pr.charge_q, mode="f64")
-    res = np.abs(Krows @ s2 - b2) / (np.abs(Krows).sum(axis=1) * np.abs(s2).max())
-    assert res.max() <= 1e-12
+    nb.add_space_charge(pos, ch)
+    sig = nb.solve()
+    b0 = orc.rhs(gs, pr.charge_pos, pr.charge_q, mode="f64")
+    assert np.max(np.abs(nb.get_rhs()[rows] - b0) / np.maximum(np.abs(b0), 1e-6 * np.abs(b0).max())) <= TOL_FAR
+    assert (np.abs(Krows @ sig - b0) / (rowsum * np.abs(sig).max())).max() <= 1e-12
+    assert np.max(np.abs(sig - s)) > 0.0                                   # the charges changed the right-hand side
+    assert pr.meta["steps"] == 10
+    for step in range(pr.meta["steps"]):
+        _, Eq = nb.eval(pos, want_phi=False)                               # E at all 1e6 charges
+        pos_h = pos.cpu().numpy()
+        cidx = np.sort(rs.choice(pr.charge_q.shape[0], 1024, replace=False))
+        tc = torch.from_numpy(cidx).cuda()
+        Eq_s = Eq[:, tc].cpu().numpy()
+        _, E_o, S = truth(orc, g, sig, pos_h[:, cidx], pos_h, pr.charge_q, mode="f64")
+        check_field(None, Eq_s, None, E_o, TOL_FAR, f"C4 step {step} E at 1024 charges", S, c_sum=C_SUM_F64)
+        if step in (0, pr.meta["steps"] - 1):
+            _, E_l, Sl = truth(orc, g, sig, pos_h[:, cidx[:64]], pos_h, pr.charge_q, mode="ld")
+            check_field(None, Eq_s[:, :64], None, E_l, TOL_FAR, f"C4 step {step} E at 64 charges (ld)", Sl)
+        nb.push(pos, Eq, mu_dt)
+        pos_o = orc.push(pos_h[:, cidx], E_o, pr.meta["mu"], pr.meta["dt"])
+        assert np.max(np.abs(pos[:, tc].cpu().numpy() - pos_o)) <= 1e-12 * np.max(np.abs(pos_o)), step
+        nb.add_space_charge(pos, ch, replace=True)
+        sig_new = nb.solve()
+        bk = orc.rhs(gs, pos.cpu().numpy(), pr.charge_q, mode="f64")
+        assert np.max(np.abs(nb.get_rhs()[rows] - bk) / np.maximum(np.abs(bk), 1e-6 * np.abs(bk).max())) <= TOL_FAR, step
+        assert (np.abs(Krows @ sig_new - bk) / (rowsum * np.abs(sig_new).max())).max() <= 1e-12, step
+        assert np.max(np.abs(sig_new - sig)) > 0.0, step
+        sig = sig_new
 
 
 # ---------------------------------------------------------------------------------------------
@@ -418,12 +512,15 @@ def test_space_charge_direct_sum(nb, orc):
     pts = np.concatenate([rs.normal(size=(3, 1000)) * 3e-3, pos[:, :50]], axis=1)      # incl. points ON charges
     phi, E = nb.eval(pts)
     phi_o, E_o = orc.point_charges(pts, pos, ch)
-    check_field(phi, E, phi_o, E_o, TOL_FAR, "point charges")
+    S = orc.evaluate_abs(orc.Geometry(pr), np.zeros(pr.n), pts, pos, ch)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "point charges", S)
     # append instead of replace
     nb.add_space_charge(pos[:, :100], ch[:100], replace=False)
     phi2, _ = nb.eval(pts)
-    phi_o2, _ = orc.point_charges(pts, np.concatenate([pos, pos[:, :100]], axis=1), np.concatenate([ch, ch[:100]]))
-    assert rel_err(phi2, phi_o2).max() <= TOL_FAR
+    pos2, ch2 = np.concatenate([pos, pos[:, :100]], axis=1), np.concatenate([ch, ch[:100]])
+    phi_o2, _ = orc.point_charges(pts, pos2, ch2)
+    S2 = orc.evaluate_abs(orc.Geometry(pr), np.zeros(pr.n), pts, pos2, ch2)
+    assert np.all(np.abs(phi2 - phi_o2) <= TOL_FAR * np.abs(phi_o2) + C_SUM * EPS * S2[0])
     nb.add_space_charge(None, None, replace=True)           # q = 0 clears
     phi3, E3 = nb.eval(pts)
     assert np.all(phi3 == 0.0) and np.all(E3 == 0.0)
@@ -465,8 +562,9 @@ def test_c4_dynamic_loop_reduced(nb, orc):
     so = lu.solve(orc.rhs(g, pos_o, pr.charge_q))
     for step in range(3):
         _, E = nb.eval(pos, want_phi=False)
-        _, E_o = orc.evaluate(g, so, pos_o, pos_o, pr.charge_q)
-        assert vec_rel_err(E.cpu().numpy(), E_o).max() <= 1e-8, step
+        _, E_o, S = truth(orc, g, so, pos_o, pos_o, pr.charge_q)
+        # the two loops run on their own sigma and positions from step to step: differences of 1e-9 in sigma compound
+        check_field(None, E.cpu().numpy(), None, E_o, 1e-8, f"C4 reduced step {step}", S)
         nb.push(pos, E, mu_dt)
         pos_o = orc.push(pos_o, E_o, mu_dt, 1.0)
         nb.add_space_charge(pos, ch, replace=True)
@@ -497,8 +595,8 @@ def test_fastvol_build_and_lookup(nb, orc, P):
     for slot, with_q in ((0, True), (2, False)):
         nb.fastvol_build(slot, shape, o, h, with_charges=with_q)
         vals = nb.fastvol_get(slot)
-        ph_o, E_o = orc.evaluate(g, s, nodes, pr.charge_pos if with_q else None, pr.charge_q if with_q else None)
-        check_field(vals[0], vals[1:], ph_o, E_o, TOL_FAR, f"fastvol nodes slot {slot}")
+        ph_o, E_o, S = truth(orc, g, s, nodes, pr.charge_pos if with_q else None, pr.charge_q if with_q else None)
+        check_field(vals[0], vals[1:], ph_o, E_o, TOL_FAR, f"fastvol nodes slot {slot}", S)
         ext = h * (np.array(shape) - 1)
         pts = o[:, None] + rs.rand(3, 3001) * ext[:, None]
         pts[:, :40] = nodes[:, rs.choice(nodes.shape[1], 40)]              # exactly on nodes (faces included)
@@ -550,14 +648,14 @@ def test_weighting_solve_and_map(nb, orc):
     assert np.max(np.abs(sw + nb.solve_weighting(rest) - s_all)) <= 1e-12 * np.max(np.abs(s_all))
     assert np.array_equal(nb.get_rhs(), b)                                 # untouched by the weighting solves
     phi0, _ = nb.eval(pr.points)
-    phi_o, _ = orc.evaluate(g, s, pr.points)
-    assert rel_err(phi0, phi_o).max() <= TOL_FAR                           # still the physical sigma
+    phi_o, _, S0 = truth(orc, g, s, pr.points)
+    assert np.all(np.abs(phi0 - phi_o) <= TOL_FAR * np.abs(phi_o) + C_SUM * EPS * S0[0])     # still the physical sigma
     nb.set_sigma(sw)
     shape, o, h = (5, 5, 9), np.array([-0.4e-3, -0.4e-3, 0.5e-3]), np.array([0.2e-3, 0.2e-3, 0.25e-3])
     nb.fastvol_build(1, shape, o, h, with_charges=False)
     vals = nb.fastvol_get(1)
-    ph_w, E_w = orc.evaluate(g, so, orc.fastvol_nodes(*shape, o, h))
-    check_field(vals[0], vals[1:], ph_w, E_w, TOL_FAR, "weighting map")
+    ph_w, E_w, Sw = truth(orc, g, so, orc.fastvol_nodes(*shape, o, h))
+    check_field(vals[0], vals[1:], ph_w, E_w, TOL_FAR, "weighting map", Sw)
     assert 0.0 < vals[0].min() and vals[0].max() < 1.0                     # a weighting potential lies in (0, 1)
     nb.set_sigma(s)
 
@@ -606,7 +704,7 @@ def test_voxelize_space_charge(nb, orc, P):
     check_field(phi2, E2, phi_e + phi_l + phi_p, E_e + E_l + E_p, TOL_FAR, "elements + lines + points")
     nb.add_space_charge(None, None, replace=True)             # clears lines and points
     phi3, E3 = nb.eval(pts)
-    check_field(phi3, E3, phi_e, E_e, TOL_FAR, "elements only")
+    check_field(phi3, E3, phi_e, E_e, TOL_FAR, "elements only", orc.evaluate_abs(g, s, pts))
     with pytest.raises(P.NebError) as e:
         nb.voxelize_space_charge(o, d, dims)                  # nothing to voxelise
     assert e.value.status == 3
@@ -614,6 +712,25 @@ def test_voxelize_space_charge(nb, orc, P):
     with pytest.raises(P.NebError) as e:
         nb.voxelize_space_charge(o, np.array([1e-4, 0.0, 1e-4]), dims)
     assert e.value.status == 1
+    # bit-reproducible totals (fixed-point accumulation, no fp64 atomics): the same cloud twice, in reversed order too
+    nb.voxelize_space_charge(o, d, dims)
+    lam1 = nb.get_line_charges()[4]
+    nb.add_space_charge(pos[:, ::-1].copy(), ch[::-1].copy())
+    nb.voxelize_space_charge(o, d, dims)
+    assert np.array_equal(nb.get_line_charges()[4], lam1)
+    # a second voxelisation folds the earlier lines in (each as its total charge at its centre) with the points added
+    # since, on another grid: the total charge is conserved (the old lines used to be dropped)
+    nb.add_space_charge(extra_pos, extra_q, replace=False)
+    o2, d2, dims2 = np.array([-3e-4, -3e-4, 0.5e-3]), np.array([1e-4, 1.5e-4, 2e-4]), np.array([6, 4, 7])
+    nl2 = nb.voxelize_space_charge(o2, d2, dims2)
+    lines2 = nb.get_line_charges()
+    centres = np.stack([lines_o[0], lines_o[1], 0.5 * (lines_o[2] + lines_o[3])])
+    lines2_o = orc.voxelize(np.concatenate([extra_pos, centres], axis=1),
+                            np.concatenate([extra_q, lines_o[4] * (lines_o[3] - lines_o[2])]), o2, d2, dims2)
+    assert nl2 == lines2_o.shape[1] and np.array_equal(lines2[:4], lines2_o[:4])
+    assert np.max(np.abs(lines2[4] - lines2_o[4])) <= 1e-12 * np.max(np.abs(lines2_o[4]))
+    total = np.sum(lines2[4] * (lines2[3] - lines2[2]))
+    assert abs(total - (ch.sum() + extra_q.sum())) <= 1e-12 * (np.abs(ch).sum() + extra_q.sum())
 
 
 # ---------------------------------------------------------------------------------------------
@@ -629,13 +746,14 @@ def test_adaptive_modelling(nb, orc):
     K = nb.get_matrix()
     s = nb.solve()
     phi_x, E_x = nb.eval(pr.points)
+    S_x = orc.evaluate_abs(g, s, pr.points)      # scale: a far copy's point charge has the magnitude of its exact term
     # simplify the outer ring / every shifted copy (the latter puts simplified copies 0.5 mm from points at the cell's edge)
     for far_mm, n_far, lim_phi, lim_E in ((1.5, 16, 1e-2, 2e-2), (0.9, 24, 5e-2, 2e-1)):
         assert np.sum(np.linalg.norm(pr.img_shift, axis=0) >= far_mm * 1e-3) == n_far
         nb.set_adaptive(far_mm * 1e-3)
         phi_a, E_a = nb.eval(pr.points)
         phi_o, E_o = orc.evaluate_adaptive(g, s, pr.points, far_mm * 1e-3)
-        check_field(phi_a, E_a, phi_o, E_o, TOL_FAR, f"adaptive {far_mm}")
+        check_field(phi_a, E_a, phi_o, E_o, TOL_FAR, f"adaptive {far_mm}", S_x)
         err_phi = np.max(np.abs(phi_a - phi_x)) / np.max(np.abs(phi_x))
         err_E = np.max(np.linalg.norm(E_a - E_x, axis=0)) / np.max(np.linalg.norm(E_x, axis=0))
         # this reduced mesh has 0.1 mm panels against a 1 mm pitch: (L/r)^2 ~ 1e-2 per far copy; at C3's 1/70 mm
@@ -657,7 +775,7 @@ def test_adaptive_modelling(nb, orc):
     nb.set_adaptive(0.5e-3)
     phi_a, E_a = nb.eval(pr2.points)
     phi_o, E_o = orc.evaluate_adaptive(g2, sig, pr2.points, 0.5e-3)
-    check_field(phi_a, E_a, phi_o, E_o, TOL_FAR, "adaptive, general path")
+    check_field(phi_a, E_a, phi_o, E_o, TOL_FAR, "adaptive, general path", orc.evaluate_abs(g2, sig, pr2.points))
     nb.set_adaptive(0.0)
 
 
@@ -687,6 +805,11 @@ def test_edge_cases_and_errors(nb, P, orc):
     assert e.value.status == 1                               # NEB_EINVAL
     bad = W.plate(n_side=2)
     bad.e1[:, 2] = 0.0
+    with pytest.raises(P.NebError) as e:
+        nb.assemble_problem(bad)
+    assert e.value.status == 1
+    bad = W.plate(n_side=2)                                  # skewed (non-perpendicular) edges are rejected, not evaluated
+    bad.e2[:, 1] += 0.05 * bad.e1[:, 1]
     with pytest.raises(P.NebError) as e:
         nb.assemble_problem(bad)
     assert e.value.status == 1

@@ -674,6 +674,11 @@ def test_eval_abs_is_the_sum_of_term_magnitudes(orc):
         we += orc.K_COULOMB * abs(ch[k]) / r ** 2
     assert np.max(np.abs(sp / wp - 1)) < 1e-13 and np.max(np.abs(se / we - 1)) < 1e-13
     phi, E = orc.evaluate(g, sig, pr.points, pos, ch)
+    for mode in ("ld", "f64"):                                         # the one-pass variant returns evaluate()'s own sums
+        sp2, se2, phi2, E2 = orc.evaluate_abs(g, sig, pr.points, pos, ch, mode=mode, with_field=True)
+        phi_m, E_m = orc.evaluate(g, sig, pr.points, pos, ch, mode=mode)
+        assert np.array_equal(phi2, phi_m) and np.array_equal(E2, E_m)
+        assert np.array_equal(sp2, orc.evaluate_abs(g, sig, pr.points, pos, ch, mode=mode)[0])
     assert np.all(sp >= np.abs(phi)) and np.all(se >= np.linalg.norm(E, axis=0) * (1 - 1e-15))
     phi1, _ = orc.evaluate(g, np.abs(sig), pr.points, pos, np.abs(ch))
     flat = np.abs(pr.kind) >= 0
