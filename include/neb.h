@@ -137,6 +137,10 @@ neb_status neb_set_adaptive(neb_ctx* ctx, double far_distance);
  * caller's element order.  Leaves the context's own sigma and right-hand side untouched.
  * Errors: NEB_ESTATE before the first neb_solve (no factors yet). */
 neb_status neb_solve_weighting(neb_ctx* ctx, const double* bc_value_w, double* sigma_w_out);
+/* The same for n_rhs read-out electrodes at once ("the same inverted matrix ... can be reused"): bc_value_w
+ * and sigma_w_out hold n_rhs rows of n values (row k = electrode k).  The triangular solves take up to 8 right-hand
+ * sides per pass over the factors, so that 8 electrodes cost one reading of the 8 n^2 bytes of L and U, not eight. */
+neb_status neb_solve_weighting_multi(neb_ctx* ctx, int32_t n_rhs, const double* bc_value_w, double* sigma_w_out);
 
 /* FastVolume (P:179, P:222 CreateFastVolPF; reading S25).  neb_fastvol_build precomputes Phi and E, from
  * the context's current sigma (all elements with their periodic copies) and, if with_charges != 0, the

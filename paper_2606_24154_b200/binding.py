@@ -54,6 +54,7 @@ def lib():
         L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
         L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
         L.neb_solve_weighting.argtypes = [vp, vp, vp]
+        L.neb_solve_weighting_multi.argtypes = [vp, i32, vp, vp]
         L.neb_set_adaptive.argtypes = [vp, dbl]
         L.neb_voxelize_space_charge.argtypes = [vp, vp, vp, vp, C.POINTER(i64)]
         L.neb_get_line_charges.argtypes = [vp, vp]
@@ -208,6 +209,15 @@ class Neb:
         if out is None:
             out = np.empty(self.n)
         self._ck(self._L.neb_solve_weighting(self._h, _ptr(bc_value_w), _ptr(out)))
+        return out
+
+    def solve_weighting_multi(self, bc_values_w, out=None):
+        """neb_solve_weighting_multi: bc_values_w (n_rhs, n) -> sigma_w (n_rhs, n), one pass per 8 electrodes."""
+        n_rhs = int(bc_values_w.shape[0])
+        bc_values_w = _check_arr(bc_values_w, np.float64, "float64", n_rhs * self.n, "bc_values_w")
+        if out is None:
+            out = np.empty((n_rhs, self.n))
+        self._ck(self._L.neb_solve_weighting_multi(self._h, n_rhs, _ptr(bc_values_w), _ptr(out)))
         return out
 
     def fastvol_build(self, slot: int, shape, origin, spacing, with_charges: bool = True):

@@ -437,7 +437,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaMalloc((void**)&c->d_ipiv, sizeof(int32_t) * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_rowperm, sizeof(int32_t) * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_b, sizeof(double) * npad));
-    NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * 2 * npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * 16 * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_dinv, sizeof(double) * 2 * (npad / 64) * 4096));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
@@ -543,7 +543,7 @@ neb_status neb_solve(neb_ctx* c, double* sigma_out) {
     }
   }
   NEB_TRY(form_rhs(c));
-  NEB_TRY(lu_solve(c));
+  NEB_TRY(lu_solve(c, c->d_b, 1, c->d_x));
   finish_sigma_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->stride, c->d_perm, c->d_x, c->d_rec, c->d_sigma);
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());
@@ -595,17 +595,21 @@ neb_status neb_set_adaptive(neb_ctx* c, double far_distance) {
   return NEB_OK;
 }
 
-neb_status neb_solve_weighting(neb_ctx* c, const double* bc_value_w, double* sigma_w_out) {
-  if (!c || !bc_value_w || !sigma_w_out) return NEB_EINVAL;
+neb_status neb_solve_weighting_multi(neb_ctx* c, int32_t n_rhs, const double* bc_value_w, double* sigma_w_out) {
+  if (!c || n_rhs < 1 || !bc_value_w || !sigma_w_out) return NEB_EINVAL;
   if (!c->factored || !c->assembled) return fail(c, NEB_ESTATE, "neb_solve_weighting before the first neb_solve (no LU factors)");
   NEB_CUDA(c, cudaSetDevice(c->device));
   Staging sg(c);
   const void* dw;
   void* dout;
-  NEB_TRY(sg.in(bc_value_w, sizeof(double) * c->n, &dw));
-  NEB_TRY(sg.out(sigma_w_out, sizeof(double) * c->n, &dout));
-  NEB_TRY(solve_weighting(c, (const double*)dw, (double*)dout));
+  NEB_TRY(sg.in(bc_value_w, sizeof(double) * (size_t)n_rhs * c->n, &dw));
+  NEB_TRY(sg.out(sigma_w_out, sizeof(double) * (size_t)n_rhs * c->n, &dout));
+  NEB_TRY(solve_weighting(c, n_rhs, (const double*)dw, (double*)dout));
   return sg.finish();
+}
+
+neb_status neb_solve_weighting(neb_ctx* c, const double* bc_value_w, double* sigma_w_out) {
+  return neb_solve_weighting_multi(c, 1, bc_value_w, sigma_w_out);
 }
 
 neb_status neb_fastvol_build(neb_ctx* c, int32_t slot, int32_t nx, int32_t ny, int32_t nz, const double* origin,

@@ -80,17 +80,22 @@ __global__ void __launch_bounds__(256) fastvol_eval_kernel(FastVol fv, int64_t m
   if (E) { E[p] = r.y; E[m + p] = r.z; E[2 * m + p] = r.w; }
 }
 
-// weighting right-hand side in the sorted order (reading S26)
-__global__ void weighting_rhs_kernel(int64_t n, int64_t npad, const int32_t* __restrict__ perm, const int32_t* __restrict__ bc_kind,
+// weighting right-hand sides in the sorted order (reading S26): b[k * npad + s], k < nrhs
+__global__ void weighting_rhs_kernel(int64_t n, int64_t npad, int nrhs, const int32_t* __restrict__ perm, const int32_t* __restrict__ bc_kind,
                                      const double* __restrict__ w_caller, double* __restrict__ b) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= npad) return;
-  b[s] = (s < n && bc_kind[s] == NEB_BC_DIRICHLET) ? w_caller[perm[s]] : 0.0;
+  const bool use = s < n && bc_kind[s] == NEB_BC_DIRICHLET;
+  const int64_t j = use ? perm[s] : 0;
+  for (int k = 0; k < nrhs; ++k) b[k * npad + s] = use ? w_caller[k * n + j] : 0.0;
 }
 
-__global__ void unpermute_kernel(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ x, double* __restrict__ out) {
+__global__ void unpermute_multi_kernel(int64_t n, int64_t npad, int nrhs, const int32_t* __restrict__ perm, const double* __restrict__ x,
+                                       double* __restrict__ out) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s < n) out[perm[s]] = x[s];
+  if (s >= n) return;
+  const int64_t j = perm[s];
+  for (int k = 0; k < nrhs; ++k) out[k * n + j] = x[k * npad + s];
 }
 
 neb_status fastvol_build(neb_ctx* c, int slot, int nx, int ny, int nz, const double* o, const double* h, bool with_charges) {
@@ -145,22 +150,21 @@ neb_status fastvol_get(neb_ctx* c, int slot, double* d_values) {
   return NEB_OK;
 }
 
-neb_status solve_weighting(neb_ctx* c, const double* d_w_caller, double* d_sigma_out) {
+neb_status solve_weighting(neb_ctx* c, int nrhs, const double* d_w_caller, double* d_sigma_out) {
   const int64_t n = c->n, npad = c->npad;
-  // the physical right-hand side (neb_get_rhs) and sigma stay as they are: the solve runs on a temporary b
-  double* tmp = nullptr;
-  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tmp, sizeof(double) * (size_t)npad, c->pool, c->stream));
-  weighting_rhs_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(n, npad, c->d_perm, c->d_bc_kind, d_w_caller, tmp);
+  // the physical right-hand side (neb_get_rhs) and sigma stay as they are: the solve runs on temporaries
+  double *tb = nullptr, *tx = nullptr;
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tb, sizeof(double) * (size_t)nrhs * npad, c->pool, c->stream));
+  NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tx, sizeof(double) * (size_t)nrhs * npad, c->pool, c->stream));
+  weighting_rhs_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(n, npad, nrhs, c->d_perm, c->d_bc_kind, d_w_caller, tb);
   c->launches++;
-  double* saved = c->d_b;
-  c->d_b = tmp;
-  neb_status st = lu_solve(c);
-  c->d_b = saved;
+  neb_status st = lu_solve(c, tb, nrhs, tx);
   if (st == NEB_OK) {
-    unpermute_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, c->d_perm, c->d_x, d_sigma_out);
+    unpermute_multi_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, npad, nrhs, c->d_perm, tx, d_sigma_out);
     c->launches++;
   }
-  cudaFreeAsync(tmp, c->stream);
+  cudaFreeAsync(tb, c->stream);
+  cudaFreeAsync(tx, c->stream);
   if (st == NEB_OK) NEB_CUDA(c, cudaGetLastError());
   return st;
 }

@@ -75,7 +75,7 @@ struct neb_ctx {
   int32_t* d_ipiv = nullptr;      // npad (0-based absolute row)
   int32_t* d_rowperm = nullptr;   // npad: composed row permutation of the factorisation
   double* d_b = nullptr;          // npad, unscaled RHS (sorted order)
-  double* d_x = nullptr;          // 2 * npad: running right-hand side + solved blocks
+  double* d_x = nullptr;          // 16 * npad: running values and solved values of up to 8 right-hand sides (neb_trisolve.cu)
   double* d_dinv = nullptr;       // inverses of the 64x64 diagonal blocks of L and U: 2 * (npad/64) * 4096
   double* d_sigma = nullptr;      // n, caller order
   void* d_panel_ws = nullptr;     // LU panel exchange buffers
@@ -138,7 +138,9 @@ neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
 // neb_lu.cu ---------------------------------------------------------------------------------------
 neb_status lu_init_device(neb_ctx* c);    // per-device kernel attributes (dynamic shared memory, cluster size); from neb_create
 neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-scaled)
-neb_status lu_solve(neb_ctx* c);          // a6: d_x <- solution of (scaled) system for RHS d_b
+// neb_trisolve.cu: a6, nrhs right-hand sides d_b[k * npad + i] (unscaled, sorted order) -> d_out[k * npad + i]
+neb_status lu_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
+neb_status trisolve_init_device(neb_ctx* c);
 size_t lu_panel_ws_bytes(int num_sms);
 
 // neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
@@ -150,7 +152,7 @@ neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream);
 neb_status fastvol_build(neb_ctx* c, int slot, int nx, int ny, int nz, const double* origin, const double* spacing, bool with_charges);
 neb_status fastvol_eval(neb_ctx* c, int slot, int64_t m, const double* d_pts, double* d_phi, double* d_E);
 neb_status fastvol_get(neb_ctx* c, int slot, double* d_values);
-neb_status solve_weighting(neb_ctx* c, const double* d_w_caller, double* d_sigma_out);
+neb_status solve_weighting(neb_ctx* c, int nrhs, const double* d_w_caller, double* d_sigma_out);
 
 // neb_voxel.cu -----------------------------------------------------------------------------------
 neb_status voxelize_charges(neb_ctx* c, const double* origin, const double* voxel, const int32_t* dims, int64_t* n_lines_out);

@@ -394,12 +394,6 @@ __global__ void compose_perm_global_kernel(const int32_t* __restrict__ ipiv, int
   }
 }
 
-__global__ void permute_scale_kernel(const double* __restrict__ b, const double* __restrict__ rscale,
-                                     const int32_t* __restrict__ rowperm, int64_t npad, double* __restrict__ x) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < npad) { int p = rowperm[i]; x[i] = b[p] * rscale[p]; }
-}
-
 // Inverses of the 64x64 diagonal blocks of L (unit lower) and U (upper), once per factorisation, so that a
 // solve step is a matrix-vector product instead of a 64-step substitution.  grid = (nblocks, 2), 64 threads;
 // thread c computes column c of the inverse by substitution.  dinv[(which * nblk + blk) * 4096 + i + 64 j].
@@ -429,59 +423,6 @@ __global__ void __launch_bounds__(NB) diag_inv_kernel(const double* __restrict__
   for (int j = 0; j < NB; ++j) out[c + NB * j] = sXc[c][j];
 }
 
-// One block step of a triangular solve, ONE launch: every CTA first forms x_B = Dinv_B * x[kb..kb+64)
-// (a 64x64 matrix-vector product, recomputed per CTA: 32 KB from L2) and then updates its 64 rows,
-// x[i] -= A[i, kb..kb+64) . x_B.  CTA 0 also stores x_B.  256 threads = 64 rows x 4 column groups of 16.
-// rows to update: [r_lo, r_hi); grid.x = ceil((r_hi - r_lo) / 64), at least 1.
-__global__ void __launch_bounds__(256) tri_step_kernel(const double* __restrict__ A, int64_t ld, const double* __restrict__ dinv_blk,
-                                                       int64_t kb, int64_t r_lo, int64_t r_hi, double* x) {
-  __shared__ double s_part[4][NB];
-  __shared__ double s_xb[NB];
-  const int tid = threadIdx.x, r = tid & (NB - 1), g = tid >> 6;
-  {
-    double acc = 0.0;
-#pragma unroll 4
-    for (int jj = 0; jj < 16; ++jj) {
-      const int j = g * 16 + jj;
-      acc = fma(dinv_blk[r + NB * j], x[kb + j], acc);
-    }
-    s_part[g][r] = acc;
-  }
-  __syncthreads();
-  if (tid < NB) s_xb[tid] = (s_part[0][tid] + s_part[1][tid]) + (s_part[2][tid] + s_part[3][tid]);
-  __syncthreads();
-  const int64_t i = r_lo + (int64_t)blockIdx.x * NB + r;
-  double acc = 0.0;
-  if (i < r_hi) {
-    const double* a = A + i + (kb + g * 16) * ld;
-    double a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-#pragma unroll
-    for (int jj = 0; jj < 16; jj += 4) {
-      a0 = fma(a[(jj + 0) * ld], s_xb[g * 16 + jj + 0], a0);
-      a1 = fma(a[(jj + 1) * ld], s_xb[g * 16 + jj + 1], a1);
-      a2 = fma(a[(jj + 2) * ld], s_xb[g * 16 + jj + 2], a2);
-      a3 = fma(a[(jj + 3) * ld], s_xb[g * 16 + jj + 3], a3);
-    }
-    acc = (a0 + a1) + (a2 + a3);
-  }
-  __syncthreads();               // s_part is reused; everyone has read it
-  s_part[g][r] = acc;
-  __syncthreads();
-  if (tid < NB) {
-    const int64_t ii = r_lo + (int64_t)blockIdx.x * NB + tid;
-    if (ii < r_hi) x[ii] -= (s_part[0][tid] + s_part[1][tid]) + (s_part[2][tid] + s_part[3][tid]);
-  }
-  // the block's own solution: written last, by CTA 0 only; no CTA of this launch reads x[kb..kb+64) after
-  // its first barrier... but other CTAs may still be reading it: CTA 0 therefore writes to a staging slot
-  if (blockIdx.x == 0 && tid < NB) x[ld + kb + tid] = s_xb[tid];
-}
-
-// x[0..npad) <- staging copy x[npad..2 npad) (the solved blocks)
-__global__ void tri_finish_kernel(int64_t npad, double* x) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < npad) x[i] = x[npad + i];
-}
-
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
@@ -493,7 +434,7 @@ neb_status lu_init_device(neb_ctx* c) {
   NEB_CUDA(c, cudaFuncSetAttribute(diag_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * NB * (NB + 1) * sizeof(double))));
   NEB_CUDA(c, cudaFuncSetAttribute(compose_perm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   c->cluster_max_ctas = panel_cluster_probe();
-  return NEB_OK;
+  return trisolve_init_device(c);
 }
 
 neb_status lu_factor(neb_ctx* c) {
@@ -620,32 +561,6 @@ neb_status lu_factor(neb_ctx* c) {
     diag_inv_kernel<<<dim3(nblk, 2), NB, 2 * NB * (NB + 1) * sizeof(double), c->stream>>>(c->d_K, ld, c->d_dinv, nblk);
     c->launches++;
   }
-  NEB_CUDA(c, cudaGetLastError());
-  return NEB_OK;
-}
-
-neb_status lu_solve(neb_ctx* c) {
-  const int64_t npad = c->npad, ld = c->npad;
-  StageTimer tt(c, NEB_STAGE_TRISOLVE);
-  permute_scale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(c->d_b, c->d_rscale, c->d_rowperm, npad, c->d_x);
-  c->launches++;
-  // d_x holds two vectors: [0, npad) the running right-hand side, [npad, 2 npad) the solved blocks
-  const int nblk = (int)(npad / NB);
-  for (int64_t kb = 0; kb < npad; kb += NB) {          // forward: L y = P b
-    const int64_t lo = kb + NB;
-    const unsigned grid = (unsigned)max((int64_t)1, (npad - lo + NB - 1) / NB);
-    tri_step_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, ld, c->d_dinv + (kb / NB) * (NB * NB), kb, lo, npad, c->d_x);
-    c->launches++;
-  }
-  tri_finish_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(npad, c->d_x);
-  c->launches++;
-  for (int64_t kb = npad - NB; kb >= 0; kb -= NB) {    // backward: U x = y
-    const unsigned grid = (unsigned)max((int64_t)1, (kb + NB - 1) / NB);
-    tri_step_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, ld, c->d_dinv + ((int64_t)nblk + kb / NB) * (NB * NB), kb, 0, kb, c->d_x);
-    c->launches++;
-  }
-  tri_finish_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(npad, c->d_x);
-  c->launches++;
   NEB_CUDA(c, cudaGetLastError());
   return NEB_OK;
 }

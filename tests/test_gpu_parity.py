@@ -660,6 +660,29 @@ def test_weighting_solve_and_map(nb, orc):
     nb.set_sigma(s)
 
 
+def test_weighting_solve_multi_rhs(nb, orc):
+    """neb_solve_weighting_multi (the same factors serve every read-out electrode): 11 electrodes at once
+    (two passes of the triangular solves: 8 + 3 right-hand sides) against the oracle's solve of each weighting
+    right-hand side, and bit-equal to eleven single solves."""
+    pr = W.thgem(d=10, n_plane=8, n_grid=4)
+    g = orc.Geometry(pr)
+    lu = orc.LU(orc.assemble(g))
+    nb.assemble_problem(pr)
+    s = nb.solve()
+    cond = pr.bc_kind == W.DIRICHLET
+    rs = np.random.RandomState(5)
+    groups = rs.randint(0, 11, size=pr.n)                    # a partition of the conductor panels into 11 electrodes
+    Wm = np.stack([((groups == k) & cond).astype(float) for k in range(11)])
+    S = nb.solve_weighting_multi(Wm)
+    assert S.shape == (11, pr.n)
+    for k in range(11):
+        so = lu.solve(orc.weighting_rhs(g, Wm[k]))
+        assert np.max(np.abs(S[k] - so)) <= TOL_SIGMA * np.max(np.abs(so)), k
+        assert np.array_equal(S[k], nb.solve_weighting(Wm[k])), k
+    assert np.max(np.abs(S.sum(axis=0) - nb.solve_weighting(cond.astype(float)))) <= 1e-12 * np.max(np.abs(S))
+    assert np.array_equal(nb.solve(), s)                     # the physical solve is untouched
+
+
 # ---------------------------------------------------------------------------------------------
 # SURVEY 8(f) item 2: Alg. 3, voxelisation of the point charges into line charges
 # ---------------------------------------------------------------------------------------------
