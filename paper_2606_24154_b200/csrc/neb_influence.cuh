@@ -94,10 +94,12 @@ __device__ __forceinline__ void rect_local(double a, double b, double ab, double
   }
   // solid angle: two fan triangles (c11,c21,c22), (c11,c22,c12); tan(Omega_t/2) = 2A_t |d| / D_t with the
   // triple product written as area x height (exact for a flat element: no far-field cancellation)
-  double p = u1 * u2, q = w1 * w2;
-  double d1122 = p + yy + q;
-  double D1 = fma(r11 * r21, r22, fma(p + B1, r22, fma(d1122, r21, (A2 + q) * r11)));
-  double D2 = fma(r11 * r22, r12, fma(d1122, r12, fma(A1 + q, r22, (p + B2) * r11)));
+  // (products folded into the sums that use them: 14 FP64-pipe operations for D1, D2 instead of 18)
+  double d1122 = fma(u1, u2, fma(w1, w2, yy));               // r11 . r22 = r12 . r21
+  double pB1 = fma(u1, u2, B1), pB2 = fma(u1, u2, B2);       // r11 . r21, r12 . r22
+  double A2q = fma(w1, w2, A2), A1q = fma(w1, w2, A1);       // r21 . r22, r11 . r12
+  double D1 = fma(fma(r11, r21, pB1), r22, fma(d1122, r21, A2q * r11));
+  double D2 = fma(fma(r11, r22, d1122), r12, fma(A1q, r22, pB2 * r11));
   double Nn = ab * y;
   if (far) om = 2.0 * M::far_atan2(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));
   else om = 2.0 * M::atan2_pos(Nn * (D1 + D2), fma(D1, D2, -Nn * Nn));

@@ -47,6 +47,24 @@ __device__ __forceinline__ double clamp_tiny(double x) {
   return __hiloint2double(max(__double2hiint(x), 0x01a56e1f), __double2loint(x));
 }
 
+// x / 2 for a normal x well inside the exponent range (here: 1/sqrt of a length squared): one integer subtraction on
+// the high word instead of a DMUL on the FP64 pipe
+__device__ __forceinline__ double half_of(double x) {
+  return __hiloint2double(__double2hiint(x) - 0x00100000, __double2loint(x));
+}
+
+// 1/sqrt(x) for x > 0 (the caller clamps and handles x = 0): MUFU.RSQ64H seed (2^-23) + ONE cubic step
+//   e = 1 - x y^2,  y <- y (1 + e/2 + 3 e^2 / 8)      (relative error ~ e^3 = 2^-69 before rounding): 5 FP64-pipe ops
+__device__ __forceinline__ double rsqrt_pos(double x) {
+  const double y = mufu_rsqrt(x);
+  const double e = fma(-x * y, y, 1.0);
+  const double p = fma(0.375, e, 0.5);
+  return fma(y * e, p, y);
+}
+
+// x == 0 (either sign) by integer operations on the bit pattern
+__device__ __forceinline__ bool is_zero(double x) { return (((__double2hiint(x) & 0x7fffffff) | __double2loint(x)) == 0); }
+
 struct MathLib {
   static constexpr bool kNeedsFar = true;    // libm path: far field through log1p
   static constexpr bool kFarPath = false;    // no warp-uniform far-field shortcut: this policy is the plain reference
@@ -68,10 +86,11 @@ struct MathFast {
   static constexpr bool kNeedsFar = false;   // z = L/s whenever the exponent fold is zero
   static constexpr bool kFarPath = true;     // warp-uniform shortcut when every lane is >= 2.5 edge lengths away
   // sqrt(x), x >= 0 finite (x = 0 -> 0).  One coupled Newton step on (g ~ sqrt x, h ~ 1/(2 sqrt x))
-  // from the 2^-23 seed, then one residual correction: 6 DFMA-class ops + 1 integer clamp + 1 MUFU.
+  // from the 2^-23 seed, then one residual correction: 5 FP64-pipe ops (the halving is an integer
+  // subtraction on the exponent) + 1 integer clamp + 1 MUFU.
   static __device__ __forceinline__ double sqrt_nn(double x) {
     double y = mufu_rsqrt(clamp_tiny(x));
-    double g = x * y, h = 0.5 * y;
+    double g = x * y, h = half_of(y);
     double r = fma(-g, h, 0.5);
     g = fma(g, r, g);                 // relative error ~2^-45
     double d = fma(-g, g, x);         // residual; the seed-accurate h is enough for the correction term
