@@ -54,6 +54,10 @@ enum {
   NEB_OPT_PROFILE = 2,  /* 1: record per-stage CUDA-event timings (neb_stage_ms); default 0      */
   NEB_OPT_LU_PANEL = 3, /* 0 (default): cluster/DSMEM panel kernel where the panel fits (<= 8192 rows),
                            grid-wide cooperative kernel above; 1: grid-wide kernel only          */
+  NEB_OPT_EVAL_SPLITS = 5, /* 0 (default): neb_eval splits the elements / charges into as many chunks as fill the GPU for
+                           the given number of points (few points -> many chunks); k > 0: always k chunks, so that the
+                           fixed-order partial sums, hence the result BITS, do not depend on how many points a call
+                           (or a rank of a sharded evaluation) is given                                          */
   NEB_OPT_LU_LOOKAHEAD = 4 /* 1 (default): panel k+1 is factored on an internal stream while the trailing
                            update of panel k runs (cluster panels only); 0: one stream, and
                            NEB_STAGE_LU_GEMM is then timed alone                                 */
@@ -210,6 +214,12 @@ neb_status neb_fp64_peak(neb_ctx* ctx, int32_t kind, double* tflops);
  * neb_reset_stats; valid when NEB_OPT_PROFILE is 1.  neb_launch_count counts every kernel this
  * library launched on the context since creation (profiling on or off). */
 neb_status neb_stage_ms(neb_ctx* ctx, int32_t stage, double* ms, int64_t* launches);
+/* Work counters of the LAST factorisation / assembly, counted by the host code that issues the launches (exact):
+ * NEB_COUNTER_GEMM_FLOP   flop of the DMMA trailing updates (2 m n k summed over the gemm_kernel launches);
+ * NEB_COUNTER_LU_FLOP     2/3 npad^3, the whole factorisation of the padded matrix;
+ * NEB_COUNTER_MATRIX_BYTES bytes of matrix the assembly kernel wrote (8 n npad). */
+enum { NEB_COUNTER_GEMM_FLOP = 0, NEB_COUNTER_LU_FLOP = 1, NEB_COUNTER_MATRIX_BYTES = 2, NEB_COUNTER_COUNT = 3 };
+neb_status neb_get_counter(neb_ctx* ctx, int32_t which, double* value);
 neb_status neb_reset_stats(neb_ctx* ctx);
 int64_t neb_launch_count(const neb_ctx* ctx);
 

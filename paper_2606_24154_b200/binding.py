@@ -9,7 +9,7 @@ from . import build as _build
 
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
-NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD = 0, 1, 2, 3, 4
+NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS = 0, 1, 2, 3, 4, 5
 STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
 
@@ -67,6 +67,7 @@ def lib():
         L.neb_get_rhs.argtypes = [vp, vp]
         L.neb_fp64_peak.argtypes = [vp, i32, C.POINTER(dbl)]
         L.neb_stage_ms.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(i64)]
+        L.neb_get_counter.argtypes = [vp, i32, C.POINTER(dbl)]
         L.neb_reset_stats.argtypes = [vp]
         L.neb_launch_count.argtypes = [vp]
         L.neb_launch_count.restype = i64
@@ -305,6 +306,12 @@ class Neb:
             self._ck(self._L.neb_stage_ms(self._h, s, C.byref(ms), C.byref(ln)))
             out[name] = (ms.value, ln.value)
         return out
+
+    def counter(self, which: int) -> float:
+        """neb_get_counter: 0 = flop of the DMMA trailing updates, 1 = flop of the whole LU, 2 = matrix bytes written."""
+        v = C.c_double(0.0)
+        self._ck(self._L.neb_get_counter(self._h, which, C.byref(v)))
+        return v.value
 
     def reset_stats(self):
         self._ck(self._L.neb_reset_stats(self._h))

@@ -399,6 +399,10 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
     case NEB_OPT_PROFILE: c->profile = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_LU_PANEL: c->panel_mode = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_LU_LOOKAHEAD: c->lu_lookahead = value ? 1 : 0; return NEB_OK;
+    case NEB_OPT_EVAL_SPLITS:
+      if (value < 0 || value > 1024) return fail(c, NEB_EINVAL, "eval splits must be 0 (automatic) .. 1024");
+      c->eval_splits = (int)value;
+      return NEB_OK;
     default: return fail(c, NEB_EINVAL, "unknown option");
   }
 }
@@ -792,6 +796,12 @@ neb_status neb_stage_ms(neb_ctx* c, int32_t stage, double* ms, int64_t* launches
   if (!c || stage < 0 || stage >= NEB_STAGE_COUNT) return NEB_EINVAL;
   if (ms) *ms = c->stat[stage].ms;
   if (launches) *launches = c->stat[stage].launches;
+  return NEB_OK;
+}
+
+neb_status neb_get_counter(neb_ctx* c, int32_t which, double* value) {
+  if (!c || !value || which < 0 || which >= NEB_COUNTER_COUNT) return NEB_EINVAL;
+  *value = c->counter[which];
   return NEB_OK;
 }
 

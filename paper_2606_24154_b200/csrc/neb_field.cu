@@ -417,9 +417,10 @@ __global__ void rhs_kernel(int64_t n, int64_t npad, int64_t stride, const int32_
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-static int pick_splits(int64_t pt_blocks, int64_t units, int64_t unit_tile, int num_sms) {
-  // aim at >= 16 waves of 4 CTAs/SM so the tail wave is small, but keep >= 2 tiles per split
-  int64_t want = (16LL * 4 * num_sms + pt_blocks - 1) / pt_blocks;
+static int pick_splits(int64_t pt_blocks, int64_t units, int64_t unit_tile, int num_sms, int fixed) {
+  // aim at >= 16 waves of 4 CTAs/SM so the tail wave is small, but keep >= 2 tiles per split; NEB_OPT_EVAL_SPLITS
+  // replaces the point-count-dependent wish by a fixed one
+  int64_t want = fixed > 0 ? fixed : (16LL * 4 * num_sms + pt_blocks - 1) / pt_blocks;
   int64_t max_split = (units + 2 * unit_tile - 1) / (2 * unit_tile);
   int64_t s = want < 1 ? 1 : want;
   if (s > max_split) s = max_split;
@@ -440,8 +441,8 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
   const bool use_lines = use_charges && c->n_lines > 0;
   use_charges = use_charges && c->q > 0;
   int64_t pt_blocks = (m + kThreads - 1) / kThreads;
-  int se = use_elements ? pick_splits(pt_blocks, c->n, kTile, c->num_sms) : 0;
-  int sq = use_charges ? pick_splits(pt_blocks, c->q, kChargeTile, c->num_sms) : 0;
+  int se = use_elements ? pick_splits(pt_blocks, c->n, kTile, c->num_sms, c->eval_splits) : 0;
+  int sq = use_charges ? pick_splits(pt_blocks, c->q, kChargeTile, c->num_sms, c->eval_splits) : 0;
   int64_t per_e = 0, per_q = 0;
   if (se) {
     per_e = (c->n + se - 1) / se;
@@ -453,7 +454,7 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
     per_q = (per_q + kChargeTile - 1) / kChargeTile * kChargeTile;
     sq = (int)((c->q + per_q - 1) / per_q);
   }
-  int sl = use_lines ? pick_splits(pt_blocks, c->n_lines, 256, c->num_sms) : 0;
+  int sl = use_lines ? pick_splits(pt_blocks, c->n_lines, 256, c->num_sms, c->eval_splits) : 0;
   int64_t per_l = 0;
   if (sl) {
     per_l = (c->n_lines + sl - 1) / sl;
@@ -504,6 +505,7 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
 
 neb_status assemble_matrix(neb_ctx* c) {
   int64_t n = c->n, npad = c->npad;
+  c->counter[NEB_COUNTER_MATRIX_BYTES] = 8.0 * (double)n * (double)n;
   NEB_TRY(ensure_scratch(c, (size_t)npad * sizeof(unsigned long long)));
   unsigned long long* rowmax = (unsigned long long*)c->d_scratch;
   NEB_CUDA(c, cudaMemsetAsync(rowmax, 0, (size_t)npad * sizeof(unsigned long long), c->stream));

@@ -52,6 +52,7 @@ struct neb_ctx {
   int profile = 0;
   int lu_lookahead = 1; // 1: factor panel k+1 on the side stream while panel k's trailing update runs
   int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
+  int eval_splits = 0;  // 0: element/charge chunks chosen from the point count; k: always k chunks (shard-invariant bits)
 
   // geometry
   int64_t n = 0, npad = 0, stride = 0;
@@ -95,6 +96,7 @@ struct neb_ctx {
   size_t scratch_bytes = 0;
 
   // stats
+  double counter[NEB_COUNTER_COUNT] = {0, 0, 0};
   int64_t launches = 0;
   neb::StageStat stat[NEB_STAGE_COUNT];
   cudaEvent_t ev0[NEB_STAGE_COUNT] = {}, ev1[NEB_STAGE_COUNT] = {};

@@ -440,6 +440,8 @@ neb_status lu_init_device(neb_ctx* c) {
 neb_status lu_factor(neb_ctx* c) {
   const int64_t npad = c->npad, ld = c->npad;
   StageTimer tt(c, NEB_STAGE_LU);
+  c->counter[NEB_COUNTER_GEMM_FLOP] = 0.0;
+  c->counter[NEB_COUNTER_LU_FLOP] = 2.0 / 3.0 * (double)npad * (double)npad * (double)npad;
   PanelWs* ws = (PanelWs*)c->d_panel_ws;
   // panels run on one cluster (neb_lu_panel.cu) whatever their height; NEB_OPT_LU_PANEL = 1 selects the grid-wide
   // cooperative kernel of round 1 instead (all SMs, no look-ahead, n <= 148 x 384 - 128): kept as a cross-check
@@ -479,6 +481,7 @@ neb_status lu_factor(neb_ctx* c) {
   const bool timed = !c->lu_lookahead;
   auto gemm = [&](cudaStream_t st, int64_t k, int K, int64_t r0, int64_t m, int64_t c_first, int64_t ncols) {
     if (m <= 0 || ncols <= 0) return;
+    c->counter[NEB_COUNTER_GEMM_FLOP] += 2.0 * (double)m * (double)ncols * (double)K;
     dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
     if (timed) {
       StageTimer tg(c, NEB_STAGE_LU_GEMM);

@@ -904,3 +904,67 @@ def test_fp64_peaks_and_stats(nb):
     st = nb.stage_ms()
     assert st["assemble"][1] >= 1 and st["lu"][1] >= 4 and st["eval"][1] >= 1 and st["eval"][0] > 0 and st["reduce"][1] >= 1
     assert nb.launch_count() > 10
+
+
+# ---------------------------------------------------------------------------------------------
+# the multi-rank path against the REAL library — two ranks (gloo; both on this one GPU, their kernels never
+# wait on one another: every collective runs on the host) through parallel.eval_sharded and parallel.c4_step_sharded
+# ---------------------------------------------------------------------------------------------
+def _rank_worker(rank, world, port, out_q):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_24154_b200 as P
+    from paper_2606_24154_b200 import parallel
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        pr = W.space_charge(W.double_thgem(d=10, n_plane=10, m_points=1501), q_count=777)
+        pr.charge_q = pr.charge_q * 1e5
+        nb = P.Neb(0)
+        # a fixed number of element / charge chunks: the partial sums, hence the bits, do not depend on the slab size
+        nb.set_option(P.binding.NEB_OPT_EVAL_SPLITS, 6)
+        nb.assemble_problem(pr)
+        pos = torch.from_numpy(pr.charge_pos.copy()).cuda()
+        ch = torch.from_numpy(pr.charge_q).cuda()
+        nb.add_space_charge(pos, ch)
+        nb.solve_resident()
+        pts = torch.from_numpy(pr.points).cuda()
+        phi, E = parallel.eval_sharded(nb, pts, gather=True)           # each rank evaluates its slab of the points
+        phi1, E1 = nb.eval(pts)                                        # the same on one rank
+        ok = torch.equal(phi, phi1) and torch.equal(E, E1)
+        mu_dt = pr.meta["mu"] * pr.meta["dt"] * 1e3
+        pos_s = pos.clone()
+        for _ in range(2):                                             # two sharded steps of the space-charge loop
+            pos_s = parallel.c4_step_sharded(nb, pos_s, ch, mu_dt)
+        sig_s = nb.solve()
+        nb.add_space_charge(pos, ch, replace=True)                     # the same two steps on one rank
+        nb.solve_resident()
+        for _ in range(2):
+            _, Eq = nb.eval(pos, want_phi=False)
+            nb.push(pos, Eq, mu_dt)
+            nb.add_space_charge(pos, ch, replace=True)
+            nb.solve_resident()
+        ok = ok and torch.equal(pos_s, pos) and np.array_equal(sig_s, nb.solve())
+        nb.close()
+        out_q.put((rank, bool(ok)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_real_library():
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out_q = ctx.Queue()
+    procs = [ctx.Process(target=_rank_worker, args=(r, 2, port, out_q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out_q.get(timeout=300) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(0, True), (1, True)]

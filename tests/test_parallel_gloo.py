@@ -28,6 +28,28 @@ class _FakeNeb:
         return pts[0] * 2.0 + pts[2], torch.stack([pts[0], pts[1] * 3.0, -pts[2]])
 
 
+class _FakeLoop:
+    """A replica of the space-charge loop's state on the CPU: E = a known function of the point and of the whole cloud."""
+
+    def __init__(self):
+        self.cloud = None
+        self.solves = 0
+
+    def add_space_charge(self, pos, charge, replace=True):
+        self.cloud = pos.clone()
+
+    def eval(self, pts, want_phi=True):
+        c = self.cloud.mean(dim=1, keepdim=True)              # depends on ALL charges, as the direct sum does
+        return None, (pts - c) * 2.0
+
+    def push(self, pos, E, mu_dt):
+        pos += mu_dt * E
+        return pos
+
+    def solve_resident(self):
+        self.solves += 1
+
+
 def _worker(rank, world, port, m, q):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -41,6 +63,18 @@ def _worker(rank, world, port, m, q):
         phi_l, _ = parallel.eval_sharded(_FakeNeb(), pts, gather=False)
         ok = ok and phi_l.shape[0] == e - s
         t = parallel.max_over_ranks(10.0 + rank)
+        # the C4 step with the charges sharded: 3 steps equal the unsharded loop, on every rank
+        pos = torch.rand((3, 1001), generator=g, dtype=torch.float64)
+        ch = torch.ones(1001, dtype=torch.float64)
+        loop, ref, pos_ref = _FakeLoop(), _FakeLoop(), pos.clone()
+        loop.add_space_charge(pos, ch)
+        ref.add_space_charge(pos_ref, ch)
+        for _ in range(3):
+            pos = parallel.c4_step_sharded(loop, pos, ch, 0.125)
+            _, E = ref.eval(pos_ref)
+            pos_ref = ref.push(pos_ref.clone(), E, 0.125)
+            ref.add_space_charge(pos_ref, ch)
+        ok = ok and torch.equal(pos, pos_ref) and loop.solves == 3 and torch.equal(loop.cloud, pos_ref)
         q.put((rank, bool(ok), t))
     finally:
         dist.destroy_process_group()
