@@ -109,7 +109,8 @@ neb_status neb_set_option(neb_ctx* ctx, int32_t option, int64_t value);
  *   eps_plus, eps_minus   may be NULL if no row is dielectric.
  *   n_img, img_shift      periodic copies (reading S12): 3*n_img SoA shift vectors, which must
  *             include (0,0,0); every coefficient sums the element's copies.  NULL / 0 = none.
- *             The same copies are applied by neb_eval; never to space charges.
+ *             The same copies are applied by neb_eval; never to space charges.  At most 16384 copies
+ *             (70 x 70 repetitions); beyond 32 the kernels run once per 32 copies.
  * Errors: NEB_EINVAL (n <= 0, NULL required array, unknown kind, zero-length edge, wire without
  * radius, eps_plus == eps_minus on a dielectric row), NEB_ENOMEM, NEB_ECUDA. */
 neb_status neb_assemble(neb_ctx* ctx, int64_t n, const int32_t* kind, const double* v0, const double* e1,

@@ -306,6 +306,7 @@ static void free_problem(neb_ctx* c) {
   c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr; c->d_dinv = nullptr;
   c->assembled = c->factored = c->have_sigma = false;
   c->n = c->npad = c->stride = 0;
+  c->img_cap = 0;
 }
 
 }  // namespace neb
@@ -416,7 +417,8 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
   const int64_t n_max = std::max<int64_t>(panel_cluster_max_rows(c), (int64_t)c->num_sms * 384) - kPad;
   if (n <= 0 || n > n_max || !kind || !v0 || !e1 || !e2 || !bc_kind)
     return fail(c, NEB_EINVAL, "neb_assemble: n must be in 1.." + std::to_string(n_max) + " and kind, v0, e1, e2, bc_kind non-NULL");
-  if (n_img < 0 || n_img > 32 || (n_img > 0 && !img_shift)) return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= 32");
+  if (n_img < 0 || n_img > kMaxImages || (n_img > 0 && !img_shift))
+    return fail(c, NEB_EINVAL, "neb_assemble: 0 <= n_img <= " + std::to_string(kMaxImages));
   NEB_CUDA(c, cudaSetDevice(c->device));
   const bool reuse = (c->n == n && c->d_K != nullptr);   // same size as the last problem: keep the buffers
   if (!reuse) {
@@ -445,11 +447,16 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaMalloc((void**)&c->d_dinv, sizeof(double) * 2 * (npad / 64) * 4096));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
-    NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * 32));
   }
   c->n_img = n_img > 0 ? n_img : 1;
-  c->h_img_len[0] = 0.0;
-  NEB_CUDA(c, cudaMemsetAsync(c->d_img, 0, sizeof(double) * 3 * c->n_img, c->stream));
+  const int64_t n_chunks = (c->n_img + NEB_IMG_CHUNK - 1) / NEB_IMG_CHUNK;
+  if (n_chunks > c->img_cap || !c->d_img) {
+    if (c->d_img) { NEB_CUDA(c, cudaStreamSynchronize(c->stream)); NEB_CUDA(c, cudaFree(c->d_img)); c->d_img = nullptr; }
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_img, sizeof(double) * 3 * NEB_IMG_CHUNK * n_chunks));
+    c->img_cap = n_chunks;
+  }
+  c->h_img_len.assign((size_t)c->n_img, 0.0);
+  NEB_CUDA(c, cudaMemsetAsync(c->d_img, 0, sizeof(double) * 3 * NEB_IMG_CHUNK * n_chunks, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_rec, 0, sizeof(double) * kRec * st, c->stream));
   NEB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int32_t), c->stream));
 
@@ -466,31 +473,30 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
   NEB_TRY(sg.in(eps_plus, sizeof(double) * n, &dep));
   NEB_TRY(sg.in(eps_minus, sizeof(double) * n, &dem));
   if (n_img > 0) {
-    // the unshifted copy goes to slot 0 (the kernels treat slot 0 as the element itself); it must be present
-    double h_img[3 * 32];
-    NEB_CUDA(c, cudaMemcpy(h_img, img_shift, sizeof(double) * 3 * n_img, cudaMemcpyDefault));
+    // the unshifted copy goes to slot 0 (the kernels treat slot 0 of the first chunk as the element itself); it must be present
+    std::vector<double> h_img((size_t)3 * n_img);
+    NEB_CUDA(c, cudaMemcpy(h_img.data(), img_shift, sizeof(double) * 3 * n_img, cudaMemcpyDefault));
+    std::vector<double> len((size_t)n_img);
+    std::vector<int> order((size_t)n_img);
     int zero = -1;
-    for (int s = 0; s < n_img && zero < 0; ++s)
-      if (h_img[s] == 0.0 && h_img[n_img + s] == 0.0 && h_img[2 * n_img + s] == 0.0) zero = s;
-    if (zero < 0) { free_problem(c); return fail(c, NEB_EINVAL, "neb_assemble: img_shift must include (0,0,0)"); }
-    // copies sorted by the length of their shift (stable insertion sort): the zero shift lands in slot 0, and the
-    // far copies of Adaptive Modelling (neb_set_adaptive) form the tail
-    double len[32];
-    int order[32];
     for (int s = 0; s < n_img; ++s) {
-      len[s] = sqrt(h_img[s] * h_img[s] + h_img[n_img + s] * h_img[n_img + s] + h_img[2 * n_img + s] * h_img[2 * n_img + s]);
+      const double x = h_img[s], y = h_img[(size_t)n_img + s], z = h_img[(size_t)2 * n_img + s];
+      if (zero < 0 && x == 0.0 && y == 0.0 && z == 0.0) zero = s;
+      len[s] = sqrt(x * x + y * y + z * z);
       order[s] = s;
     }
-    for (int s = 1; s < n_img; ++s)
-      for (int t = s; t > 0 && len[order[t]] < len[order[t - 1]]; --t) { int tmp = order[t]; order[t] = order[t - 1]; order[t - 1] = tmp; }
-    double sorted[3 * 32];
+    if (zero < 0) { free_problem(c); return fail(c, NEB_EINVAL, "neb_assemble: img_shift must include (0,0,0)"); }
+    // copies sorted by the length of their shift (stable): the zero shift lands in slot 0, and the far copies of
+    // Adaptive Modelling (neb_set_adaptive) form the tail; packed in chunks of NEB_IMG_CHUNK, [chunk][3][32]
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len[a] < len[b]; });
+    std::vector<double> packed((size_t)3 * NEB_IMG_CHUNK * n_chunks, 0.0);
     for (int s = 0; s < n_img; ++s) {
-      for (int k = 0; k < 3; ++k) sorted[k * n_img + s] = h_img[k * n_img + order[s]];
+      const size_t base = (size_t)(s / NEB_IMG_CHUNK) * 3 * NEB_IMG_CHUNK + (size_t)(s % NEB_IMG_CHUNK);
+      for (int k = 0; k < 3; ++k) packed[base + (size_t)k * NEB_IMG_CHUNK] = h_img[(size_t)k * n_img + order[s]];
       c->h_img_len[s] = len[order[s]];
     }
-    for (int k = 0; k < 3 * n_img; ++k) h_img[k] = sorted[k];
-    NEB_CUDA(c, cudaMemcpyAsync(c->d_img, h_img, sizeof(double) * 3 * n_img, cudaMemcpyHostToDevice, c->stream));
-    NEB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_img is a stack buffer
+    NEB_CUDA(c, cudaMemcpyAsync(c->d_img, packed.data(), sizeof(double) * packed.size(), cudaMemcpyHostToDevice, c->stream));
+    NEB_CUDA(c, cudaStreamSynchronize(c->stream));   // packed is a local buffer
   }
   int32_t* d_counts = nullptr;
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&d_counts, 3 * sizeof(int32_t), c->pool, c->stream));

@@ -10,15 +10,21 @@
 // kind), every case distinction inside the influence function is a select: warps never diverge.
 // Work is split over element (or charge) chunks in grid.y so that small M still fills 148 SMs; the
 // per-chunk partial sums are added by reduce_kernel in a fixed order (deterministic, no fp64 atomics).
+#include <algorithm>
+
 #include "neb_internal.h"
 #include "neb_influence.cuh"
 
 namespace neb {
 
+#ifndef NEB_EVAL_UNROLL
+#define NEB_EVAL_UNROLL 2             // elements of a uniform window in flight per thread
+#endif
+constexpr int kEvalUnroll = NEB_EVAL_UNROLL;
 constexpr int kThreads = 128;   // threads per CTA = points per CTA
 constexpr int kTile = 64;       // elements per shared-memory tile
 constexpr int kChargeTile = 256;
-constexpr int kMaxImg = 32;     // periodic copies kept in shared memory
+constexpr int kMaxImg = NEB_IMG_CHUNK;   // periodic copies per launch (kept in shared memory); more copies: more launches
 
 // Element tiles are staged by the TMA unit: one thread arms an mbarrier with the tile's byte count and issues one
 // 1-D bulk copy (cp.async.bulk, SASS UBLKCP) per record field (64 elements x 8 bytes, contiguous in the SoA table);
@@ -96,7 +102,9 @@ __device__ __forceinline__ void far_copy(double area, double dx, double dy, doub
 
 // All elements of one kind in [lo, hi): tile loop, image loop, sink(j, weight_j, sum over copies).
 // seq = number of tiles this CTA has consumed so far (buffer = seq & 1, mbarrier parity = (seq >> 1) & 1).
-template <class M, int KIND, class Sink>
+// self0 (compile time: a runtime flag cost 4 % on the hot path): slot 0 of this chunk of copies is the element itself
+// (the first chunk); later chunks hold shifted copies only.
+template <class M, int KIND, bool self0, class Sink>
 __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img, int n_near,
                                              double px, double py, double pz, Sink& sink, unsigned& seq) {
   const int64_t tb0 = lo & ~(int64_t)(kTile - 1);
@@ -127,15 +135,17 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
       const double PY = fma(px, ax.eyx, fma(py, ax.eyy, pz * ax.eyz));
       const double PZ = fma(px, ax.ezx, fma(py, ax.ezy, pz * ax.ezz));
       sink.tile_begin(ax);
-#pragma unroll 2
+#pragma unroll kEvalUnroll
       for (int e = e0; e < e1; ++e) {
         const double a = sm.rec[buf][12][e], b = sm.rec[buf][13][e], aux = sm.rec[buf][14][e], far2 = sm.rec[buf][16][e];
         const double X0 = PX - sm.rec[buf][17][e], Y0 = PY - sm.rec[buf][18][e], Z0 = PZ - sm.rec[buf][19][e];
-        double phi, lx, ly, lz;
-        local_pair<M, KIND>(a, b, aux, far2, X0, Y0, Z0, phi, lx, ly, lz);
-        if (sink.self_pv(tb + e)) { lx = 0.0; ly = 0.0; lz = 0.0; }   // principal value (S5, S8)
+        double phi = 0.0, lx = 0.0, ly = 0.0, lz = 0.0;
+        if (self0) {
+          local_pair<M, KIND>(a, b, aux, far2, X0, Y0, Z0, phi, lx, ly, lz);
+          if (sink.self_pv(tb + e)) { lx = 0.0; ly = 0.0; lz = 0.0; }   // principal value (S5, S8)
+        }
 #pragma unroll 1
-        for (int s = 1; s < n_near; ++s) {
+        for (int s = self0 ? 1 : 0; s < n_near; ++s) {
           double p1, x1, y1, z1;
           local_pair<M, KIND>(a, b, aux, far2, X0 - sm.limg[0][s], Y0 - sm.limg[1][s], Z0 - sm.limg[2][s], p1, x1, y1, z1);
           phi += p1; lx += x1; ly += y1; lz += z1;
@@ -157,10 +167,13 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
         Frame fr = frame_of(sm, buf, e);
         // slot 0 is the unshifted copy (the host puts it there).  For the pair (collocation point of element j,
         // element j) its field is dropped: principal value of a flat element's normal field on itself (S5, S8)
-        Infl acc = influence<M, KIND>(fr, px, py, pz);   // slot 0 holds the zero shift
-        if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
+        Infl acc = {0.0, 0.0, 0.0, 0.0};
+        if (self0) {
+          acc = influence<M, KIND>(fr, px, py, pz);      // slot 0 of the first chunk holds the zero shift
+          if (sink.self_pv(tb + e)) { acc.ex = 0.0; acc.ey = 0.0; acc.ez = 0.0; }
+        }
 #pragma unroll 1
-        for (int s = 1; s < n_near; ++s) {
+        for (int s = self0 ? 1 : 0; s < n_near; ++s) {
           Infl o = influence<M, KIND>(fr, px - sm.img[0][s], py - sm.img[1][s], pz - sm.img[2][s]);
           acc.phi += o.phi; acc.ex += o.ex; acc.ey += o.ey; acc.ez += o.ez;
         }
@@ -183,22 +196,26 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
   }
 }
 
-template <class M, class Sink>
+template <class M, bool self0, class Sink>
 __device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, int64_t j1, TileSmem& sm, int n_img, int n_near,
                                               double px, double py, double pz, Sink& sink) {
   int64_t r1 = g.n_rect, t1 = r1 + g.n_tri, w1 = t1 + g.n_wire;
   int64_t lo, hi;
   unsigned seq = 0;
   lo = max(j0, (int64_t)0); hi = min(j1, r1);
-  if (lo < hi) process_kind<M, 0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 0, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, r1); hi = min(j1, t1);
-  if (lo < hi) process_kind<M, 1>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 1, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, t1); hi = min(j1, w1);
-  if (lo < hi) process_kind<M, 2>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 2, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
 }
 
+// img: one chunk of the copy table, [3][kMaxImg] (the host packs the sorted shifts in chunks of kMaxImg)
 __device__ __forceinline__ void load_images(TileSmem& sm, const double* img, int n_img) {
-  for (int idx = threadIdx.x; idx < 3 * n_img; idx += blockDim.x) sm.img[idx / n_img][idx % n_img] = img[idx];
+  for (int idx = threadIdx.x; idx < 3 * kMaxImg; idx += blockDim.x) {
+    const int k = idx / kMaxImg, sidx = idx % kMaxImg;
+    sm.img[k][sidx] = (sidx < n_img) ? img[idx] : 0.0;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -232,7 +249,7 @@ struct EvalSink {
 #ifndef NEB_EVAL_MINB
 #define NEB_EVAL_MINB 4
 #endif
-template <class M>
+template <class M, bool FIRST>
 __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img, int n_near,
                                                         const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                         double* __restrict__ partial) {
@@ -246,10 +263,11 @@ __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables
   int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
   int64_t j0 = (int64_t)blockIdx.y * per_split, j1 = min(n, j0 + per_split);
   EvalSink sink;
-  process_range<M>(g, j0, j1, sm, n_img, n_near, px, py, pz, sink);
+  process_range<M, FIRST>(g, j0, j1, sm, n_img, n_near, px, py, pz, sink);
   if (p < m) {
     double* o = partial + (int64_t)blockIdx.y * 4 * m;
-    o[p] = sink.phi; o[m + p] = sink.ex; o[2 * m + p] = sink.ey; o[3 * m + p] = sink.ez;
+    if (FIRST) { o[p] = sink.phi; o[m + p] = sink.ex; o[2 * m + p] = sink.ey; o[3 * m + p] = sink.ez; }
+    else { o[p] += sink.phi; o[m + p] += sink.ex; o[2 * m + p] += sink.ey; o[3 * m + p] += sink.ez; }   // later chunks of copies
   }
 }
 
@@ -316,14 +334,17 @@ __global__ void reduce_kernel(const double* __restrict__ partial, int n_elem_spl
 // Row maxima (for the S15 equilibration) are accumulated with an order-independent integer max.
 // ------------------------------------------------------------------------------------------------
 struct AsmSink {
-  double* K; int64_t ld, i; double nx, ny, nz, diag; bool dielectric, active; double rmax;
+  double* K; int64_t ld, i; double nx, ny, nz, diag; bool dielectric, active, first; double rmax;   // first: the first chunk of copies
   __device__ __forceinline__ bool self_pv(int64_t j) const { return j == i; }
-  __device__ __forceinline__ void operator()(int64_t j, double, const Infl& a) {
-    double vd = fma(nx, a.ex, fma(ny, a.ey, nz * a.ez));
-    double v = kCoulomb * (dielectric ? vd : a.phi);
-    v += (dielectric && j == i) ? diag : 0.0;
+  __device__ __forceinline__ void put(int64_t j, double v) {
+    v += (dielectric && j == i && first) ? diag : 0.0;
+    if (!first && active) v += K[i + j * ld];            // later chunks of copies add to the coefficient
     rmax = fmax(rmax, fabs(v));
     if (active) K[i + j * ld] = v;
+  }
+  __device__ __forceinline__ void operator()(int64_t j, double, const Infl& a) {
+    double vd = fma(nx, a.ex, fma(ny, a.ey, nz * a.ez));
+    put(j, kCoulomb * (dielectric ? vd : a.phi));
   }
   // uniform window: the row's normal in the window's axes, so that n . E' needs no rotation per pair
   double nlx = 0, nly = 0, nlz = 0;
@@ -334,17 +355,14 @@ struct AsmSink {
   }
   __device__ __forceinline__ void local(int64_t j, double, double p, double fx, double fy, double fz) {
     double vd = fma(nlx, fx, fma(nly, fy, nlz * fz));
-    double v = kCoulomb * (dielectric ? vd : p);
-    v += (dielectric && j == i) ? diag : 0.0;
-    rmax = fmax(rmax, fabs(v));
-    if (active) K[i + j * ld] = v;
+    put(j, kCoulomb * (dielectric ? vd : p));
   }
   __device__ __forceinline__ void tile_end(const Axes&) {}
   __device__ __forceinline__ void gtile_begin() {}
   __device__ __forceinline__ void gtile_end() {}
 };
 
-template <class M>
+template <class M, bool FIRST>
 __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const double* __restrict__ img, int n_img,
                                                             const double* __restrict__ colloc, int64_t stride,
                                                             const double* __restrict__ normal,
@@ -359,14 +377,16 @@ __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const d
   int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   int64_t ic = min(i, n - 1);
   AsmSink sink;
-  sink.K = K; sink.ld = ld; sink.i = ic; sink.active = i < n; sink.rmax = 0.0;
+  sink.K = K; sink.ld = ld; sink.i = ic; sink.active = i < n; sink.rmax = 0.0; sink.first = FIRST;
   sink.nx = normal[ic]; sink.ny = normal[stride + ic]; sink.nz = normal[2 * stride + ic];
   sink.dielectric = bc_kind[ic] == NEB_BC_DIELECTRIC;
   sink.diag = diag[ic];
   double px = colloc[ic], py = colloc[stride + ic], pz = colloc[2 * stride + ic];
   int64_t j0 = (int64_t)blockIdx.y * kTile, j1 = min(n, j0 + kTile);
-  process_range<M>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
-  if (i < n) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
+  process_range<M, FIRST>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
+  // the running maximum of a row whose coefficients are still being summed is not the row's maximum: with several
+  // chunks of copies only the LAST chunk's values (the finished coefficients) count
+  if (i < n && rowmax_bits) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
 }
 
 // rows/columns >= n of the padded matrix: identity
@@ -468,16 +488,25 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
   int n_near = c->n_img;
   if (c->adaptive_far > 0.0) {
     n_near = 1;
-    while (n_near < c->n_img && c->h_img_len[n_near] < c->adaptive_far) ++n_near;
+    while (n_near < c->n_img && c->h_img_len[(size_t)n_near] < c->adaptive_far) ++n_near;
   }
   if (se) {
     StageTimer t(c, NEB_STAGE_EVAL);
     dim3 grid((unsigned)pt_blocks, (unsigned)se);
-    if (c->math_fast)
-      eval_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, n_near, d_pts, m, per_e, partial);
-    else
-      eval_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, n_near, d_pts, m, per_e, partial);
-    c->launches++;
+    // more than kMaxImg copies: one launch per chunk of the (length-sorted) copy table, later chunks add to the partials
+    for (int ch = 0; ch * kMaxImg < c->n_img; ++ch) {
+      const int len = std::min(kMaxImg, c->n_img - ch * kMaxImg);
+      const int near_ch = std::max(0, std::min(len, n_near - ch * kMaxImg));
+      const double* img = c->d_img + (size_t)ch * 3 * kMaxImg;
+      if (c->math_fast) {
+        if (ch == 0) eval_kernel<MathFast, true><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+        else eval_kernel<MathFast, false><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+      } else {
+        if (ch == 0) eval_kernel<MathLib, true><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+        else eval_kernel<MathLib, false><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+      }
+      c->launches++;
+    }
     NEB_CUDA(c, cudaGetLastError());
   }
   if (sq) {
@@ -512,13 +541,22 @@ neb_status assemble_matrix(neb_ctx* c) {
   {
     StageTimer t(c, NEB_STAGE_ASSEMBLE);
     dim3 grid((unsigned)((n + kThreads - 1) / kThreads), (unsigned)((n + kTile - 1) / kTile));
-    if (c->math_fast)
-      assemble_kernel<MathFast><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, c->d_colloc, c->stride,
-                                                                   c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rowmax);
-    else
-      assemble_kernel<MathLib><<<grid, kThreads, 0, c->stream>>>(tables(c), c->d_img, c->n_img, c->d_colloc, c->stride,
-                                                                  c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rowmax);
-    c->launches++;
+    const int n_chunks = (c->n_img + kMaxImg - 1) / kMaxImg;
+    for (int ch = 0; ch < n_chunks; ++ch) {
+      const int len = std::min(kMaxImg, c->n_img - ch * kMaxImg);
+      const double* img = c->d_img + (size_t)ch * 3 * kMaxImg;
+      unsigned long long* rm = (ch == n_chunks - 1) ? rowmax : nullptr;      // row maxima from the finished coefficients
+#define NEB_ASM_ARGS tables(c), img, len, c->d_colloc, c->stride, c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rm
+      if (c->math_fast) {
+        if (ch == 0) assemble_kernel<MathFast, true><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        else assemble_kernel<MathFast, false><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+      } else {
+        if (ch == 0) assemble_kernel<MathLib, true><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        else assemble_kernel<MathLib, false><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+      }
+#undef NEB_ASM_ARGS
+      c->launches++;
+    }
     NEB_CUDA(c, cudaGetLastError());
     int64_t padcells = (npad - n) * npad + n * (npad - n);
     if (padcells > 0) {

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/neb.h"
 
@@ -12,6 +13,8 @@ constexpr double kEps0 = 8.8541878128e-12;                 // F/m (reading S3)
 constexpr double kCoulomb = 1.0 / (4.0 * 3.14159265358979323846 * kEps0);
 constexpr int kRec = 20;                                   // doubles per frame-table record
 constexpr int kPad = 128;                                  // matrix dimension is padded to a multiple of this
+#define NEB_IMG_CHUNK 32                                   // periodic copies per kernel launch (shared-memory table)
+constexpr int kMaxImages = 16384;                          // copies per element accepted by neb_assemble
 
 // Frame tables (a1), elements sorted by kind: [rect | tri | wire].  SoA, field-major:
 // rec[f * stride + j], f < kRec (fields listed in neb_influence.cuh).
@@ -65,8 +68,9 @@ struct neb_ctx {
   int32_t* d_bc_kind = nullptr;   // sorted
   double* d_bc_value = nullptr;   // sorted
   double* d_diag = nullptr;       // sorted: 1/(2 eps0 lambda) on dielectric rows, else 0
-  double* d_img = nullptr;        // 3 * n_img, sorted by length (slot 0 = the zero shift)
-  double h_img_len[32] = {0};     // their lengths (host)
+  double* d_img = nullptr;        // copies sorted by length (slot 0 = the zero shift), packed in chunks of NEB_IMG_CHUNK: [chunk][3][32]
+  int64_t img_cap = 0;            // chunks allocated
+  std::vector<double> h_img_len;  // their lengths (host)
   double adaptive_far = 0.0;      // Adaptive Modelling: copies at least this far are simplified in neb_eval (0 = off)
   int32_t* d_flag = nullptr;      // device error flags (validation, singular pivot)
 

@@ -11,11 +11,18 @@ import torch
 import torch.distributed as dist
 
 
-def shard_bounds(m: int, world: int, rank: int):
-    """Contiguous, balanced slab [start, stop) of m units for `rank`; the slabs tile [0, m) exactly."""
-    base, extra = divmod(int(m), int(world))
-    start = rank * base + min(rank, extra)
-    return start, start + base + (1 if rank < extra else 0)
+ALIGN = 128      # points per CTA of the evaluation kernels
+
+
+def shard_bounds(m: int, world: int, rank: int, align: int = 1):
+    """Contiguous, balanced slab [start, stop) of m units for `rank`; the slabs tile [0, m) exactly.  With align > 1 every
+    boundary but the last is a multiple of `align`: the evaluation kernels decide their near/far branch per WARP, so only
+    slabs cut at CTA boundaries (align = 128) give every point the warp it has in the unsharded launch, hence the same bits."""
+    blocks = -(-int(m) // align)
+    base, extra = divmod(blocks, int(world))
+    start = (rank * base + min(rank, extra)) * align
+    stop = start + (base + (1 if rank < extra else 0)) * align
+    return min(start, int(m)), min(stop, int(m))
 
 
 def max_over_ranks(value: float, device="cpu") -> float:
@@ -27,13 +34,13 @@ def max_over_ranks(value: float, device="cpu") -> float:
     return float(t.item())
 
 
-def all_gather_points(local: torch.Tensor, m: int) -> torch.Tensor:
+def all_gather_points(local: torch.Tensor, m: int, align: int = 1) -> torch.Tensor:
     """All-gather of per-rank slabs along the LAST dimension (Phi: (m_local,), E: (3, m_local)) into the
     full (…, m) tensor on every rank.  Slabs are the ones of shard_bounds, so they may differ by one."""
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
         return local
     world = dist.get_world_size()
-    width = max(shard_bounds(m, world, r)[1] - shard_bounds(m, world, r)[0] for r in range(world))
+    width = max(shard_bounds(m, world, r, align)[1] - shard_bounds(m, world, r, align)[0] for r in range(world))
     # a CPU-only backend (gloo: the multi-rank tests, also with the ranks' kernels on one shared GPU) gathers on the host
     via_host = local.is_cuda and dist.get_backend() == "gloo"
     src = local.cpu() if via_host else local
@@ -43,7 +50,7 @@ def all_gather_points(local: torch.Tensor, m: int) -> torch.Tensor:
     dist.all_gather(parts, pad)
     out = []
     for r in range(world):
-        s, e = shard_bounds(m, world, r)
+        s, e = shard_bounds(m, world, r, align)
         out.append(parts[r][..., : e - s])
     res = torch.cat(out, dim=-1)
     return res.to(local.device) if via_host else res
@@ -61,11 +68,11 @@ def c4_step_sharded(nb, pos: torch.Tensor, charge: torch.Tensor, mu_dt: float):
     q = pos.shape[1]
     world = dist.get_world_size() if dist.is_initialized() else 1
     rank = dist.get_rank() if dist.is_initialized() else 0
-    s, e = shard_bounds(q, world, rank)
+    s, e = shard_bounds(q, world, rank, ALIGN)
     mine = pos[:, s:e].contiguous()
     _, E = nb.eval(mine, want_phi=False)
     nb.push(mine, E, mu_dt)
-    new_pos = all_gather_points(mine, q).contiguous()
+    new_pos = all_gather_points(mine, q, ALIGN).contiguous()
     nb.add_space_charge(new_pos, charge, replace=True)
     nb.solve_resident()
     return new_pos
@@ -79,8 +86,8 @@ def eval_sharded(nb, pts: torch.Tensor, gather: bool = True):
     m = pts.shape[1]
     world = dist.get_world_size() if dist.is_initialized() else 1
     rank = dist.get_rank() if dist.is_initialized() else 0
-    s, e = shard_bounds(m, world, rank)
+    s, e = shard_bounds(m, world, rank, ALIGN)
     phi, E = nb.eval(pts[:, s:e].contiguous())
     if gather:
-        return all_gather_points(phi, m), all_gather_points(E, m)
+        return all_gather_points(phi, m, ALIGN), all_gather_points(E, m, ALIGN)
     return phi, E

@@ -235,6 +235,34 @@ def test_assembly_and_eval_random_mixed(nb, orc, math):
     check_field(phi, E, phi_o, E_o, TOL_FAR, f"random mixed math={math}", S)
 
 
+def test_more_than_32_image_copies(nb, orc):
+    """7 x 7 = 49 periodic copies (P:391 uses 70 x 70): the kernels run once per chunk of 32 copies, later chunks add to
+    the coefficients / partial sums; assembly (Dirichlet and dielectric rows) and eval against the oracle, and
+    Adaptive Modelling with the near/far boundary inside the second chunk."""
+    pr = W.random_elements(150, seed=77, kinds=(W.RECT, W.TRI, W.WIRE), size_mm=(0.05, 0.2), box_mm=0.4, m_points=1500,
+                           dielectric_fraction=0.3)
+    pr.img_shift = W.image_shifts(3, pitch_mm=1.0)
+    assert pr.n_img == 49
+    g = orc.Geometry(pr)
+    nb.assemble_problem(pr)
+    K, Ko = nb.get_matrix(), orc.assemble(g)
+    assert np.max(np.abs(K - Ko) / np.abs(Ko).max(axis=1, keepdims=True)) <= TOL_K
+    s = nb.solve()
+    so = orc.solve(Ko, orc.rhs(g))
+    assert np.max(np.abs(s - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    pts = pr.points * 0.25                                                  # inside the central cell
+    phi, E = nb.eval(pts)
+    phi_o, E_o, S = truth(orc, g, s, pts)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "49 image copies", S)
+    far = 3.3e-3                                                            # 37 of the 49 copies stay exact: 32 + 5
+    assert np.sum(np.linalg.norm(pr.img_shift, axis=0) < far) == 37
+    nb.set_adaptive(far)
+    phi_a, E_a = nb.eval(pts)
+    phi_ao, E_ao = orc.evaluate_adaptive(g, s, pts, far)
+    check_field(phi_a, E_a, phi_ao, E_ao, TOL_FAR, "49 image copies, adaptive", S)
+    nb.set_adaptive(0.0)
+
+
 def test_explicit_collocation_points(nb, orc):
     pr = W.random_elements(40, seed=8, kinds=(W.RECT, W.TRI))
     col = pr.centroids() + 1e-5 * pr.normals()
@@ -842,6 +870,11 @@ def test_edge_cases_and_errors(nb, P, orc):
     with pytest.raises(P.NebError) as e:
         nb.solve()
     assert e.value.status == 4                               # NEB_ESINGULAR
+    big = W.plate(n_side=2)                                  # more copies than the ABI accepts
+    big.img_shift = np.zeros((3, 16385))
+    with pytest.raises(P.NebError) as e:
+        nb.assemble_problem(big)
+    assert e.value.status == 1
     shifts = W.image_shifts(1)[:, 1:]                        # image set without the zero shift
     ok = W.plate(n_side=2)
     ok.img_shift = shifts

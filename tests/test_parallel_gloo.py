@@ -19,6 +19,9 @@ def test_shard_bounds_tile_exactly():
             assert all(b[r][1] == b[r + 1][0] for r in range(world - 1))
             sizes = [e - s for s, e in b]
             assert max(sizes) - min(sizes) <= 1
+            a = [parallel.shard_bounds(m, world, r, align=128) for r in range(world)]
+            assert a[0][0] == 0 and a[-1][1] == m and all(a[r][1] == a[r + 1][0] for r in range(world - 1))
+            assert all(s % 128 == 0 or s == m for s, _ in a) and max(e - s for s, e in a) - min(e - s for s, e in a) <= 255
 
 
 class _FakeNeb:
@@ -59,7 +62,7 @@ def _worker(rank, world, port, m, q):
         pts = torch.rand((3, m), generator=g, dtype=torch.float64)          # same points on every rank
         phi, E = parallel.eval_sharded(_FakeNeb(), pts, gather=True)
         ok = torch.equal(phi, pts[0] * 2.0 + pts[2]) and torch.equal(E, torch.stack([pts[0], pts[1] * 3.0, -pts[2]]))
-        s, e = parallel.shard_bounds(m, world, rank)
+        s, e = parallel.shard_bounds(m, world, rank, parallel.ALIGN)
         phi_l, _ = parallel.eval_sharded(_FakeNeb(), pts, gather=False)
         ok = ok and phi_l.shape[0] == e - s
         t = parallel.max_over_ranks(10.0 + rank)
