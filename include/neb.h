@@ -195,6 +195,58 @@ neb_status neb_get_line_charges(neb_ctx* ctx, double* lines);
  * 3*q values, in place.  Stateless; pos and E must both be device or both be host pointers. */
 neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, double mu_dt);
 
+/* Scale-out of the solve (InvertMatrix with OptLU, Alg. 1, for a matrix spread over
+ * several GPUs).  Right-looking block LU with partial pivoting on a matrix whose 256-column blocks are dealt
+ * cyclically to `world` contexts, one per GPU, one process each: block g lives on rank g % world; every rank holds
+ * all rows of its blocks, the whole geometry and, after the factorisation, all pivots.  The library performs every
+ * step of the arithmetic; the exchanges BETWEEN the steps belong to the caller (torch.distributed over NCCL / NVLink:
+ * paper_2606_24154_b200/parallel.py, dist_solve): a minimum of the row scales, one broadcast per block, a 256-value
+ * sum per block and triangle in the solves, one sum of the solution vector.  Order of calls on EVERY rank:
+ *
+ *   neb_dist_configure(rank, world)       on a fresh context; world = 1 runs the same code on one context
+ *   neb_assemble(...)                     assembles the rank's column blocks only (8 npad ncol_local bytes); the padded
+ *                                         dimension npad = neb_dist_npad() is a multiple of 256
+ *   neb_dist_row_scales(s, 0)             s (npad, device) <- 1/max_j|K_ij| over THIS rank's columns (+inf: none);
+ *   [caller: element-wise MIN over ranks] = the S15 row scales of the whole matrix
+ *   neb_dist_row_scales(s, 1)             stores them and scales the local columns
+ *   for g = 0 .. npad/256 - 1:
+ *     owner g % world: neb_dist_factor_block(g, panel, piv, stream)   factors the block (4 panels of 64 columns on one
+ *                                         cluster each, in-block row exchanges, TRSM, rank-64 DMMA updates) and packs
+ *                                         rows 256 g .. npad of it into panel ((npad - 256 g) x 256, column-major,
+ *                                         device) and its 256 pivot rows into piv (int32, device); stream (a
+ *                                         cudaStream_t, NULL = the context's) lets the next block be factored beside
+ *                                         the trailing update (look-ahead)
+ *     [caller: broadcast panel, piv from the owner]
+ *     all ranks: neb_dist_apply_block(g, panel, piv, part)            row exchanges, U12 = L11^-1 A12 and the rank-256
+ *                                         DMMA update on the rank's columns right of block g (L read from panel), row
+ *                                         exchanges on the columns left of it.  part 0: everything; part 1: only the
+ *                                         columns of block g + 1 (no-op unless this rank owns it); part 2: the rest
+ *   neb_dist_finish_factor(&singular)     composed row permutation; singular (host) = 1 if one of THIS rank's panels
+ *                                         met a zero / NaN pivot [caller: MAX over ranks]
+ *   neb_dist_rhs(y)                       y (npad, device) <- the scaled, row-permuted right-hand side (a4, replicated)
+ *   forward, g ascending, acc = 0 (npad, device):  [caller: acc[256 g .. +256) <- its sum over the ranks]
+ *     neb_dist_tri_block(0, g, y, acc)    owner: y_g <- L_gg^-1 (y_g - acc_g); acc[below] += L[below, g] y_g
+ *   backward, g descending, acc = 0:      [same sum]
+ *     neb_dist_tri_block(1, g, y, acc)    owner: y_g <- U_gg^-1 (y_g - acc_g); acc[above] += U[above, g] y_g
+ *   [caller: x = sum over ranks of (y restricted to the rank's own blocks)]
+ *   neb_dist_set_solution(x, sigma_out)   sigma in the caller's element order (n doubles, host or device, may be NULL);
+ *                                         neb_eval, neb_fastvol_* and neb_add_space_charge then work as on one GPU
+ *                                         (every rank a replica of the element tables); a new right-hand side repeats
+ *                                         the steps from neb_dist_rhs on the resident factors.
+ * neb_solve, neb_solve_weighting*, neb_get_matrix* return NEB_ESTATE on a distributed context.
+ * Errors: NEB_EINVAL (rank/world, block index, a block this rank does not own, host pointers where device ones are
+ * required), NEB_ESTATE (order of calls), NEB_ECUDA. */
+#define NEB_DIST_BLOCK 256
+neb_status neb_dist_configure(neb_ctx* ctx, int32_t rank, int32_t world);
+int64_t neb_dist_npad(const neb_ctx* ctx);
+neb_status neb_dist_row_scales(neb_ctx* ctx, double* scales, int32_t set);
+neb_status neb_dist_factor_block(neb_ctx* ctx, int64_t g, double* panel, int32_t* piv, void* cuda_stream);
+neb_status neb_dist_apply_block(neb_ctx* ctx, int64_t g, const double* panel, const int32_t* piv, int32_t part);
+neb_status neb_dist_finish_factor(neb_ctx* ctx, int32_t* singular);
+neb_status neb_dist_rhs(neb_ctx* ctx, double* y);
+neb_status neb_dist_tri_block(neb_ctx* ctx, int32_t upper, int64_t g, double* y, double* acc);
+neb_status neb_dist_set_solution(neb_ctx* ctx, const double* x, double* sigma_out);
+
 /* Test hooks.  neb_get_matrix: the UNSCALED matrix in the caller's element order, n*n
  * column-major (K_out[i + j*n] = row i, column j); only between neb_assemble and the first
  * neb_solve (NEB_ESTATE afterwards: the factors overwrite it).  neb_get_rhs: the RHS the last

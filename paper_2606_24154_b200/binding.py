@@ -9,6 +9,7 @@ from . import build as _build
 
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
+NEB_DIST_BLOCK = 256
 NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS = 0, 1, 2, 3, 4, 5
 STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
@@ -71,6 +72,16 @@ def lib():
         L.neb_reset_stats.argtypes = [vp]
         L.neb_launch_count.argtypes = [vp]
         L.neb_launch_count.restype = i64
+        L.neb_dist_configure.argtypes = [vp, i32, i32]
+        L.neb_dist_npad.argtypes = [vp]
+        L.neb_dist_npad.restype = i64
+        L.neb_dist_row_scales.argtypes = [vp, vp, i32]
+        L.neb_dist_factor_block.argtypes = [vp, i64, vp, vp, vp]
+        L.neb_dist_apply_block.argtypes = [vp, i64, vp, vp, i32]
+        L.neb_dist_finish_factor.argtypes = [vp, C.POINTER(i32)]
+        L.neb_dist_rhs.argtypes = [vp, vp]
+        L.neb_dist_tri_block.argtypes = [vp, i32, i64, vp, vp]
+        L.neb_dist_set_solution.argtypes = [vp, vp, vp]
         _lib = L
     return _lib
 
@@ -318,3 +329,34 @@ class Neb:
 
     def launch_count(self) -> int:
         return int(self._L.neb_launch_count(self._h))
+
+    # ---- scale-out of the solve (neb_dist_*): device tensors only; the exchanges are parallel.dist_solve's
+    def dist_configure(self, rank: int, world: int):
+        self._ck(self._L.neb_dist_configure(self._h, rank, world))
+
+    def dist_npad(self) -> int:
+        return int(self._L.neb_dist_npad(self._h))
+
+    def dist_row_scales(self, scales, set_: bool):
+        self._ck(self._L.neb_dist_row_scales(self._h, _ptr(scales), 1 if set_ else 0))
+
+    def dist_factor_block(self, g: int, panel, piv, stream=None):
+        self._ck(self._L.neb_dist_factor_block(self._h, g, _ptr(panel), _ptr(piv), C.c_void_p(stream.cuda_stream) if stream is not None else None))
+
+    def dist_apply_block(self, g: int, panel, piv, part: int = 0):
+        self._ck(self._L.neb_dist_apply_block(self._h, g, _ptr(panel), _ptr(piv), part))
+
+    def dist_finish_factor(self) -> int:
+        s = C.c_int32(0)
+        self._ck(self._L.neb_dist_finish_factor(self._h, C.byref(s)))
+        return int(s.value)
+
+    def dist_rhs(self, y):
+        self._ck(self._L.neb_dist_rhs(self._h, _ptr(y)))
+
+    def dist_tri_block(self, upper: bool, g: int, y, acc):
+        self._ck(self._L.neb_dist_tri_block(self._h, 1 if upper else 0, g, _ptr(y), _ptr(acc)))
+
+    def dist_set_solution(self, x, out=None):
+        self._ck(self._L.neb_dist_set_solution(self._h, _ptr(x), _ptr(out)))
+        return out

@@ -52,6 +52,8 @@ static bool is_device_ptr(const void* p) {
   return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
+bool is_device_pointer(const void* p) { return is_device_ptr(p); }
+
 struct Staging {   // temporaries of one ABI call
   neb_ctx* c;
   std::vector<void*> temps;
@@ -309,6 +311,14 @@ static void free_problem(neb_ctx* c) {
   c->img_cap = 0;
 }
 
+neb_status finish_sigma(neb_ctx* c, const double* d_x) {
+  finish_sigma_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->stride, c->d_perm, d_x, c->d_rec, c->d_sigma);
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  c->have_sigma = true;
+  return NEB_OK;
+}
+
 }  // namespace neb
 
 using namespace neb;
@@ -425,10 +435,13 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));
     free_problem(c);
     c->n = n;
-    c->npad = (n + kPad - 1) / kPad * kPad;
+    const int64_t pad = c->dist_mode ? kDistBlock : kPad;     // distributed: whole 256-column blocks
+    c->npad = (n + pad - 1) / pad * pad;
     c->stride = c->npad;
+    c->ncol_loc = dist_local_cols(c->npad, c->dist_world, c->dist_rank);
   }
   c->assembled = c->factored = c->have_sigma = false;
+  c->dist_scaled = false;
   const int64_t st = c->stride, npad = c->npad;
   if (!reuse) {
     NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
@@ -446,7 +459,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
     NEB_CUDA(c, cudaMalloc((void**)&c->d_x, sizeof(double) * 16 * npad));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_dinv, sizeof(double) * 2 * (npad / 64) * 4096));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_sigma, sizeof(double) * n));
-    NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)npad));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_K, sizeof(double) * (size_t)npad * (size_t)c->ncol_loc));
   }
   c->n_img = n_img > 0 ? n_img : 1;
   const int64_t n_chunks = (c->n_img + NEB_IMG_CHUNK - 1) / NEB_IMG_CHUNK;
@@ -539,6 +552,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
 neb_status neb_solve(neb_ctx* c, double* sigma_out) {
   if (!c) return NEB_EINVAL;
   if (!c->assembled) return fail(c, NEB_ESTATE, "neb_solve before neb_assemble");
+  if (c->dist_mode) return fail(c, NEB_ESTATE, "neb_solve on a distributed context: the factorisation runs through the neb_dist_* calls");
   NEB_CUDA(c, cudaSetDevice(c->device));
   if (!c->factored) {
     NEB_TRY(scale_matrix_rows(c));
@@ -554,10 +568,7 @@ neb_status neb_solve(neb_ctx* c, double* sigma_out) {
   }
   NEB_TRY(form_rhs(c));
   NEB_TRY(lu_solve(c, c->d_b, 1, c->d_x));
-  finish_sigma_kernel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(c->n, c->stride, c->d_perm, c->d_x, c->d_rec, c->d_sigma);
-  c->launches++;
-  NEB_CUDA(c, cudaGetLastError());
-  c->have_sigma = true;
+  NEB_TRY(finish_sigma(c, c->d_x));
   if (sigma_out) {
     if (is_device_ptr(sigma_out)) {
       NEB_CUDA(c, cudaMemcpyAsync(sigma_out, c->d_sigma, sizeof(double) * c->n, cudaMemcpyDeviceToDevice, c->stream));
@@ -608,6 +619,7 @@ neb_status neb_set_adaptive(neb_ctx* c, double far_distance) {
 neb_status neb_solve_weighting_multi(neb_ctx* c, int32_t n_rhs, const double* bc_value_w, double* sigma_w_out) {
   if (!c || n_rhs < 1 || !bc_value_w || !sigma_w_out) return NEB_EINVAL;
   if (!c->factored || !c->assembled) return fail(c, NEB_ESTATE, "neb_solve_weighting before the first neb_solve (no LU factors)");
+  if (c->dist_mode) return fail(c, NEB_ESTATE, "neb_solve_weighting: not available on a distributed context");
   NEB_CUDA(c, cudaSetDevice(c->device));
   Staging sg(c);
   const void* dw;
@@ -741,6 +753,7 @@ neb_status neb_push(neb_ctx* c, int64_t q, double* pos, const double* E, double 
 neb_status neb_get_matrix(neb_ctx* c, double* K_out) {
   if (!c || !K_out) return NEB_EINVAL;
   if (!c->assembled || c->factored) return fail(c, NEB_ESTATE, "neb_get_matrix: only between neb_assemble and the first neb_solve");
+  if (c->dist_mode) return fail(c, NEB_ESTATE, "neb_get_matrix: not available on a distributed context (each rank holds only its column blocks)");
   NEB_CUDA(c, cudaSetDevice(c->device));
   Staging sg(c);
   void* dout;
@@ -755,6 +768,7 @@ neb_status neb_get_matrix(neb_ctx* c, double* K_out) {
 neb_status neb_get_matrix_rows(neb_ctx* c, int64_t n_rows, const int32_t* rows, double* K_out) {
   if (!c || n_rows < 0 || (n_rows > 0 && (!rows || !K_out))) return NEB_EINVAL;
   if (!c->assembled || c->factored) return fail(c, NEB_ESTATE, "neb_get_matrix_rows: only between neb_assemble and the first neb_solve");
+  if (c->dist_mode) return fail(c, NEB_ESTATE, "neb_get_matrix_rows: not available on a distributed context (each rank holds only its column blocks)");
   if (n_rows == 0) return NEB_OK;
   if (n_rows > 65535) return fail(c, NEB_EINVAL, "neb_get_matrix_rows: at most 65535 rows per call");
   NEB_CUDA(c, cudaSetDevice(c->device));

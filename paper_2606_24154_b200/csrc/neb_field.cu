@@ -272,42 +272,56 @@ __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables
 }
 
 // ------------------------------------------------------------------------------------------------
-// a8: point charges.  charges SoA x,y,z,q with stride q_stride; grid = (ceil(m/128), n_split)
+// a8: point charges.  charges SoA x,y,z,q with stride q_stride; grid = (ceil(m / (128 kChargePpt)), n_split).
+// A thread owns kChargePpt points (p, p + 128, ...: coalesced) so that one pair of 16-byte shared-memory loads of a
+// charge (x, y, z, q packed per charge in the tile) serves kChargePpt pairs and their dependent 1/r chains interleave.
 // ------------------------------------------------------------------------------------------------
+#ifndef NEB_CHARGE_PPT
+#define NEB_CHARGE_PPT 2
+#endif
+constexpr int kChargePpt = NEB_CHARGE_PPT;
 __global__ void __launch_bounds__(kThreads) charge_kernel(const double* __restrict__ ch, int64_t q, int64_t q_stride,
                                                           const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                           double* __restrict__ partial) {
-  __shared__ double sc[4][kChargeTile];
-  int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
-  int64_t pc = min(p, m - 1);
-  double px = pts[pc], py = pts[m + pc], pz = pts[2 * m + pc];
+  __shared__ double4 sc[kChargeTile];
+  const int64_t p0 = (int64_t)blockIdx.x * (kThreads * kChargePpt) + threadIdx.x;
+  double px[kChargePpt], py[kChargePpt], pz[kChargePpt];
+  double phi[kChargePpt], ex[kChargePpt], ey[kChargePpt], ez[kChargePpt];
+#pragma unroll
+  for (int u = 0; u < kChargePpt; ++u) {
+    const int64_t pc = min(p0 + u * kThreads, m - 1);
+    px[u] = pts[pc]; py[u] = pts[m + pc]; pz[u] = pts[2 * m + pc];
+    phi[u] = 0; ex[u] = 0; ey[u] = 0; ez[u] = 0;
+  }
   int64_t k0 = (int64_t)blockIdx.y * per_split, k1 = min(q, k0 + per_split);
-  double phi = 0, ex = 0, ey = 0, ez = 0;
   for (int64_t base = k0; base < k1; base += kChargeTile) {
     int cnt = (int)min((int64_t)kChargeTile, k1 - base);
     __syncthreads();
-    for (int idx = threadIdx.x; idx < 4 * kChargeTile; idx += blockDim.x) {
-      int f = idx / kChargeTile, e = idx % kChargeTile;
-      if (e < cnt) sc[f][e] = ch[f * q_stride + base + e];
-    }
+    for (int e = threadIdx.x; e < cnt; e += blockDim.x)
+      sc[e] = make_double4(ch[base + e], ch[q_stride + base + e], ch[2 * q_stride + base + e], ch[3 * q_stride + base + e]);
     __syncthreads();
-#pragma unroll 4
+#pragma unroll 2
     for (int e = 0; e < cnt; ++e) {
-      double dx = px - sc[0][e], dy = py - sc[1][e], dz = pz - sc[2][e];
-      double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-      // 1/r: MUFU.RSQ64H seed + one cubic step; a charge exactly at the point is skipped.  The clamp and
-      // the r = 0 test are integer operations on the bit pattern: 18 FP64-pipe operations per pair in all (30 flop)
-      double y = rsqrt_pos(clamp_tiny(r2));
-      y = is_zero(r2) ? 0.0 : y;
-      const double q = sc[3][e];
-      const double qr3 = (q * y) * (y * y);
-      phi = fma(q, y, phi);
-      ex = fma(qr3, dx, ex); ey = fma(qr3, dy, ey); ez = fma(qr3, dz, ez);
+      const double4 c4 = sc[e];
+#pragma unroll
+      for (int u = 0; u < kChargePpt; ++u) {
+        double dx = px[u] - c4.x, dy = py[u] - c4.y, dz = pz[u] - c4.z;
+        double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        // 1/r: MUFU.RSQ64H seed + one cubic step; a charge exactly at the point is skipped.  The clamp
+        // and the r = 0 test are integer operations on the bit pattern: 18 FP64-pipe operations per pair (27 flop)
+        double y = rsqrt_pos(clamp_tiny(r2));
+        y = is_zero(r2) ? 0.0 : y;
+        const double qr3 = (c4.w * y) * (y * y);
+        phi[u] = fma(c4.w, y, phi[u]);
+        ex[u] = fma(qr3, dx, ex[u]); ey[u] = fma(qr3, dy, ey[u]); ez[u] = fma(qr3, dz, ez[u]);
+      }
     }
   }
-  if (p < m) {
-    double* o = partial + (int64_t)blockIdx.y * 4 * m;
-    o[p] = phi; o[m + p] = ex; o[2 * m + p] = ey; o[3 * m + p] = ez;
+  double* o = partial + (int64_t)blockIdx.y * 4 * m;
+#pragma unroll
+  for (int u = 0; u < kChargePpt; ++u) {
+    const int64_t p = p0 + u * kThreads;
+    if (p < m) { o[p] = phi[u]; o[m + p] = ex[u]; o[2 * m + p] = ey[u]; o[3 * m + p] = ez[u]; }
   }
 }
 
@@ -368,7 +382,13 @@ __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const d
                                                             const double* __restrict__ normal,
                                                             const int32_t* __restrict__ bc_kind,
                                                             const double* __restrict__ diag, double* __restrict__ K,
-                                                            int64_t ld, unsigned long long* __restrict__ rowmax_bits) {
+                                                            int64_t ld, unsigned long long* __restrict__ rowmax_bits,
+                                                            int world, int rank) {
+  // distributed matrix (neb_dist.cu): this context holds the 256-column blocks g = rank, rank + world, ... side by side;
+  // grid.y counts LOCAL 64-column tiles, lt -> global tile gt, and K is shifted so that column j lands in its local slot
+  const int64_t lt = blockIdx.y, gt = ((lt >> 2) * world + rank) * 4 + (lt & 3);
+  if (gt * kTile >= (int64_t)g.n_rect + g.n_tri + g.n_wire) return;
+  K += (lt - gt) * kTile * ld;
   __shared__ TileSmem sm;
   tile_pipe_init(sm);
   load_images(sm, img, n_img);
@@ -382,11 +402,19 @@ __global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const d
   sink.dielectric = bc_kind[ic] == NEB_BC_DIELECTRIC;
   sink.diag = diag[ic];
   double px = colloc[ic], py = colloc[stride + ic], pz = colloc[2 * stride + ic];
-  int64_t j0 = (int64_t)blockIdx.y * kTile, j1 = min(n, j0 + kTile);
+  int64_t j0 = gt * kTile, j1 = min(n, j0 + kTile);
   process_range<M, FIRST>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
   // the running maximum of a row whose coefficients are still being summed is not the row's maximum: with several
   // chunks of copies only the LAST chunk's values (the finished coefficients) count
   if (i < n && rowmax_bits) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
+}
+
+// distributed layout: rows n..npad of every local column, and the local columns whose global index is >= n
+__global__ void pad_identity_dist_kernel(double* K, int64_t n, int64_t npad, int64_t ncol_loc, int world, int rank) {
+  const int64_t lc = blockIdx.y, gc = ((lc >> 8) * world + rank) * 256 + (lc & 255);
+  const int64_t i0 = gc >= n ? 0 : n;
+  for (int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < npad; i += (int64_t)gridDim.x * blockDim.x)
+    K[i + lc * npad] = (i == gc) ? 1.0 : 0.0;
 }
 
 // rows/columns >= n of the padded matrix: identity
@@ -405,11 +433,13 @@ __global__ void pad_identity_kernel(double* K, int64_t n, int64_t npad) {
   }
 }
 
-__global__ void rscale_kernel(const unsigned long long* rowmax_bits, int64_t n, int64_t npad, double* rscale) {
+// dist: a row with no non-zero entry in THIS rank's columns gets +inf, so that the minimum over the ranks (= 1 / the
+// row's maximum over all columns) ignores it; neb_dist_row_scales turns a surviving +inf into 1
+__global__ void rscale_kernel(const unsigned long long* rowmax_bits, int64_t n, int64_t npad, double* rscale, bool dist) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
   double mx = (i < n) ? __longlong_as_double((long long)rowmax_bits[i]) : 1.0;
-  rscale[i] = (mx > 0.0) ? 1.0 / mx : 1.0;
+  rscale[i] = (mx > 0.0) ? 1.0 / mx : (dist ? __longlong_as_double(0x7ff0000000000000LL) : 1.0);
 }
 
 __global__ void scale_rows_kernel(double* K, int64_t n, int64_t ld, const double* __restrict__ rscale) {
@@ -511,7 +541,7 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
   }
   if (sq) {
     StageTimer t(c, NEB_STAGE_CHARGES);
-    dim3 grid((unsigned)pt_blocks, (unsigned)sq);
+    dim3 grid((unsigned)((m + kThreads * kChargePpt - 1) / (kThreads * kChargePpt)), (unsigned)sq);
     charge_kernel<<<grid, kThreads, 0, c->stream>>>(c->d_charges, c->q, c->q_cap, d_pts, m, per_q,
                                                     partial + (size_t)se * 4 * m);
     c->launches++;
@@ -534,19 +564,20 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
 
 neb_status assemble_matrix(neb_ctx* c) {
   int64_t n = c->n, npad = c->npad;
-  c->counter[NEB_COUNTER_MATRIX_BYTES] = 8.0 * (double)n * (double)n;
+  c->counter[NEB_COUNTER_MATRIX_BYTES] = 8.0 * (double)n * (double)(c->dist_mode ? std::min(c->ncol_loc, n) : n);
   NEB_TRY(ensure_scratch(c, (size_t)npad * sizeof(unsigned long long)));
   unsigned long long* rowmax = (unsigned long long*)c->d_scratch;
   NEB_CUDA(c, cudaMemsetAsync(rowmax, 0, (size_t)npad * sizeof(unsigned long long), c->stream));
   {
     StageTimer t(c, NEB_STAGE_ASSEMBLE);
-    dim3 grid((unsigned)((n + kThreads - 1) / kThreads), (unsigned)((n + kTile - 1) / kTile));
+    const bool dist = c->dist_mode != 0;
+    dim3 grid((unsigned)((n + kThreads - 1) / kThreads), (unsigned)(dist ? c->ncol_loc / kTile : (n + kTile - 1) / kTile));
     const int n_chunks = (c->n_img + kMaxImg - 1) / kMaxImg;
     for (int ch = 0; ch < n_chunks; ++ch) {
       const int len = std::min(kMaxImg, c->n_img - ch * kMaxImg);
       const double* img = c->d_img + (size_t)ch * 3 * kMaxImg;
       unsigned long long* rm = (ch == n_chunks - 1) ? rowmax : nullptr;      // row maxima from the finished coefficients
-#define NEB_ASM_ARGS tables(c), img, len, c->d_colloc, c->stride, c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rm
+#define NEB_ASM_ARGS tables(c), img, len, c->d_colloc, c->stride, c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rm, c->dist_world, c->dist_rank
       if (c->math_fast) {
         if (ch == 0) assemble_kernel<MathFast, true><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
         else assemble_kernel<MathFast, false><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
@@ -559,7 +590,11 @@ neb_status assemble_matrix(neb_ctx* c) {
     }
     NEB_CUDA(c, cudaGetLastError());
     int64_t padcells = (npad - n) * npad + n * (npad - n);
-    if (padcells > 0) {
+    if (dist) {
+      pad_identity_dist_kernel<<<dim3(4, (unsigned)c->ncol_loc), 256, 0, c->stream>>>(c->d_K, n, npad, c->ncol_loc, c->dist_world, c->dist_rank);
+      c->launches++;
+      NEB_CUDA(c, cudaGetLastError());
+    } else if (padcells > 0) {
       pad_identity_kernel<<<(unsigned)((padcells + 255) / 256), 256, 0, c->stream>>>(c->d_K, n, npad);
       c->launches++;
       NEB_CUDA(c, cudaGetLastError());
@@ -567,7 +602,7 @@ neb_status assemble_matrix(neb_ctx* c) {
   }
   {
     StageTimer t(c, NEB_STAGE_EQUIL);
-    rscale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(rowmax, n, npad, c->d_rscale);
+    rscale_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(rowmax, n, npad, c->d_rscale, c->dist_mode != 0);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }
@@ -578,7 +613,7 @@ neb_status assemble_matrix(neb_ctx* c) {
 // returns the unscaled matrix without a second copy).
 neb_status scale_matrix_rows(neb_ctx* c) {
   StageTimer t(c, NEB_STAGE_EQUIL);
-  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)c->n);
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)(c->dist_mode ? c->ncol_loc : c->n));   // pad columns are zero above row n
   scale_rows_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, c->n, c->npad, c->d_rscale);
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());

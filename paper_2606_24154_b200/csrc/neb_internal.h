@@ -14,6 +14,7 @@ constexpr double kCoulomb = 1.0 / (4.0 * 3.14159265358979323846 * kEps0);
 constexpr int kRec = 20;                                   // doubles per frame-table record
 constexpr int kPad = 128;                                  // matrix dimension is padded to a multiple of this
 #define NEB_IMG_CHUNK 32                                   // periodic copies per kernel launch (shared-memory table)
+constexpr int kDistBlock = 256;                            // columns per block of the distributed factorisation (neb_dist.cu)
 constexpr int kMaxImages = 16384;                          // copies per element accepted by neb_assemble
 
 // Frame tables (a1), elements sorted by kind: [rect | tri | wire].  SoA, field-major:
@@ -57,6 +58,12 @@ struct neb_ctx {
   int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
   int eval_splits = 0;  // 0: element/charge chunks chosen from the point count; k: always k chunks (shard-invariant bits)
 
+  // scale-out of the solve (neb_dist.cu): 256-column blocks dealt cyclically to dist_world contexts; 1 = not distributed
+  int dist_world = 1, dist_rank = 0;
+  int dist_mode = 0;              // set by neb_dist_configure (world = 1 allowed: the same code on one context)
+  bool dist_scaled = false;       // the agreed row scales have been applied (neb_dist_row_scales)
+  int64_t ncol_loc = 0;           // columns of d_K held here (npad when not distributed)
+
   // geometry
   int64_t n = 0, npad = 0, stride = 0;
   int32_t n_rect = 0, n_tri = 0, n_wire = 0, n_img = 0;
@@ -75,7 +82,7 @@ struct neb_ctx {
   int32_t* d_flag = nullptr;      // device error flags (validation, singular pivot)
 
   // matrix / factors
-  double* d_K = nullptr;          // npad x npad column-major
+  double* d_K = nullptr;          // npad x ncol_loc column-major
   double* d_rscale = nullptr;     // npad
   int32_t* d_ipiv = nullptr;      // npad (0-based absolute row)
   int32_t* d_rowperm = nullptr;   // npad: composed row permutation of the factorisation
@@ -124,6 +131,8 @@ neb_status fail(neb_ctx* c, neb_status st, const std::string& msg);
   } while (0)
 
 neb_status ensure_scratch(neb_ctx* c, size_t bytes);
+bool is_device_pointer(const void* p);
+int64_t dist_local_cols(int64_t npad, int world, int rank);   // neb_dist.cu: columns of the matrix a rank holds
 
 struct StageTimer {   // records device time of a stage when profiling is on
   neb_ctx* c;
@@ -140,6 +149,7 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
 neb_status assemble_matrix(neb_ctx* c);   // a3 + S15 row scales (computed, not yet applied)
 neb_status scale_matrix_rows(neb_ctx* c); // applies the row scales in place
 neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
+neb_status finish_sigma(neb_ctx* c, const double* d_x);   // solved values (sorted order) -> d_sigma (caller order) and the table weights
 
 // neb_lu.cu ---------------------------------------------------------------------------------------
 neb_status lu_init_device(neb_ctx* c);    // per-device kernel attributes (dynamic shared memory, cluster size); from neb_create
@@ -148,11 +158,17 @@ neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-sc
 neb_status lu_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
 neb_status trisolve_init_device(neb_ctx* c);
 size_t lu_panel_ws_bytes(int num_sms);
+// launch wrappers of the LU update kernels (A: column-major with leading dimension ld; Lp/ldl: the L operand, row index absolute)
+void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi);
+void lu_launch_trsm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int64_t c_first, int64_t ncols);
+void lu_launch_gemm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int K, int64_t r0, int64_t m,
+                    int64_t c_first, int64_t ncols, bool timed);
+neb_status lu_finish_factors(neb_ctx* c);   // rowperm from ipiv
 
 // neb_lu_cluster.cu: panel factorisation on one thread-block cluster (panels of <= 16 x 512 rows)
 int panel_cluster_probe();
 int64_t panel_cluster_max_rows(neb_ctx* c);
-neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream);
+neb_status panel_cluster_launch(neb_ctx* c, double* A, int64_t k, cudaStream_t stream);
 
 // neb_fastvol.cu (device pointers only; the ABI wrappers in neb_api.cu stage host arrays) --------------
 neb_status fastvol_build(neb_ctx* c, int slot, int nx, int ny, int nz, const double* origin, const double* spacing, bool with_charges);

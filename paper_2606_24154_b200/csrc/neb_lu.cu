@@ -200,7 +200,10 @@ __global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, cons
 constexpr int TRSM_THREADS = NB;
 constexpr int TRSM_LD = 2 * NB;
 constexpr size_t TRSM_SMEM = (size_t)NB * TRSM_LD * sizeof(double);
-__global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int64_t c_first) {
+// L11 is read from Lp: Lp[i + j * ldl] = element (absolute row i, panel column j); on one GPU Lp = A + k * ld, in the
+// distributed factorisation (neb_dist.cu) it is the broadcast panel.
+__global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__ A, int64_t ld, const double* __restrict__ Lp, int64_t ldl,
+                                                            int64_t k, int64_t c_first) {
   extern __shared__ __align__(16) double s_trsm[];             // s_trsm[j * TRSM_LD + i] = L11[i][j], 0 for i >= NB
   const int tid = threadIdx.x;
   double* col = A + k + (c_first + (int64_t)blockIdx.x * NB + tid) * ld;
@@ -208,7 +211,7 @@ __global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__
   {
     // thread j stages column j of L11: 32 independent 16-byte loads in flight (a rolled element loop over 64
     // threads would pay one L2 round trip per element)
-    const double* lcol = A + k + (k + tid) * ld;
+    const double* lcol = Lp + k + tid * ldl;
 #pragma unroll
     for (int i = 0; i < NB; i += 2) {
       const double2 v = *reinterpret_cast<const double2*>(lcol + i);
@@ -245,7 +248,9 @@ __global__ void __launch_bounds__(TRSM_THREADS) trsm_kernel(double* __restrict__
 
 // ------------------------------------------------------------------------------------------------
 // Trailing update C -= L * U on the FP64 tensor cores, any depth K (a multiple of 32):
-//   C = A[r0 .. r0+m, c_first ..],  L = A[r0 .. r0+m, k .. k+K),  U = A[k .. k+K, c_first ..].
+//   C = A[r0 .. r0+m, c_first ..],  L = A[r0 .. r0+m, k .. k+K),  U = A[k .. k+K, c_first ..];
+//   L is read through Lp (Lp[i + kk * ldl] = L[i][kk], absolute row i): A + k * ld on one GPU, the broadcast panel in
+//   the distributed factorisation (neb_dist.cu).
 // CTA tile 128 (rows) x 64 (cols), 8 warps as 4 (rows) x 2 (cols), warp tile 32 x 32 = 4 x 4 DMMA tiles
 // (mma.sync.m8n8k4.f64).  The accumulators start from C and stay in registers over the whole K loop; L and U
 // arrive in chunks of 32 k through a two-stage cp.async pipeline (the next chunk loads while this one is
@@ -274,8 +279,8 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, int64_t k, int K, int64_t r0,
-                                                               int64_t m, int64_t c_first) {
+__global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, const double* __restrict__ Lp, int64_t ldl,
+                                                               int64_t k, int K, int64_t r0, int64_t m, int64_t c_first) {
   extern __shared__ __align__(16) double smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t i0 = r0 + (int64_t)blockIdx.x * GM;       // first row of the tile
@@ -289,7 +294,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restric
     const int64_t kc = k + (int64_t)ch * GKC;
     for (int idx = tid; idx < GKC * (GM / 2); idx += GEMM_THREADS) {     // 32 k-columns x 64 16-byte chunks
       const int kk = idx / (GM / 2), c2 = idx % (GM / 2);
-      if (2 * c2 < rows_here) cp_async16(sL + kk * LDL + 2 * c2, A + (i0 + 2 * c2) + (kc + kk) * ld);
+      if (2 * c2 < rows_here) cp_async16(sL + kk * LDL + 2 * c2, Lp + (i0 + 2 * c2) + ((int64_t)ch * GKC + kk) * ldl);
     }
     for (int idx = tid; idx < GN * (GKC / 2); idx += GEMM_THREADS) {     // 64 columns x 16 chunks
       const int j = idx / (GKC / 2), c2 = idx % (GKC / 2);
@@ -437,6 +442,50 @@ neb_status lu_init_device(neb_ctx* c) {
   return trisolve_init_device(c);
 }
 
+// Launch wrappers of the update kernels: used by lu_factor below and by the distributed factorisation (neb_dist.cu),
+// where A is a rank's local block of columns and the L operand (Lp, ldl) is the broadcast panel.
+void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo,
+                     int64_t skip_hi) {
+  const int64_t ncols = (c_hi - c_lo) - (skip_hi - skip_lo);
+  if (ncols <= 0) return;
+  laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, st>>>(A, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
+  c->launches++;
+}
+
+void lu_launch_trsm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int64_t c_first,
+                    int64_t ncols) {
+  if (ncols <= 0) return;
+  trsm_kernel<<<(unsigned)(ncols / NB), TRSM_THREADS, TRSM_SMEM, st>>>(A, ld, Lp, ldl, k, c_first);
+  c->launches++;
+}
+
+void lu_launch_gemm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int K, int64_t r0,
+                    int64_t m, int64_t c_first, int64_t ncols, bool timed) {
+  if (m <= 0 || ncols <= 0) return;
+  c->counter[NEB_COUNTER_GEMM_FLOP] += 2.0 * (double)m * (double)ncols * (double)K;
+  dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
+  if (timed) {
+    StageTimer tg(c, NEB_STAGE_LU_GEMM);
+    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first);
+  } else {
+    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first);
+  }
+  c->launches++;
+}
+
+// rowperm (the composed row permutation) from ipiv, for the solves
+neb_status lu_finish_factors(neb_ctx* c) {
+  const int64_t npad = c->npad;
+  if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
+    compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * sizeof(unsigned), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+  } else {
+    compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+  }
+  c->launches++;
+  NEB_CUDA(c, cudaGetLastError());
+  return NEB_OK;
+}
+
 neb_status lu_factor(neb_ctx* c) {
   const int64_t npad = c->npad, ld = c->npad;
   StageTimer tt(c, NEB_STAGE_LU);
@@ -452,7 +501,7 @@ neb_status lu_factor(neb_ctx* c) {
   // panel k on stream st: the cluster kernel where the panel fits, else the grid-wide cooperative kernel
   auto launch_panel = [&](int64_t k, cudaStream_t st) -> neb_status {
     const int64_t mrows = npad - k;
-    if (mrows <= cluster_rows) return panel_cluster_launch(c, k, st);
+    if (mrows <= cluster_rows) return panel_cluster_launch(c, c->d_K, k, st);
     // rows per CTA: multiple of 32, at most 200 KB of shared memory (390 rows -> 384)
     int G = (int)min((int64_t)c->num_sms, (mrows + 63) / 64);
     int mc = (int)((mrows + G - 1) / G);
@@ -472,29 +521,15 @@ neb_status lu_factor(neb_ctx* c) {
   };
   // row exchanges of panel k on the columns [c_lo, c_hi) \ [skip_lo, skip_hi)
   auto laswp = [&](cudaStream_t st, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
-    const int64_t ncols = (c_hi - c_lo) - (skip_hi - skip_lo);
-    if (ncols <= 0) return;
-    laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, st>>>(c->d_K, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
-    c->launches++;
+    lu_launch_laswp(c, st, c->d_K, ld, k, c_lo, c_hi, skip_lo, skip_hi);
   };
   // C[r0 .. r0+m, c_first .. c_first+ncols) -= A[r0 .., k .. k+K) * A[k .. k+K, c_first ..) on the tensor cores
   const bool timed = !c->lu_lookahead;
   auto gemm = [&](cudaStream_t st, int64_t k, int K, int64_t r0, int64_t m, int64_t c_first, int64_t ncols) {
-    if (m <= 0 || ncols <= 0) return;
-    c->counter[NEB_COUNTER_GEMM_FLOP] += 2.0 * (double)m * (double)ncols * (double)K;
-    dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
-    if (timed) {
-      StageTimer tg(c, NEB_STAGE_LU_GEMM);
-      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(c->d_K, ld, k, K, r0, m, c_first);
-    } else {
-      gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(c->d_K, ld, k, K, r0, m, c_first);
-    }
-    c->launches++;
+    lu_launch_gemm(c, st, c->d_K, ld, c->d_K + k * ld, ld, k, K, r0, m, c_first, ncols, timed);
   };
   auto trsm = [&](cudaStream_t st, int64_t k, int64_t c_first, int64_t ncols) {
-    if (ncols <= 0) return;
-    trsm_kernel<<<(unsigned)(ncols / NB), TRSM_THREADS, TRSM_SMEM, st>>>(c->d_K, ld, k, c_first);
-    c->launches++;
+    lu_launch_trsm(c, st, c->d_K, ld, c->d_K + k * ld, ld, k, c_first, ncols);
   };
 
   // Two-level right-looking factorisation.  Outer blocks of OB = 256 columns = 4 panels of 64:
@@ -553,12 +588,7 @@ neb_status lu_factor(neb_ctx* c) {
     kb = nb;
   }
   // composed permutation for the solves
-  if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
-    compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * sizeof(unsigned), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
-  } else {
-    compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
-  }
-  c->launches++;
+  NEB_TRY(lu_finish_factors(c));
   {
     const int nblk = (int)(npad / NB);
     diag_inv_kernel<<<dim3(nblk, 2), NB, 2 * NB * (NB + 1) * sizeof(double), c->stream>>>(c->d_K, ld, c->d_dinv, nblk);

@@ -470,7 +470,7 @@ int panel_cluster_probe() {
 int64_t panel_cluster_max_rows(neb_ctx* c) { return (int64_t)c->cluster_max_ctas * PS_THREADS * 32; }
 
 template <int R, int W>
-static cudaError_t ps_launch(neb_ctx* c, int cs, int64_t k, cudaStream_t stream) {
+static cudaError_t ps_launch(neb_ctx* c, double* A, int cs, int64_t k, cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(cs);
   cfg.blockDim = dim3(PS_THREADS);
@@ -481,17 +481,19 @@ static cudaError_t ps_launch(neb_ctx* c, int cs, int64_t k, cudaStream_t stream)
   at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, panel_stream_kernel<R, W>, c->d_K, c->npad, c->npad, k, c->d_ipiv, c->d_flag);
+  return cudaLaunchKernelEx(&cfg, panel_stream_kernel<R, W>, A, c->npad, c->npad, k, c->d_ipiv, c->d_flag);
 }
 
-neb_status panel_cluster_launch(neb_ctx* c, int64_t k, cudaStream_t stream) {
+// A: base such that the panel's columns are A + (k .. k+63) * npad (c->d_K on one GPU; a rank's local block shifted to
+// its global column position in the distributed factorisation)
+neb_status panel_cluster_launch(neb_ctx* c, double* A, int64_t k, cudaStream_t stream) {
   const int64_t mrows = c->npad - k;
   int cs = 1;
   while (cs < c->cluster_max_ctas && (int64_t)cs * PS_THREADS < mrows) cs <<= 1;
   const int64_t per_thread = (mrows + (int64_t)cs * PS_THREADS - 1) / ((int64_t)cs * PS_THREADS);
   cudaError_t e = cudaErrorInvalidValue;
   bool launched = false;
-#define X(R, W) if (!launched && per_thread <= R) { e = ps_launch<R, W>(c, cs, k, stream); launched = true; }
+#define X(R, W) if (!launched && per_thread <= R) { e = ps_launch<R, W>(c, A, cs, k, stream); launched = true; }
   NEB_PS_VARIANTS(X)
 #undef X
   if (!launched) return fail(c, NEB_EINVAL, "LU panel: more than 32 rows per thread of the cluster (n too large for this device)");

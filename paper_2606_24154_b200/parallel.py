@@ -1,7 +1,8 @@
 """Multi-GPU plumbing: one process per GPU, torch.distributed.
 
 The path shards over evaluation points (a7/a8) and over matrix columns (a3) with replicated element
-tables and NO data-path collective; the LU does not shard (replicas only).  What is left for the host
+tables and NO data-path collective; the LU runs as replicas, or — for matrices beyond one GPU, SURVEY §8(f).4 —
+block-cyclic over the ranks with the exchanges of DistSolver below.  What is left for the host
 side is: which slab of points a rank owns, the max-over-ranks of a device time, — if the caller
 wants the field on every rank — one all-gather of the outputs, and the per-step all-gather of the pushed charge
 positions of the space-charge loop (c4_step_sharded).  These helpers hold no arithmetic of the
@@ -91,3 +92,165 @@ def eval_sharded(nb, pts: torch.Tensor, gather: bool = True):
     if gather:
         return all_gather_points(phi, m, ALIGN), all_gather_points(E, m, ALIGN)
     return phi, E
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Scale-out of the solve: 1-D block-cyclic LU over the ranks.  The library (neb_dist_* in include/neb.h)
+# does the arithmetic; this class owns the buffers that travel and issues the exchanges between the library's steps.
+# ---------------------------------------------------------------------------------------------------------------
+DIST_BLOCK = 256
+
+
+def dist_owner(g: int, world: int) -> int:
+    """Rank that holds column block g (256 columns) of the block-cyclic matrix."""
+    return g % world
+
+
+def dist_local_blocks(n_blocks: int, world: int, rank: int):
+    """Global indices of the column blocks a rank holds, in their local order."""
+    return list(range(rank, n_blocks, world))
+
+
+def _group():
+    on = dist.is_available() and dist.is_initialized()
+    return (dist.get_world_size(), dist.get_rank()) if on else (1, 0)
+
+
+def _via_host(t: torch.Tensor) -> bool:
+    return t.is_cuda and dist.get_backend() == "gloo"      # CPU-only backend (the tests): stage through the host
+
+
+def _broadcast(t: torch.Tensor, src: int):
+    world, rank = _group()
+    if world == 1:
+        return
+    if _via_host(t):
+        h = t.cpu()
+        dist.broadcast(h, src)
+        if rank != src:
+            t.copy_(h)
+    else:
+        dist.broadcast(t, src)
+
+
+def _all_reduce(t: torch.Tensor, op):
+    world, _ = _group()
+    if world == 1:
+        return
+    if _via_host(t):
+        h = t.cpu()
+        dist.all_reduce(h, op=op)
+        t.copy_(h)
+    else:
+        dist.all_reduce(t, op=op)
+
+
+class _HostStream:
+    """Stream stand-in for a CPU device (the gloo test of the exchange protocol): everything is in order already."""
+    cuda_stream = 0
+
+    def wait_stream(self, other):
+        pass
+
+    def wait_event(self, ev):
+        pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        return False
+
+
+class _HostEvent:
+    def record(self, stream):
+        pass
+
+
+class DistSolver:
+    """Assemble + LU + solve of ONE system spread over the ranks of the default process group (one process per GPU).
+
+        nb = Neb(local_rank); ds = DistSolver(nb); ds.assemble(problem); ds.factor(); sigma = ds.solve()
+
+    Every rank calls the same methods in the same order and ends with the same sigma and a context that evaluates
+    fields as a replica (eval_sharded).  Exchanges per system: one MIN of the row scales (8 npad bytes), one broadcast
+    per 256-column block ((npad - 256 g) x 2 KB + 1 KB of pivots; overlapped with the trailing update when
+    lookahead is on), and per solve 2 npad/256 sums of 256 doubles plus one sum of the solution vector."""
+
+    def __init__(self, nb, lookahead: bool = True):
+        self.nb = nb
+        self.world, self.rank = _group()
+        self.lookahead = lookahead
+        nb.dist_configure(self.rank, self.world)
+        # a context is bound to a CUDA device; the CPU stand-in of the gloo test names its own
+        self.dev = getattr(nb, "torch_device", None) or torch.device("cuda", nb.device)
+        self.npad = 0
+
+    def assemble(self, pr):
+        nb = self.nb
+        nb.assemble_problem(pr)
+        self.npad = nb.dist_npad()
+        self.n_blocks = self.npad // DIST_BLOCK
+        f64 = dict(dtype=torch.float64, device=self.dev)
+        scales = torch.empty(self.npad, **f64)
+        nb.dist_row_scales(scales, False)
+        _all_reduce(scales, dist.ReduceOp.MIN)              # 1 / (row maximum over ALL columns): reading S15
+        nb.dist_row_scales(scales, True)
+        self.panel = [torch.empty(self.npad * DIST_BLOCK, **f64) for _ in range(2)]
+        self.piv = [torch.empty(DIST_BLOCK, dtype=torch.int32, device=self.dev) for _ in range(2)]
+        self.y = torch.empty(self.npad, **f64)
+        self.acc = torch.empty(self.npad, **f64)
+
+    def factor(self):
+        """The block loop.  Buffer b = g % 2 carries block g; with lookahead the owner of block g + 1 updates that block
+        first, factors it on the side stream and the broadcast of g + 1 is issued there, beside the trailing update of g."""
+        nb, world, rank, B = self.nb, self.world, self.rank, DIST_BLOCK
+        main = torch.cuda.current_stream(self.dev) if self.dev.type == "cuda" else _HostStream()
+        side = torch.cuda.Stream(self.dev, priority=-1) if (self.lookahead and self.dev.type == "cuda") else main
+        new_event = torch.cuda.Event if self.dev.type == "cuda" else _HostEvent
+        applied = [None, None]                              # event: the update that read buffer b has run (main stream)
+        if dist_owner(0, world) == rank:
+            side.wait_stream(main)
+            nb.dist_factor_block(0, self.panel[0], self.piv[0], stream=side)
+        for g in range(self.n_blocks):
+            b = g % 2
+            rows = self.npad - g * B
+            if applied[b] is not None:                      # update g - 2 read this buffer: it must be done before the
+                side.wait_event(applied[b])                 # broadcast of block g overwrites it
+            with (torch.cuda.stream(side) if self.dev.type == "cuda" else _HostStream()):
+                _broadcast(self.panel[b][: rows * B], dist_owner(g, world))
+                _broadcast(self.piv[b], dist_owner(g, world))
+            main.wait_stream(side)
+            nxt = g + 1
+            if nxt < self.n_blocks and dist_owner(nxt, world) == rank:
+                nb.dist_apply_block(g, self.panel[b], self.piv[b], part=1)
+                side.wait_stream(main)                      # block g + 1 is up to date, update g - 1 has released its buffer
+                nb.dist_factor_block(nxt, self.panel[nxt % 2], self.piv[nxt % 2], stream=side)
+                nb.dist_apply_block(g, self.panel[b], self.piv[b], part=2)
+            else:
+                nb.dist_apply_block(g, self.panel[b], self.piv[b], part=0)
+            applied[b] = new_event()
+            applied[b].record(main)
+        main.wait_stream(side)
+        flag = torch.tensor([nb.dist_finish_factor()], dtype=torch.int32, device=self.dev)
+        _all_reduce(flag, dist.ReduceOp.MAX)
+        if int(flag.item()):
+            raise RuntimeError("NEB_ESINGULAR: zero or NaN pivot in the distributed factorisation")
+
+    def solve(self, out=None):
+        """Right-hand side (with the space charges the context holds) -> sigma (n) on every rank, on the resident factors."""
+        nb, world, rank, B = self.nb, self.world, self.rank, DIST_BLOCK
+        nb.dist_rhs(self.y)
+        for upper in (False, True):
+            self.acc.zero_()
+            order = range(self.n_blocks - 1, -1, -1) if upper else range(self.n_blocks)
+            for g in order:
+                _all_reduce(self.acc[g * B:(g + 1) * B], dist.ReduceOp.SUM)
+                nb.dist_tri_block(upper, g, self.y, self.acc)
+        mine = (torch.arange(self.n_blocks, device=self.dev) % world == rank)[:, None]
+        x = torch.where(mine, self.y.view(self.n_blocks, B), torch.zeros((), dtype=torch.float64, device=self.dev)).reshape(-1).contiguous()
+        _all_reduce(x, dist.ReduceOp.SUM)
+        if out is None:
+            out = torch.empty(nb.n, dtype=torch.float64, device=self.dev)
+        nb.dist_set_solution(x, out)
+        return out

@@ -1001,3 +1001,114 @@ def test_two_ranks_real_library():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res == [(0, True), (1, True)]
+
+
+# ---------------------------------------------------------------------------------------------
+# scale-out of the solve — block-cyclic LU through the neb_dist_* calls (include/neb.h) and
+# parallel.DistSolver.  (a) one context, world = 1: the same code path against the oracle and against neb_solve;
+# (b) two ranks sharing this GPU (gloo: every exchange runs on the host, no kernel waits on another rank's kernel),
+# each holding only ITS column blocks, against the single-GPU sigma of the same system.
+# ---------------------------------------------------------------------------------------------
+def _dist_problem(which):
+    if which == "mixed":                 # rectangles + right triangles, dielectric rows
+        return W.thgem(d=20, n_plane=20, n_grid=10)
+    return W.cube(n_side=20)             # N = 2400
+
+
+def test_dist_lu_one_context_against_oracle_and_solve(P):
+    import torch
+    from paper_2606_24154_b200 import parallel
+    import oracle as orc
+    pr = W.random_elements(700, seed=21, kinds=(W.RECT, W.TRI), dielectric_fraction=0.3, size_mm=(0.5, 1.5), box_mm=10.0)
+    ref = P.Neb()
+    ref.assemble_problem(pr)
+    sig_ref = ref.solve()
+    ref.close()
+    nb = P.Neb()
+    ds = parallel.DistSolver(nb)                     # no process group: world = 1
+    ds.assemble(pr)
+    assert nb.dist_npad() == 768 and nb.dist_npad() % P.binding.NEB_DIST_BLOCK == 0
+    with pytest.raises(P.NebError):
+        nb.solve()                                   # NEB_ESTATE on a distributed context
+    ds.factor()
+    sig = ds.solve().cpu().numpy()
+    g = orc.Geometry(pr)
+    so = orc.solve(orc.assemble(g), orc.rhs(g))
+    assert np.max(np.abs(sig - so)) <= TOL_SIGMA * np.max(np.abs(so))
+    assert np.max(np.abs(sig - sig_ref)) <= TOL_SIGMA * np.max(np.abs(sig_ref))
+    # a new right-hand side on the resident factors (space charge), and the context evaluates as usual
+    rs = np.random.RandomState(5)
+    pos, q = rs.uniform(-8e-3, 8e-3, size=(3, 300)), np.full(300, W.Q_E * 1e6)
+    nb.add_space_charge(pos, q)
+    sig2 = ds.solve().cpu().numpy()
+    so2 = orc.solve(orc.assemble(g), orc.rhs(g, pos, q))
+    assert np.max(np.abs(sig2 - so2)) <= TOL_SIGMA * np.max(np.abs(so2))
+    pts = rs.uniform(-12e-3, 12e-3, size=(3, 200))
+    phi, E = nb.eval(pts)
+    phi_o, E_o, scale = truth(orc, g, sig2, pts, pos, q)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "dist one context", scale)
+    nb.close()
+
+
+def _dist_rank_worker(rank, world, port, out_q):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_24154_b200 as P
+    from paper_2606_24154_b200 import parallel
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        res = {}
+        for which in ("mixed", "cube"):
+            pr = _dist_problem(which)
+            for lookahead in (True, False):
+                nb = P.Neb(0)
+                ds = parallel.DistSolver(nb, lookahead=lookahead)
+                ds.assemble(pr)
+                ds.factor()
+                sig = ds.solve().cpu().numpy()
+                res[(which, lookahead)] = sig
+                if lookahead:
+                    pts = torch.from_numpy(pr.points[:, :1000].copy()).cuda()
+                    phi, E = parallel.eval_sharded(nb, pts, gather=True)          # the replicas evaluate their slabs
+                    res[(which, "phi")] = phi.cpu().numpy()
+                nb.close()
+            if rank == 0:
+                one = P.Neb(0)
+                one.assemble_problem(pr)
+                res[(which, "single")] = one.solve()
+                phi1, _ = one.eval(pr.points[:, :1000])
+                res[(which, "phi1")] = phi1
+                one.close()
+        out_q.put((rank, res))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_dist_lu_two_ranks_real_library():
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out_q = ctx.Queue()
+    procs = [ctx.Process(target=_dist_rank_worker, args=(r, 2, port, out_q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict(out_q.get(timeout=600) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for which in ("mixed", "cube"):
+        single = got[0][(which, "single")]
+        for la in (True, False):
+            a, b = got[0][(which, la)], got[1][(which, la)]
+            assert np.array_equal(a, b), "both ranks must end with the same sigma"
+            assert np.max(np.abs(a - single)) <= TOL_SIGMA * np.max(np.abs(single)), which
+        # with and without look-ahead the same operations run in the same order on every column: same bits
+        assert np.array_equal(got[0][(which, True)], got[0][(which, False)])
+        phi, phi1 = got[0][(which, "phi")], got[0][(which, "phi1")]
+        assert np.array_equal(phi, got[1][(which, "phi")])
+        assert np.max(np.abs(phi - phi1)) <= 1e-8 * np.max(np.abs(phi1))     # sigma differs by <= 1e-9 between the two solves
