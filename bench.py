@@ -364,6 +364,7 @@ class Runner:
             "traffic": self.traffic.get((self.name, "eval_kernel")), "kernel_ms": eval_ms, "flop_per_pair": fl,
             "fp64_instr_per_pair": inst, "fp64_pipe_slot_frac": inst * eval_pairs / (eval_ms * 1e-3) / (0.5e12 * dfma),
             "pairs_per_s_kernel": eval_pairs / (eval_ms * 1e-3), "field_map_points_per_s": self.m / (eval_ms * 1e-3),
+            "frac_of_3operand_dfma_peak": ach / self.peaks["dfma3"],
             "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process (nominal 148 SM x 64 DFMA/clk x "
                            "2 x 1.965 GHz = 37.2); MEASURED_PEAKS.json has no FP64 entry",
             "constants_source": "profiles/r2_opcounts.md (ncu smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on per pair)"}))
@@ -385,7 +386,7 @@ class Runner:
             out.append((stages["charges"], {
                 "bound": "alu", "kernel": "charge_kernel (a8)", "achieved": ach, "peak": dfma, "unit": "TFLOP/s", "frac": ach / dfma,
                 "traffic": self.traffic.get((self.name, "charge_kernel")), "kernel_ms": c_ms, "flop_per_pair": ops["charges"]["flop"],
-                "pairs_per_s_kernel": pairs / (c_ms * 1e-3),
+                "pairs_per_s_kernel": pairs / (c_ms * 1e-3), "frac_of_3operand_dfma_peak": ach / self.peaks["dfma3"],
                 "fp64_pipe_slot_frac": ops["charges"]["fp64_instr"] * pairs / (c_ms * 1e-3) / (0.5e12 * dfma)}))
         if stages.get("assemble"):
             a_ms = stages["assemble"]
@@ -421,14 +422,14 @@ class Runner:
 
 def measure_peaks(P, local):
     nb = P.Neb(local)
-    dfma, dmma = nb.fp64_peak(0), nb.fp64_peak(1)
+    dfma, dmma, dfma3, dfma2c = nb.fp64_peak(0), nb.fp64_peak(1), nb.fp64_peak(2), nb.fp64_peak(3)
     nb.close()
     try:
         mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         hbm, src, bf16 = mp["hbm_gbs"], "MEASURED_PEAKS.json hbm_gbs (measured copy rate)", mp.get("bf16_tflops", 1590.0)
     except Exception:
         hbm, src, bf16 = 6650.0, "fallback 6.65 TB/s of B200_PROFILING.md", 1590.0
-    return {"dfma": dfma, "dmma": dmma, "hbm": hbm, "hbm_source": src, "dmma_from_bf16": bf16 * 40.0 / 2250.0}
+    return {"dfma": dfma, "dmma": dmma, "dfma3": dfma3, "dfma2c": dfma2c, "hbm": hbm, "hbm_source": src, "dmma_from_bf16": bf16 * 40.0 / 2250.0}
 
 
 def extra_record(name, dev, P, ops, traffic, peaks, steps):
@@ -465,6 +466,8 @@ def main():
     ap.add_argument("--m-points", type=int, default=None, help="cap on the evaluation points (C3) / charges (C4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the full-size C3 step and the 10 C4 steps")
+    ap.add_argument("--set-option", action="append", default=[], metavar="ID=VALUE",
+                    help="neb_set_option(ID, VALUE) on the bench context before the first step (A/B runs of a library option)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -489,6 +492,9 @@ def main():
     name = args.workload
     pr = load_problem(name, args.m_points, seed_shift=rank)   # same geometry on every rank, its own points / charges
     rn = Runner(name, pr, dev, P, ops, traffic, peaks)
+    for kv in args.set_option:
+        k, v = kv.split("=")
+        rn.nb.set_option(int(k), int(v))
     if rn.is_c4:
         rn.prepare_c4()
 
@@ -523,7 +529,9 @@ def main():
             "gpu_launches": launches, "clocks": _clocks_summary(samples),
             "roofline": roofs[0], "roofline_second": roofs[1] if len(roofs) > 1 else None, "rooflines_other": roofs[2:],
             "stages_ms": stages, "lu": rn.lu_summary(stages, counters),
-            "peaks": {"fp64_dfma_tflops": peaks["dfma"], "fp64_dmma_tflops": peaks["dmma"], "hbm_gbs": peaks["hbm"],
+            "peaks": {"fp64_dfma_tflops": peaks["dfma"], "fp64_dmma_tflops": peaks["dmma"], "fp64_dfma_3operand_tflops": peaks["dfma3"],
+                      "fp64_dfma_2operand_const_tflops": peaks["dfma2c"],
+                      "hbm_gbs": peaks["hbm"],
                       "hbm_source": peaks["hbm_source"]},
         }
         if not args.no_cpu_baseline and world == 1:

@@ -58,6 +58,10 @@ enum {
                            the given number of points (few points -> many chunks); k > 0: always k chunks, so that the
                            fixed-order partial sums, hence the result BITS, do not depend on how many points a call
                            (or a rank of a sharded evaluation) is given                                          */
+  NEB_OPT_SOLVER = 6,   /* InvertMatrix: 0 (default) = OptLU, the blocked LU; 1 = OptSVD, one-sided Jacobi SVD and the
+                           minimum-norm least-squares solution (for meshes with coincident / overlapping panels, whose
+                           matrix is rank-deficient: the LU reports NEB_ESINGULAR there).  Read at the next factorisation
+                           (the first neb_solve after neb_assemble)                                              */
   NEB_OPT_LU_LOOKAHEAD = 4 /* 1 (default): panel k+1 is factored on an internal stream while the trailing
                            update of panel k runs (cluster panels only); 0: one stream, and
                            NEB_STAGE_LU_GEMM is then timed alone                                 */
@@ -195,6 +199,15 @@ neb_status neb_get_line_charges(neb_ctx* ctx, double* lines);
  * 3*q values, in place.  Stateless; pos and E must both be device or both be host pointers. */
 neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, double mu_dt);
 
+/* OptSVD (reading S31 of DESIGN.md).  With NEB_OPT_SOLVER = 1 neb_solve factorises the row-scaled matrix as
+ * K V = U diag(s) by one-sided Jacobi rotations (16 npad^2 bytes of device memory: K and V) and returns
+ * sigma = sum over s_j > rcond s_max of v_j (u_j . b) / s_j; neb_solve_weighting* and re-solves use the same factors.
+ * neb_set_svd_cutoff: rcond in [0, 1), default 1e-10.  neb_get_singular_values (test hook): the npad singular values
+ * in column order (the npad - n padding columns contribute exact ones), host or device, and the number of sweeps
+ * the factorisation took (host, may be NULL); NEB_ESTATE without SVD factors. */
+neb_status neb_set_svd_cutoff(neb_ctx* ctx, double rcond);
+neb_status neb_get_singular_values(neb_ctx* ctx, double* s_out, int32_t* sweeps);
+
 /* Scale-out of the solve (InvertMatrix with OptLU, Alg. 1, for a matrix spread over
  * several GPUs).  Right-looking block LU with partial pivoting on a matrix whose 256-column blocks are dealt
  * cyclically to `world` contexts, one per GPU, one process each: block g lives on rank g % world; every rank holds
@@ -260,7 +273,10 @@ neb_status neb_get_matrix_rows(neb_ctx* ctx, int64_t n_rows, const int32_t* rows
 neb_status neb_get_rhs(neb_ctx* ctx, double* b_out);
 
 /* Measurement aids: register-only FP64 microbenchmarks on all SMs.
- * kind 0: DFMA chains; kind 1: mma.sync m8n8k4 f64 (DMMA).  Result in TFLOP/s (FMA = 2 flop). */
+ * kind 0: DFMA chains; kind 1: mma.sync m8n8k4 f64 (DMMA); kind 2: independent DFMA whose three source operands are
+ * three different registers (what the FP64 pipe sustains for instructions shaped like the influence kernels'); kind 3:
+ * the same with one multiplicand from the constant bank (a Horner step with a stored coefficient).
+ * Result in TFLOP/s (FMA = 2 flop). */
 neb_status neb_fp64_peak(neb_ctx* ctx, int32_t kind, double* tflops);
 
 /* Accumulated device time (ms) and number of kernel launches of a stage since the last

@@ -192,6 +192,19 @@ def solve_library(K: np.ndarray, b: np.ndarray) -> np.ndarray:
     return np.linalg.solve(K * r[:, None], b * r)
 
 
+def solve_svd(K: np.ndarray, b: np.ndarray, rcond: float = 1e-10) -> np.ndarray:
+    """OptSVD (P:195: "overlapping surfaces ... Singular Value Decomposition can be used to obtain the solution"; the
+    paper does not say which solution — reading S31): the MINIMUM-NORM least-squares solution of the row-equilibrated
+    system (reading S15), sigma = sum over s_i > rcond s_max of v_i (u_i . b) / s_i, with numpy.linalg.svd (LAPACK
+    gesdd) as the library step.  Coincident panels make K exactly rank-deficient: their columns are equal, the
+    singular value of the difference direction is ~eps s_max and is dropped, the charge is shared equally."""
+    K, b = _d(K), _d(b)
+    r = 1.0 / np.abs(K).max(axis=1)
+    U, S, Vt = np.linalg.svd(K * r[:, None])
+    keep = S > rcond * S[0]
+    return Vt[keep].T @ ((U[:, keep].T @ (b * r)) / S[keep])
+
+
 def push(pos, E, mu, dt, mode="ld"):
     pos = np.array(pos, dtype=np.float64, order="C")
     E = _d(E)

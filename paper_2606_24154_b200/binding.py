@@ -10,7 +10,7 @@ from . import build as _build
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
 NEB_DIST_BLOCK = 256
-NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS = 0, 1, 2, 3, 4, 5
+NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS, NEB_OPT_SOLVER = 0, 1, 2, 3, 4, 5, 6
 STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
 
@@ -72,6 +72,8 @@ def lib():
         L.neb_reset_stats.argtypes = [vp]
         L.neb_launch_count.argtypes = [vp]
         L.neb_launch_count.restype = i64
+        L.neb_set_svd_cutoff.argtypes = [vp, dbl]
+        L.neb_get_singular_values.argtypes = [vp, vp, C.POINTER(i32)]
         L.neb_dist_configure.argtypes = [vp, i32, i32]
         L.neb_dist_npad.argtypes = [vp]
         L.neb_dist_npad.restype = i64
@@ -329,6 +331,15 @@ class Neb:
 
     def launch_count(self) -> int:
         return int(self._L.neb_launch_count(self._h))
+
+    def set_svd_cutoff(self, rcond: float):
+        self._ck(self._L.neb_set_svd_cutoff(self._h, float(rcond)))
+
+    def get_singular_values(self, npad: int):
+        """(singular values in column order (npad), sweeps) of the resident SVD factors (test hook)."""
+        s, sw = np.empty(npad), C.c_int32(0)
+        self._ck(self._L.neb_get_singular_values(self._h, _ptr(s), C.byref(sw)))
+        return s, int(sw.value)
 
     # ---- scale-out of the solve (neb_dist_*, SURVEY §8(f).4): device tensors only; the exchanges are parallel.dist_solve's
     def dist_configure(self, rank: int, world: int):

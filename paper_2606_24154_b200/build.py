@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libneb.so")
-SOURCES = ["neb_api.cu", "neb_field.cu", "neb_lu.cu", "neb_lu_panel.cu", "neb_trisolve.cu", "neb_dist.cu", "neb_fastvol.cu", "neb_voxel.cu", "neb_peaks.cu"]
+SOURCES = ["neb_api.cu", "neb_field.cu", "neb_lu.cu", "neb_lu_panel.cu", "neb_trisolve.cu", "neb_dist.cu", "neb_svd.cu", "neb_fastvol.cu", "neb_voxel.cu", "neb_peaks.cu"]
 HEADERS = ["neb_internal.h", "neb_math.cuh", "neb_influence.cuh", os.path.join("..", "..", "include", "neb.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=true"]

@@ -300,12 +300,13 @@ __global__ void push_kernel(int64_t n3, double* __restrict__ pos, const double* 
 
 static void free_problem(neb_ctx* c) {
   void* ptrs[] = {c->d_rec, c->d_uniform, c->d_perm, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_img,
-                  c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma, c->d_dinv};
+                  c->d_K, c->d_rscale, c->d_ipiv, c->d_rowperm, c->d_b, c->d_x, c->d_sigma, c->d_dinv, c->d_V, c->d_s2, c->d_svd_w};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   c->d_rec = nullptr; c->d_uniform = nullptr; c->d_perm = nullptr; c->d_colloc = nullptr; c->d_normal = nullptr; c->d_bc_kind = nullptr;
   c->d_bc_value = nullptr; c->d_diag = nullptr; c->d_img = nullptr; c->d_K = nullptr; c->d_rscale = nullptr;
   c->d_ipiv = nullptr; c->d_rowperm = nullptr; c->d_b = nullptr; c->d_x = nullptr; c->d_sigma = nullptr; c->d_dinv = nullptr;
+  c->d_V = nullptr; c->d_s2 = nullptr; c->d_svd_w = nullptr;
   c->assembled = c->factored = c->have_sigma = false;
   c->n = c->npad = c->stride = 0;
   c->img_cap = 0;
@@ -413,6 +414,10 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
     case NEB_OPT_EVAL_SPLITS:
       if (value < 0 || value > 1024) return fail(c, NEB_EINVAL, "eval splits must be 0 (automatic) .. 1024");
       c->eval_splits = (int)value;
+      return NEB_OK;
+    case NEB_OPT_SOLVER:
+      if (value != 0 && value != 1) return fail(c, NEB_EINVAL, "solver must be 0 (LU) or 1 (SVD)");
+      c->solver = (int)value;
       return NEB_OK;
     default: return fail(c, NEB_EINVAL, "unknown option");
   }
@@ -556,7 +561,9 @@ neb_status neb_solve(neb_ctx* c, double* sigma_out) {
   NEB_CUDA(c, cudaSetDevice(c->device));
   if (!c->factored) {
     NEB_TRY(scale_matrix_rows(c));
-    NEB_TRY(lu_factor(c));
+    c->factored_with = c->solver;
+    if (c->solver == 1) NEB_TRY(svd_factor(c));
+    else NEB_TRY(lu_factor(c));
     int32_t h_flag = 0;
     NEB_CUDA(c, cudaMemcpyAsync(&h_flag, c->d_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -567,7 +574,7 @@ neb_status neb_solve(neb_ctx* c, double* sigma_out) {
     }
   }
   NEB_TRY(form_rhs(c));
-  NEB_TRY(lu_solve(c, c->d_b, 1, c->d_x));
+  NEB_TRY(factors_solve(c, c->d_b, 1, c->d_x));
   NEB_TRY(finish_sigma(c, c->d_x));
   if (sigma_out) {
     if (is_device_ptr(sigma_out)) {
@@ -608,6 +615,25 @@ neb_status neb_eval(neb_ctx* c, int64_t m, const double* pts, double* phi, doubl
   NEB_TRY(sg.out(E, sizeof(double) * 3 * m, &dE));
   NEB_TRY(field_at_points(c, m, (const double*)dp, true, true, (double*)dphi, (double*)dE));
   return sg.finish();
+}
+
+neb_status neb_set_svd_cutoff(neb_ctx* c, double rcond) {
+  if (!c || !(rcond >= 0.0) || !(rcond < 1.0)) return NEB_EINVAL;
+  c->svd_rcond = rcond;
+  return NEB_OK;
+}
+
+neb_status neb_get_singular_values(neb_ctx* c, double* s_out, int32_t* sweeps) {
+  if (!c || !s_out) return NEB_EINVAL;
+  if (!c->factored || c->factored_with != 1) return fail(c, NEB_ESTATE, "neb_get_singular_values: no SVD factors (NEB_OPT_SOLVER = 1, then neb_solve)");
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  std::vector<double> h((size_t)c->npad);
+  NEB_CUDA(c, cudaMemcpyAsync(h.data(), c->d_s2, sizeof(double) * c->npad, cudaMemcpyDeviceToHost, c->stream));
+  NEB_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (double& v : h) v = sqrt(v);
+  NEB_CUDA(c, cudaMemcpy(s_out, h.data(), sizeof(double) * c->npad, cudaMemcpyDefault));
+  if (sweeps) *sweeps = c->svd_sweeps;
+  return NEB_OK;
 }
 
 neb_status neb_set_adaptive(neb_ctx* c, double far_distance) {

@@ -158,7 +158,7 @@ neb_status solve_weighting(neb_ctx* c, int nrhs, const double* d_w_caller, doubl
   NEB_CUDA(c, cudaMallocFromPoolAsync((void**)&tx, sizeof(double) * (size_t)nrhs * npad, c->pool, c->stream));
   weighting_rhs_kernel<<<(unsigned)((npad + 255) / 256), 256, 0, c->stream>>>(n, npad, nrhs, c->d_perm, c->d_bc_kind, d_w_caller, tb);
   c->launches++;
-  neb_status st = lu_solve(c, tb, nrhs, tx);
+  neb_status st = factors_solve(c, tb, nrhs, tx);
   if (st == NEB_OK) {
     unpermute_multi_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, npad, nrhs, c->d_perm, tx, d_sigma_out);
     c->launches++;

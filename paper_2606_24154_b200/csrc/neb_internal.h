@@ -56,6 +56,8 @@ struct neb_ctx {
   int profile = 0;
   int lu_lookahead = 1; // 1: factor panel k+1 on the side stream while panel k's trailing update runs
   int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
+  int solver = 0;       // NEB_OPT_SOLVER: 0 = LU (OptLU), 1 = one-sided Jacobi SVD (OptSVD), used by the NEXT factorisation
+  double svd_rcond = 1e-10;   // singular values <= svd_rcond x the largest are dropped (neb_set_svd_cutoff)
   int eval_splits = 0;  // 0: element/charge chunks chosen from the point count; k: always k chunks (shard-invariant bits)
 
   // scale-out of the solve (neb_dist.cu): 256-column blocks dealt cyclically to dist_world contexts; 1 = not distributed
@@ -91,6 +93,12 @@ struct neb_ctx {
   double* d_dinv = nullptr;       // inverses of the 64x64 diagonal blocks of L and U: 2 * (npad/64) * 4096
   double* d_sigma = nullptr;      // n, caller order
   void* d_panel_ws = nullptr;     // LU panel exchange buffers
+  // OptSVD (neb_svd.cu): right singular vectors, squared singular values (+ their maximum in slot npad), weights
+  double* d_V = nullptr;
+  double* d_s2 = nullptr;
+  double* d_svd_w = nullptr;
+  int factored_with = 0;          // which factors are resident: 0 LU, 1 SVD
+  int svd_sweeps = 0;
   bool assembled = false, factored = false, have_sigma = false;
 
   // space charges: SoA x,y,z,q (4 * q_cap)
@@ -157,6 +165,10 @@ neb_status lu_factor(neb_ctx* c);         // a5, in place on d_K (already row-sc
 // neb_trisolve.cu: a6, nrhs right-hand sides d_b[k * npad + i] (unscaled, sorted order) -> d_out[k * npad + i]
 neb_status lu_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
 neb_status trisolve_init_device(neb_ctx* c);
+// neb_svd.cu: OptSVD; factors_solve = the solve on whichever factors are resident
+neb_status svd_factor(neb_ctx* c);
+neb_status svd_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
+neb_status factors_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
 size_t lu_panel_ws_bytes(int num_sms);
 // launch wrappers of the LU update kernels (A: column-major with leading dimension ld; Lp/ldl: the L operand, row index absolute)
 void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi);

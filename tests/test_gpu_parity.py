@@ -1112,3 +1112,71 @@ def test_dist_lu_two_ranks_real_library():
         phi, phi1 = got[0][(which, "phi")], got[0][(which, "phi1")]
         assert np.array_equal(phi, got[1][(which, "phi")])
         assert np.max(np.abs(phi - phi1)) <= 1e-8 * np.max(np.abs(phi1))     # sigma differs by <= 1e-9 between the two solves
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY 8(f).4, OptSVD (reading S31): one-sided Jacobi SVD, minimum-norm solution on overlapping panels
+# ---------------------------------------------------------------------------------------------
+def test_optsvd_overlapping_panels(P):
+    import oracle as orc
+    pr = W.plate(n_side=10)
+    idx = np.array([0, 17, 44, 45, 99])
+    pr2 = W.with_coincident_panels(pr, idx)
+    g2 = orc.Geometry(pr2)
+    K2, b2 = orc.assemble(g2), orc.rhs(g2)
+    so = orc.solve_svd(K2, b2)
+    nb = P.Neb()
+    nb.assemble_problem(pr2)
+    with pytest.raises(P.NebError) as ei:                    # OptLU: exactly equal rows -> zero pivot
+        nb.solve()
+    assert ei.value.status == 4
+    nb.set_option(P.binding.NEB_OPT_SOLVER, 1)
+    nb.assemble_problem(pr2)
+    sig = nb.solve()
+    scale = np.max(np.abs(so))
+    assert np.max(np.abs(sig - so)) <= TOL_SIGMA * scale
+    assert np.max(np.abs(sig[idx] - sig[pr.n:])) <= TOL_SIGMA * scale          # the doubled panels share their charge equally
+    npad = -(-pr2.n // 128) * 128
+    s, sweeps = nb.get_singular_values(npad)
+    r = 1.0 / np.abs(K2).max(axis=1)
+    s_o = np.linalg.svd(K2 * r[:, None], compute_uv=False)
+    want = np.sort(np.concatenate([s_o, np.ones(npad - pr2.n)]))[::-1]
+    got = np.sort(s)[::-1]
+    big = want > 1e-10 * want[0]
+    assert np.max(np.abs(got[big] - want[big]) / want[big]) <= 1e-11         # Jacobi: relative accuracy
+    assert np.all(got[~big] <= 1e-13 * want[0]) and (~big).sum() == idx.size
+    assert 2 <= sweeps <= 30, sweeps
+    # field from the minimum-norm sigma = field of the mesh without the overlap
+    phi, E = nb.eval(pr.points[:, :200])
+    phi_o, E_o, scl = truth(orc, g2, sig, pr.points[:, :200])
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "optsvd", scl)
+    one = P.Neb()
+    one.assemble_problem(pr)
+    s1 = one.solve()
+    phi1, _ = one.eval(pr.points[:, :200])
+    assert np.max(np.abs(phi - phi1)) <= 1e-8 * np.max(np.abs(phi1))
+    # re-solve with space charge and a weighting solve on the same factors
+    rs = np.random.RandomState(2)
+    pos, q = rs.uniform(-8e-3, 8e-3, size=(3, 100)), np.full(100, W.Q_E * 1e6)
+    nb.add_space_charge(pos, q)
+    sig2 = nb.solve()
+    so2 = orc.solve_svd(K2, orc.rhs(g2, pos, q))
+    assert np.max(np.abs(sig2 - so2)) <= TOL_SIGMA * np.max(np.abs(so2))
+    w = nb.solve_weighting(np.ones(pr2.n))
+    assert np.max(np.abs(w - so)) <= TOL_SIGMA * scale                            # all conductors at 1 V = the plate problem
+    one.close()
+    nb.close()
+
+
+def test_optsvd_equals_lu_on_a_regular_mesh(P):
+    pr = W.thgem(d=10, n_plane=6, n_grid=2)                  # rectangles, right triangles, dielectric rows
+    a = P.Neb()
+    a.assemble_problem(pr)
+    s_lu = a.solve()
+    a.close()
+    bnb = P.Neb()
+    bnb.set_option(P.binding.NEB_OPT_SOLVER, 1)
+    bnb.assemble_problem(pr)
+    s_svd = bnb.solve()
+    bnb.close()
+    assert np.max(np.abs(s_svd - s_lu)) <= TOL_SIGMA * np.max(np.abs(s_lu))

@@ -703,6 +703,50 @@ def test_solve_library_equals_plain_lu(orc):
     assert np.max(np.abs(x0 - x1)) < 1e-9 * np.max(np.abs(x0))
 
 
+def test_solve_svd_minimum_norm_on_overlapping_panels(orc):
+    """OptSVD (reading S31).  Pins of oracle.solve_svd to things other than itself:
+    (i) on a non-singular system it gives what the plain C elimination gives (a different algorithm);
+    (ii) with k panels listed twice the matrix has k pairs of equal columns (and rows): the LU path fails; the
+        minimum-norm solution must share each doubled panel's charge EQUALLY between the two copies (for equal columns
+        a, a the norm x1^2 + x2^2 at fixed x1 + x2 is least at x1 = x2) and reproduce the non-overlapping solution:
+        sigma_a + sigma_a' = sigma_single, every other sigma unchanged;
+    (iii) the Moore-Penrose conditions on a random rank-deficient matrix M = L R: the residual is orthogonal to the
+        range (M^T (M x - v) = 0) and x is orthogonal to the null space of R, built independently by a QR of R^T."""
+    pr = W.plate(n_side=10)
+    g = orc.Geometry(pr)
+    K, b = orc.assemble(g, mode="f64"), orc.rhs(g, mode="f64")
+    s_lu = orc.solve(K, b, mode="ld")
+    s_svd = orc.solve_svd(K, b)
+    assert np.max(np.abs(s_svd - s_lu)) < 1e-10 * np.max(np.abs(s_lu))
+    idx = np.array([0, 17, 44, 45, 99])
+    pr2 = W.with_coincident_panels(pr, idx)
+    g2 = orc.Geometry(pr2)
+    K2, b2 = orc.assemble(g2, mode="f64"), orc.rhs(g2, mode="f64")
+    assert np.array_equal(K2[:, idx], K2[:, pr.n:]) and np.array_equal(K2[idx, :], K2[pr.n:, :])
+    with pytest.raises(np.linalg.LinAlgError):
+        orc.solve(K2, b2, mode="ld")
+    s2 = orc.solve_svd(K2, b2)
+    scale = np.max(np.abs(s_lu))
+    assert np.max(np.abs(s2[idx] - s2[pr.n:])) < 1e-9 * scale                      # equal split
+    merged = s2[: pr.n].copy()
+    merged[idx] += s2[pr.n:]
+    assert np.max(np.abs(merged - s_lu)) < 1e-9 * scale                           # same physics as without the overlap
+    phi1, E1 = orc.evaluate(g, s_lu, pr.points[:, :50])
+    phi2, E2 = orc.evaluate(g2, s2, pr.points[:, :50])
+    assert np.max(np.abs(phi2 - phi1)) < 1e-9 * np.max(np.abs(phi1))
+    rs = np.random.RandomState(8)
+    n, k = 60, 41
+    L, R = rs.normal(size=(n, k)), rs.normal(size=(k, n))
+    M = L @ R
+    M /= np.abs(M).max(axis=1)[:, None]                                          # rows already equilibrated: r = 1
+    v = rs.normal(size=n)
+    x = orc.solve_svd(M, v)
+    assert np.max(np.abs(M.T @ (M @ x - v))) < 1e-10 * np.linalg.norm(v) * np.linalg.norm(M, 2)
+    Q, _ = np.linalg.qr(R.T, mode="complete")
+    null = Q[:, k:]                                                               # R null = 0
+    assert np.max(np.abs(R @ null)) < 1e-12 and np.max(np.abs(null.T @ x)) < 1e-10 * np.linalg.norm(x)
+
+
 def test_push_is_axpy(orc):
     pos = np.array([[1.0, 2.0], [3.0, 4.0], [5.0, 6.0]])
     E = np.array([[1e3, 0.0], [0.0, -2e3], [4e3, 0.0]])

@@ -296,6 +296,17 @@ def random_elements(n: int, seed: int, kinds=(RECT, TRI, WIRE), size_mm=(0.05, 1
     return pr
 
 
+def with_coincident_panels(pr: Problem, idx) -> Problem:
+    """pr with the elements idx listed a second time (appended): coincident panels, the "overlapping surfaces" that the
+    repetition of primitives produces and that make the influence matrix exactly rank-deficient (OptSVD tests)."""
+    idx = np.asarray(idx, dtype=np.int64)
+    cat1 = lambda a: np.concatenate([a, a[idx]])
+    cat3 = lambda a: np.ascontiguousarray(np.concatenate([a, a[:, idx]], axis=1))
+    return Problem(name=pr.name + "_overlap", kind=cat1(pr.kind), v0=cat3(pr.v0), e1=cat3(pr.e1), e2=cat3(pr.e2),
+                   radius=cat1(pr.radius), bc_kind=cat1(pr.bc_kind), bc_value=cat1(pr.bc_value), eps_plus=cat1(pr.eps_plus),
+                   eps_minus=cat1(pr.eps_minus), img_shift=pr.img_shift, points=pr.points, meta=dict(pr.meta, duplicated=idx))
+
+
 def by_name(name: str) -> Problem:
     """Full-size BASELINE configs by short name."""
     if name == "C0":
