@@ -41,6 +41,9 @@ sys.path.insert(0, ROOT)
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
 DEFAULT_WORKLOAD = "C2"
+# flop per rectangle pair when every element is evaluated on its own (NEB_OPT_PAIR_STRIPS = 0): the counts of the same
+# ncu table before the strip pairs (profiles/r2_opcounts.md, "Reading")
+ELEMENTWISE_RECT_FLOP = {"eval_rect_uniform": 243.2, "eval_images": 248.7}
 L2_NOTE = "256 MiB buffer written between timed steps; the matrix exceeds L2"
 WORKLOADS = {
     "C1": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
@@ -355,6 +358,7 @@ class Runner:
         pr, ops = self.pr, self.ops
         dfma, dmma = self.peaks["dfma"], self.peaks["dmma"]
         fl, inst = flop_per_pair(pr, ops)
+        rect_key = "eval_images" if pr.n_img > 1 else "eval_rect_uniform"
         out = []
         eval_ms = stages["eval"] / max(1, launches["eval"])
         eval_pairs = self.copies * self.m * self.n
@@ -365,6 +369,9 @@ class Runner:
             "fp64_instr_per_pair": inst, "fp64_pipe_slot_frac": inst * eval_pairs / (eval_ms * 1e-3) / (0.5e12 * dfma),
             "pairs_per_s_kernel": eval_pairs / (eval_ms * 1e-3), "field_map_points_per_s": self.m / (eval_ms * 1e-3),
             "frac_of_3operand_dfma_peak": ach / self.peaks["dfma3"],
+            # the same pairs at the element-by-element operation count (strip pairs share an edge's two corner distances and
+            # its logarithm: fewer executed flop for the same closed forms; profiles/r2_opcounts.md)
+            "frac_elementwise": ach / dfma * ELEMENTWISE_RECT_FLOP[rect_key] / ops[rect_key]["flop"],
             "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process (nominal 148 SM x 64 DFMA/clk x "
                            "2 x 1.965 GHz = 37.2); MEASURED_PEAKS.json has no FP64 entry",
             "constants_source": "profiles/r2_opcounts.md (ncu smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on per pair)"}))
@@ -453,6 +460,37 @@ def extra_record(name, dev, P, ops, traffic, peaks, steps):
     del rn
     torch.cuda.empty_cache()
     return rec
+
+
+def dist_lu_record(dev, P):
+    """SURVEY 8(f).4 on the one GPU at hand: the block-cyclic factorisation and solves of C2 driven by parallel.DistSolver
+    with a single rank (every kernel of the distributed path runs; the broadcasts are no-ops), with and without
+    look-ahead, beside which the single-GPU factorisation of the line can be read."""
+    import torch
+    from paper_2606_24154_b200 import parallel
+    pr = load_problem("C2")
+    out = {"workload": "C2", "n_elements": int(pr.n), "ranks": 1}
+    for la in (True, False):
+        nb = P.Neb(dev.index)
+        ds = parallel.DistSolver(nb, lookahead=la)
+        ds.assemble(pr)
+        ds.factor()
+        ds.solve()
+        ds.assemble(pr)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record()
+        ds.factor()
+        ev[1].record()
+        ds.solve()
+        ev[2].record()
+        torch.cuda.synchronize()
+        key = "lookahead" if la else "no_lookahead"
+        out[f"factor_ms_{key}"] = ev[0].elapsed_time(ev[1])
+        out[f"solve_ms_{key}"] = ev[1].elapsed_time(ev[2])
+        out["lu_flop"] = nb.counter(1)
+        nb.close()
+    out["tflops_lookahead"] = out["lu_flop"] / (out["factor_ms_lookahead"] * 1e-3) * 1e-12
+    return out
 
 
 def main():
@@ -545,7 +583,8 @@ def main():
     torch.cuda.empty_cache()
     if rank == 0 and world == 1 and name == DEFAULT_WORKLOAD and not args.no_extra:
         line["extra"] = {"C3": extra_record("C3", dev, P, ops, traffic, peaks, steps=1),
-                         "C4": extra_record("C4", dev, P, ops, traffic, peaks, steps=10)}
+                         "C4": extra_record("C4", dev, P, ops, traffic, peaks, steps=10),
+                         "dist_lu_one_rank": dist_lu_record(dev, P)}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

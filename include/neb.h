@@ -58,6 +58,9 @@ enum {
                            the given number of points (few points -> many chunks); k > 0: always k chunks, so that the
                            fixed-order partial sums, hence the result BITS, do not depend on how many points a call
                            (or a rank of a sharded evaluation) is given                                          */
+  NEB_OPT_PAIR_STRIPS = 7, /* 1 (default): two rectangles of the table that are neighbours of one strip (same plane and axes, a
+                           shared edge, found by neb_assemble) are evaluated together, sharing the edge's two corner
+                           distances and its logarithm; 0: every element on its own.  Read by the next neb_assemble   */
   NEB_OPT_SOLVER = 6,   /* InvertMatrix: 0 (default) = OptLU, the blocked LU; 1 = OptSVD, one-sided Jacobi SVD and the
                            minimum-norm least-squares solution (for meshes with coincident / overlapping panels, whose
                            matrix is rank-deficient: the LU reports NEB_ESINGULAR there).  Read at the next factorisation

@@ -10,7 +10,7 @@ from . import build as _build
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
 NEB_DIST_BLOCK = 256
-NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS, NEB_OPT_SOLVER = 0, 1, 2, 3, 4, 5, 6
+NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS, NEB_OPT_SOLVER, NEB_OPT_PAIR_STRIPS = 0, 1, 2, 3, 4, 5, 6, 7
 STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
 

@@ -235,9 +235,16 @@ __global__ void frames_kernel(int64_t n, int64_t stride, const int32_t* __restri
   diag[s] = dg;
 }
 
-// One 64-thread CTA per 64-element window of the sorted table: do all its elements have bit-identical unit axes?
+// One 64-thread CTA per 64-element window of the sorted table.  uniform[3 w] = 1 if all its elements have bit-identical
+// unit axes (a face of a mesh); uniform[3 w + 1], [3 w + 2] = bit k set when the rectangles 2k and 2k + 1 of the window
+// are neighbours of one strip — same plane, same axes, the second one starts where the first one ends along local X
+// (mask 1) or local Z (mask 2), equal extent across — so that the pair shares an edge and two corners and is evaluated
+// by rect_pair_local (neb_influence.cuh).  Agreement is asked to 1e-13 of the smaller side: the table's coordinates
+// carry rounding errors of ~1e-16 x |v0|, and treating the shared edge as one line moves it by no more than that.
 __global__ void __launch_bounds__(64) tile_uniform_kernel(int64_t n, int64_t stride, const double* __restrict__ rec,
+                                                          const int32_t* __restrict__ counts, int pairs_enabled,
                                                           int32_t* __restrict__ uniform) {
+  __shared__ unsigned s_bx[2], s_bz[2];
   const int64_t j0 = (int64_t)blockIdx.x * 64, j = j0 + threadIdx.x;
   int same = 1;
   if (j < n) {
@@ -245,8 +252,31 @@ __global__ void __launch_bounds__(64) tile_uniform_kernel(int64_t n, int64_t str
     for (int f = 3; f < 12; ++f)
       same &= __double_as_longlong(rec[f * stride + j]) == __double_as_longlong(rec[f * stride + j0]);
   }
+  bool chain_x = false, chain_z = false;
+  if (pairs_enabled && (threadIdx.x & 1) == 0 && j + 1 < (int64_t)counts[0]) {
+    bool axes = true;
+#pragma unroll
+    for (int f = 3; f < 12; ++f) axes = axes && __double_as_longlong(rec[f * stride + j]) == __double_as_longlong(rec[f * stride + j + 1]);
+    const double a0 = rec[12 * stride + j], a1 = rec[12 * stride + j + 1], b0 = rec[13 * stride + j], b1 = rec[13 * stride + j + 1];
+    const double dx = rec[17 * stride + j + 1] - rec[17 * stride + j], dy = rec[18 * stride + j + 1] - rec[18 * stride + j],
+                 dz = rec[19 * stride + j + 1] - rec[19 * stride + j];
+    const double t = 1e-13 * fmin(a0, b0);
+    chain_x = axes && fabs(b1 - b0) <= t && fabs(dy) <= t && fabs(dz) <= t && fabs(dx - a0) <= t;
+    chain_z = axes && fabs(a1 - a0) <= t && fabs(dy) <= t && fabs(dx) <= t && fabs(dz - b0) <= t;
+  }
+  const unsigned bx = __ballot_sync(0xffffffffu, chain_x), bz = __ballot_sync(0xffffffffu, chain_z);
+  if ((threadIdx.x & 31) == 0) { s_bx[threadIdx.x >> 5] = bx; s_bz[threadIdx.x >> 5] = bz; }
   same = __syncthreads_and(same);
-  if (threadIdx.x == 0) uniform[blockIdx.x] = (j0 < n) ? same : 0;
+  if (threadIdx.x == 0) {
+    unsigned mx = 0, mz = 0;
+    for (int k = 0; k < 32; ++k) {                        // pair k = lanes 2k, 2k + 1 of the window
+      mx |= ((s_bx[k >> 4] >> (2 * (k & 15))) & 1u) << k;
+      mz |= ((s_bz[k >> 4] >> (2 * (k & 15))) & 1u) << k;
+    }
+    uniform[3 * blockIdx.x] = (j0 < n) ? same : 0;
+    uniform[3 * blockIdx.x + 1] = same ? (int32_t)mx : 0;
+    uniform[3 * blockIdx.x + 2] = same ? (int32_t)mz : 0;
+  }
 }
 
 __global__ void set_weights_kernel(int64_t n, int64_t stride, const int32_t* __restrict__ perm, const double* __restrict__ sigma_caller,
@@ -415,6 +445,7 @@ neb_status neb_set_option(neb_ctx* c, int32_t option, int64_t value) {
       if (value < 0 || value > 1024) return fail(c, NEB_EINVAL, "eval splits must be 0 (automatic) .. 1024");
       c->eval_splits = (int)value;
       return NEB_OK;
+    case NEB_OPT_PAIR_STRIPS: c->pair_strips = value ? 1 : 0; return NEB_OK;
     case NEB_OPT_SOLVER:
       if (value != 0 && value != 1) return fail(c, NEB_EINVAL, "solver must be 0 (LU) or 1 (SVD)");
       c->solver = (int)value;
@@ -450,7 +481,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
   const int64_t st = c->stride, npad = c->npad;
   if (!reuse) {
     NEB_CUDA(c, cudaMalloc((void**)&c->d_rec, sizeof(double) * kRec * st));
-    NEB_CUDA(c, cudaMalloc((void**)&c->d_uniform, sizeof(int32_t) * (st / 64)));
+    NEB_CUDA(c, cudaMalloc((void**)&c->d_uniform, sizeof(int32_t) * 3 * (st / 64)));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_perm, sizeof(int32_t) * st));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_colloc, sizeof(double) * 3 * st));
     NEB_CUDA(c, cudaMalloc((void**)&c->d_normal, sizeof(double) * 3 * st));
@@ -528,7 +559,7 @@ neb_status neb_assemble(neb_ctx* c, int64_t n, const int32_t* kind, const double
         (const double*)drad, (const double*)dcol, (const int32_t*)dbk, (const double*)dbv, (const double*)dep,
         (const double*)dem, c->d_rec, c->d_colloc, c->d_normal, c->d_bc_kind, c->d_bc_value, c->d_diag, c->d_flag);
     c->launches++;
-    tile_uniform_kernel<<<(unsigned)(st / 64), 64, 0, c->stream>>>(n, st, c->d_rec, c->d_uniform);
+    tile_uniform_kernel<<<(unsigned)(st / 64), 64, 0, c->stream>>>(n, st, c->d_rec, d_counts, c->pair_strips, c->d_uniform);
     c->launches++;
     NEB_CUDA(c, cudaGetLastError());
   }

@@ -65,37 +65,30 @@ __global__ void dist_fix_scales_kernel(double* rscale, int64_t npad) {
 template <bool UPPER>
 __global__ void __launch_bounds__(DB) dist_diag_solve_kernel(const double* __restrict__ T, int64_t ld, const double* __restrict__ t,
                                                              double* __restrict__ y) {
-  __shared__ double s_x[8];
+  __shared__ double s_x[2][8];
   const int i = threadIdx.x;
   double v = y[i] - t[i];
-  if (!UPPER) {
-    for (int j0 = 0; j0 < DB; j0 += 8) {
-      double col[8];
+  // group gi = columns 8 gi .. 8 gi + 7 (lower) or DB-1-8 gi downwards (upper); the next group's columns are in flight
+  // while this group's 8 dependent steps run
+  auto column = [&](int gi, int u) { return UPPER ? DB - 1 - (8 * gi + u) : 8 * gi + u; };
+  double col[8], nxt[8];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) col[u] = T[i + (int64_t)(j0 + u) * ld];
+  for (int u = 0; u < 8; ++u) col[u] = T[i + (int64_t)column(0, u) * ld];
+  for (int gi = 0; gi < DB / 8; ++gi) {
+    if (gi + 1 < DB / 8) {
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const int j = j0 + u;
-        if (i == j) s_x[u] = v;                       // unit diagonal
-        __syncthreads();
-        if (i > j) v = fma(-col[u], s_x[u], v);
-      }
-      __syncthreads();
+      for (int u = 0; u < 8; ++u) nxt[u] = T[i + (int64_t)column(gi + 1, u) * ld];
     }
-  } else {
-    for (int j0 = DB - 1; j0 >= 0; j0 -= 8) {
-      double col[8];
+    double* sx = s_x[gi & 1];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) col[u] = T[i + (int64_t)(j0 - u) * ld];
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const int j = j0 - u;
-        if (i == j) { v = v / col[u]; s_x[u] = v; }
-        __syncthreads();
-        if (i < j) v = fma(-col[u], s_x[u], v);
-      }
+    for (int u = 0; u < 8; ++u) {
+      const int j = column(gi, u);
+      if (i == j) { if (UPPER) v = v / col[u]; sx[u] = v; }      // L has a unit diagonal
       __syncthreads();
+      if (UPPER ? (i < j) : (i > j)) v = fma(-col[u], sx[u], v);
     }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) col[u] = nxt[u];
   }
   y[i] = v;
 }

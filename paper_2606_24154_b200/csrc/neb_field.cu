@@ -21,6 +21,14 @@ namespace neb {
 #define NEB_EVAL_UNROLL 2             // elements of a uniform window in flight per thread
 #endif
 constexpr int kEvalUnroll = NEB_EVAL_UNROLL;
+#ifndef NEB_PAIR_UNROLL
+#define NEB_PAIR_UNROLL 1
+#endif
+#ifndef NEB_PAIR_STRIPS
+#define NEB_PAIR_STRIPS 1
+#endif
+constexpr int kPairUnroll = NEB_PAIR_UNROLL;
+constexpr bool kPairStrips = NEB_PAIR_STRIPS != 0;   // strip neighbours evaluated as pairs (rect_pair_local)
 constexpr int kThreads = 128;   // threads per CTA = points per CTA
 constexpr int kTile = 64;       // elements per shared-memory tile
 constexpr int kChargeTile = 256;
@@ -114,7 +122,7 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
     tile_wait(sm, seq);
     const unsigned buf = seq & 1u;
     const int e0 = (int)max(lo - tb, (int64_t)0), e1 = (int)min(hi - tb, (int64_t)kTile);
-    if (KIND != 2 && g.uniform[tb >> 6]) {
+    if (KIND != 2 && g.uniform[3 * (tb >> 6)]) {
       // Uniform window: all 64 elements share one set of unit axes (a face of a mesh).  The point's products with
       // the axes are formed once per window, an element's local coordinates are three subtractions, and the field
       // is accumulated in the LOCAL frame and rotated to global once per window instead of once per pair.
@@ -135,8 +143,12 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
       const double PY = fma(px, ax.eyx, fma(py, ax.eyy, pz * ax.eyz));
       const double PZ = fma(px, ax.ezx, fma(py, ax.ezy, pz * ax.ezz));
       sink.tile_begin(ax);
-#pragma unroll kEvalUnroll
-      for (int e = e0; e < e1; ++e) {
+      // strip neighbours (rectangles 2k, 2k + 1 of the window sharing an edge: masks from tile_uniform_kernel) are
+      // evaluated as a pair, 6 corner distances and 7 edge logarithms for the two instead of 8 and 8; the masks are
+      // the same for every thread of the grid, so the choice costs no divergence
+      const unsigned mask_x = (KIND == 0 && kPairStrips) ? (unsigned)g.uniform[3 * (tb >> 6) + 1] : 0u;
+      const unsigned mask_z = (KIND == 0 && kPairStrips) ? (unsigned)g.uniform[3 * (tb >> 6) + 2] : 0u;
+      auto single = [&](int e) {
         const double a = sm.rec[buf][12][e], b = sm.rec[buf][13][e], aux = sm.rec[buf][14][e], far2 = sm.rec[buf][16][e];
         const double X0 = PX - sm.rec[buf][17][e], Y0 = PY - sm.rec[buf][18][e], Z0 = PZ - sm.rec[buf][19][e];
         double phi = 0.0, lx = 0.0, ly = 0.0, lz = 0.0;
@@ -158,7 +170,41 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
           for (int s = n_near; s < n_img; ++s) far_copy(area, cxl - sm.limg[0][s], Y0 - sm.limg[1][s], czl - sm.limg[2][s], phi, lx, ly, lz);
         }
         sink.local(tb + e, sm.rec[buf][15][e], phi, lx, ly, lz);
+      };
+      int e = e0;
+      if (e & 1) { single(e); ++e; }                        // pairs sit at even positions of the window
+#pragma unroll kPairUnroll
+      for (; e + 1 < e1; e += 2) {
+        const bool along_x = (mask_x >> (e >> 1)) & 1u, along_z = (mask_z >> (e >> 1)) & 1u;
+        if (KIND == 0 && n_near == n_img && (along_x || along_z)) {
+          // the pair in the first element's frame; a strip along local Z is the same figure with X and Z exchanged
+          const double a1 = sm.rec[buf][12][e], b1 = sm.rec[buf][13][e], a2 = sm.rec[buf][12][e + 1], b2 = sm.rec[buf][13][e + 1];
+          const double la1 = along_x ? a1 : b1, la2 = along_x ? a2 : b2, lb = along_x ? b1 : a1;
+          const double ab1 = sm.rec[buf][14][e], ab2 = sm.rec[buf][14][e + 1], fa = sm.rec[buf][16][e], fb = sm.rec[buf][16][e + 1];
+          const double X0 = PX - sm.rec[buf][17][e], Y0 = PY - sm.rec[buf][18][e], Z0 = PZ - sm.rec[buf][19][e];
+          const double S0 = along_x ? X0 : Z0, T0 = along_x ? Z0 : X0;      // along / across the strip
+          double p1 = 0.0, s1 = 0.0, y1 = 0.0, t1 = 0.0, p2 = 0.0, s2 = 0.0, y2 = 0.0, t2 = 0.0;
+          if (self0) {
+            rect_pair_local<M>(la1, la2, lb, ab1, ab2, fa, fb, S0, Y0, T0, p1, s1, y1, t1, p2, s2, y2, t2);
+            if (sink.self_pv(tb + e)) { s1 = 0.0; y1 = 0.0; t1 = 0.0; }
+            if (sink.self_pv(tb + e + 1)) { s2 = 0.0; y2 = 0.0; t2 = 0.0; }
+          }
+#pragma unroll 1
+          for (int s = self0 ? 1 : 0; s < n_near; ++s) {
+            const double sx = sm.limg[0][s], sz = sm.limg[2][s];
+            double q1, u1, v1, w1, q2, u2, v2, w2;
+            rect_pair_local<M>(la1, la2, lb, ab1, ab2, fa, fb, S0 - (along_x ? sx : sz), Y0 - sm.limg[1][s], T0 - (along_x ? sz : sx),
+                               q1, u1, v1, w1, q2, u2, v2, w2);
+            p1 += q1; s1 += u1; y1 += v1; t1 += w1; p2 += q2; s2 += u2; y2 += v2; t2 += w2;
+          }
+          sink.local(tb + e, sm.rec[buf][15][e], p1, along_x ? s1 : t1, y1, along_x ? t1 : s1);
+          sink.local(tb + e + 1, sm.rec[buf][15][e + 1], p2, along_x ? s2 : t2, y2, along_x ? t2 : s2);
+        } else {
+          single(e);
+          single(e + 1);
+        }
       }
+      if (e < e1) single(e);
       sink.tile_end(ax);
     } else {
       sink.gtile_begin();

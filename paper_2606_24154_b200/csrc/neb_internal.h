@@ -21,7 +21,8 @@ constexpr int kMaxImages = 16384;                          // copies per element
 // rec[f * stride + j], f < kRec (fields listed in neb_influence.cuh).
 struct GeoTables {
   const double* rec;
-  const int32_t* uniform;   // per 64-element window: 1 if all its elements share one set of unit axes (bitwise)
+  const int32_t* uniform;   // 3 per 64-element window: [0] 1 if all its elements share one set of unit axes (bitwise);
+                            // [1], [2] bit k: rectangles 2k, 2k+1 are strip neighbours along local X / Z (tile_uniform_kernel)
   int64_t stride;
   int32_t n_rect, n_tri, n_wire;
 };
@@ -58,6 +59,7 @@ struct neb_ctx {
   int panel_mode = 0;   // 0: cluster kernel where it fits, 1: grid-wide cooperative kernel only
   int solver = 0;       // NEB_OPT_SOLVER: 0 = LU (OptLU), 1 = one-sided Jacobi SVD (OptSVD), used by the NEXT factorisation
   double svd_rcond = 1e-10;   // singular values <= svd_rcond x the largest are dropped (neb_set_svd_cutoff)
+  int pair_strips = 1;  // NEB_OPT_PAIR_STRIPS: strip-neighbour rectangles evaluated as pairs (read by neb_assemble)
   int eval_splits = 0;  // 0: element/charge chunks chosen from the point count; k: always k chunks (shard-invariant bits)
 
   // scale-out of the solve (neb_dist.cu): 256-column blocks dealt cyclically to dist_world contexts; 1 = not distributed
@@ -70,7 +72,7 @@ struct neb_ctx {
   int64_t n = 0, npad = 0, stride = 0;
   int32_t n_rect = 0, n_tri = 0, n_wire = 0, n_img = 0;
   double* d_rec = nullptr;        // kRec * stride
-  int32_t* d_uniform = nullptr;   // stride / 64 window flags (see GeoTables)
+  int32_t* d_uniform = nullptr;   // 3 x stride / 64 window flags and pair masks (see GeoTables)
   int32_t* d_perm = nullptr;      // sorted position -> caller index
   double* d_colloc = nullptr;     // 3 * stride, sorted order
   double* d_normal = nullptr;     // 3 * stride, sorted order

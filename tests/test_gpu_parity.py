@@ -1180,3 +1180,37 @@ def test_optsvd_equals_lu_on_a_regular_mesh(P):
     s_svd = bnb.solve()
     bnb.close()
     assert np.max(np.abs(s_svd - s_lu)) <= TOL_SIGMA * np.max(np.abs(s_lu))
+
+
+def test_strip_pairs_equal_single_elements(P):
+    """NEB_OPT_PAIR_STRIPS: neighbouring rectangles of a strip evaluated as a pair (shared edge: 6 corner distances and 7
+    logarithms for two elements) against every element on its own — same closed form, so K, Phi, E agree to rounding;
+    both against the oracle.  C1-like cube (strips along local X and local Z), a C3-like mesh with 3 x 3 copies and
+    dielectric rows, points in the far and in the near field."""
+    import oracle as orc
+    rs = np.random.RandomState(11)
+    for pr in (W.cube(n_side=8, m_points=400), W.double_thgem(d=10, n_plane=10, m_points=300, k_img=1)):
+        near = near_surface_points(pr, rs, 100)
+        pts = np.concatenate([pr.points, near], axis=1)
+        out = []
+        for on in (1, 0):
+            nb = P.Neb()
+            nb.set_option(P.binding.NEB_OPT_PAIR_STRIPS, on)
+            nb.assemble_problem(pr)
+            K = nb.get_matrix()
+            sig = nb.solve()
+            nb.set_sigma(np.linspace(1e-8, 3e-8, pr.n))
+            phi, E = nb.eval(pts)
+            out.append((K, sig, phi, E))
+            nb.close()
+        (K1, s1, p1, E1), (K0, s0, p0, E0) = out
+        assert np.max(np.abs(K1 - K0)) <= 1e-12 * np.max(np.abs(K0))
+        assert not np.array_equal(K1, K0)                              # the pair path really ran (different rounding)
+        assert np.max(np.abs(s1 - s0)) <= TOL_SIGMA * np.max(np.abs(s0))
+        g = orc.Geometry(pr)
+        phi_o, E_o, scale = truth(orc, g, np.linspace(1e-8, 3e-8, pr.n), pts)
+        for phi, E in ((p1, E1), (p0, E0)):
+            check_field(phi[: pr.points.shape[1]], E[:, : pr.points.shape[1]], phi_o[: pr.points.shape[1]], E_o[:, : pr.points.shape[1]],
+                        TOL_FAR, "strip pairs far", tuple(s[: pr.points.shape[1]] for s in scale))
+            check_field(phi[pr.points.shape[1]:], E[:, pr.points.shape[1]:], phi_o[pr.points.shape[1]:], E_o[:, pr.points.shape[1]:],
+                        TOL_NEAR, "strip pairs near", tuple(s[pr.points.shape[1]:] for s in scale))
