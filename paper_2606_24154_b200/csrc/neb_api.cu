@@ -391,6 +391,9 @@ neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);   // hi = numerically lowest = greatest priority
     ok = cudaStreamCreateWithPriority(&c->side_stream, cudaStreamNonBlocking, hi) == cudaSuccess &&
+         cudaStreamCreateWithPriority(&c->left_stream, cudaStreamNonBlocking, lo) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->ev_chain, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->ev_left, cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&c->ev_next, cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&c->ev_panel, cudaEventDisableTiming) == cudaSuccess;
   }
@@ -419,6 +422,9 @@ void neb_destroy(neb_ctx* c) {
     if (c->fastvol[s].nodes) cudaFree((void*)c->fastvol[s].nodes);
   if (c->pool) cudaMemPoolDestroy(c->pool);
   if (c->side_stream) { cudaStreamSynchronize(c->side_stream); cudaStreamDestroy(c->side_stream); }
+  if (c->left_stream) { cudaStreamSynchronize(c->left_stream); cudaStreamDestroy(c->left_stream); }
+  if (c->ev_chain) cudaEventDestroy(c->ev_chain);
+  if (c->ev_left) cudaEventDestroy(c->ev_left);
   if (c->ev_next) cudaEventDestroy(c->ev_next);
   if (c->ev_panel) cudaEventDestroy(c->ev_panel);
   for (int s = 0; s < NEB_STAGE_COUNT; ++s) {

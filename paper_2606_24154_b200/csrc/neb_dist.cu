@@ -181,7 +181,7 @@ neb_status neb_dist_factor_block(neb_ctx* c, int64_t g, double* panel, int32_t* 
   for (int64_t k = kb; k < kb + DB; k += 64) {
     NEB_TRY(panel_cluster_launch(c, A, k, st));
     const int64_t in_cols = kb + DB - (k + 64);
-    lu_launch_laswp(c, st, A, ld, k, kb, kb + DB, k, k + 64);
+    lu_launch_laswp(c, st, A, ld, k, 64, kb, kb + DB, k, k + 64);
     lu_launch_trsm(c, st, A, ld, A + k * ld, ld, k, k + 64, in_cols);
     lu_launch_gemm(c, st, A, ld, A + k * ld, ld, k, 64, k + 64, npad - (k + 64), k + 64, in_cols, false);
   }
@@ -211,7 +211,7 @@ neb_status neb_dist_apply_block(neb_ctx* c, int64_t g, const double* panel, cons
   const int64_t nc = c1 - c0;
   const double* Pb = panel - kb;                     // Pb[i + j * ldl] = element (absolute row i, block column j)
   if (nc > 0) {
-    for (int64_t k = kb; k < kb + DB; k += 64) lu_launch_laswp(c, st, c->d_K, ld, k, c0, c1, c1, c1);
+    lu_launch_laswp(c, st, c->d_K, ld, kb, DB, c0, c1, c1, c1);      // the block's 256 exchanges in one launch
     for (int64_t k = kb; k < kb + DB; k += 64) {
       const double* Lk = Pb + (k - kb) * ldl;
       lu_launch_trsm(c, st, c->d_K, ld, Lk, ldl, k, c0, nc);
@@ -221,7 +221,7 @@ neb_status neb_dist_apply_block(neb_ctx* c, int64_t g, const double* panel, cons
   }
   if (part != 1) {   // the factors to the left follow the rows
     const int64_t left = blocks_before(g, world, rank) * DB;
-    for (int64_t k = kb; k < kb + DB; k += 64) lu_launch_laswp(c, st, c->d_K, ld, k, 0, left, left, left);
+    lu_launch_laswp(c, st, c->d_K, ld, kb, DB, 0, left, left, left);
   }
   NEB_CUDA(c, cudaGetLastError());
   return NEB_OK;

@@ -422,8 +422,11 @@ struct AsmSink {
   __device__ __forceinline__ void gtile_end() {}
 };
 
+#ifndef NEB_ASM_MINB
+#define NEB_ASM_MINB 4
+#endif
 template <class M, bool FIRST>
-__global__ void __launch_bounds__(kThreads) assemble_kernel(GeoTables g, const double* __restrict__ img, int n_img,
+__global__ void __launch_bounds__(kThreads, NEB_ASM_MINB) assemble_kernel(GeoTables g, const double* __restrict__ img, int n_img,
                                                             const double* __restrict__ colloc, int64_t stride,
                                                             const double* __restrict__ normal,
                                                             const int32_t* __restrict__ bc_kind,

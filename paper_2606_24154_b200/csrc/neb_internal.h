@@ -45,7 +45,9 @@ struct neb_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
   cudaStream_t side_stream = nullptr;   // LU look-ahead: next panel, concurrent with the trailing update
-  cudaEvent_t ev_next = nullptr, ev_panel = nullptr;
+  cudaStream_t left_stream = nullptr;   // LU: row exchanges of the finished columns LEFT of the current block (nothing waits for them
+                                        // before the solves), off the streams that carry the factorisation
+  cudaEvent_t ev_next = nullptr, ev_panel = nullptr, ev_chain = nullptr, ev_left = nullptr;
   cudaMemPool_t pool = nullptr;   // staging temporaries (stream-ordered, memory kept across syncs)
   int num_sms = 0;
   int cluster_max_ctas = 0;   // largest cluster the device schedules for the LU panel kernel (set by lu_init_device)
@@ -173,7 +175,7 @@ neb_status svd_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
 neb_status factors_solve(neb_ctx* c, const double* d_b, int nrhs, double* d_out);
 size_t lu_panel_ws_bytes(int num_sms);
 // launch wrappers of the LU update kernels (A: column-major with leading dimension ld; Lp/ldl: the L operand, row index absolute)
-void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi);
+void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int npiv, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi);
 void lu_launch_trsm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int64_t c_first, int64_t ncols);
 void lu_launch_gemm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const double* Lp, int64_t ldl, int64_t k, int K, int64_t r0, int64_t m,
                     int64_t c_first, int64_t ncols, bool timed);

@@ -171,18 +171,19 @@ __global__ void __launch_bounds__(PANEL_THREADS) panel_kernel(double* __restrict
   }
 }
 
-// Row exchanges of panel k applied to the columns [c_lo, c_hi), minus the columns [skip_lo, skip_hi) (the panel's
-// own, and with look-ahead the next panel's, which were exchanged ahead of the others).  One thread per column.
-__global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, const int32_t* __restrict__ ipiv, int64_t c_lo,
+// The npiv (<= 256) row exchanges of the panels k, k + 64, ... applied in order to the columns [c_lo, c_hi), minus the
+// columns [skip_lo, skip_hi) (the panel's own, and with look-ahead the next panel's, which were exchanged ahead of the
+// others).  One thread per column; a whole 256-column block's exchanges take one launch.
+__global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, int npiv, const int32_t* __restrict__ ipiv, int64_t c_lo,
                              int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
-  __shared__ int s_piv[NB];
-  if (threadIdx.x < NB) s_piv[threadIdx.x] = ipiv[k + threadIdx.x];
+  __shared__ int s_piv[4 * NB];
+  for (int t = threadIdx.x; t < npiv; t += blockDim.x) s_piv[t] = ipiv[k + t];
   __syncthreads();
   int64_t c = c_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= skip_lo) c += skip_hi - skip_lo;
   if (c >= c_hi) return;
   double* col = A + c * ld;
-  for (int t = 0; t < NB; ++t) {
+  for (int t = 0; t < npiv; ++t) {
     int p = s_piv[t];
     if (p != k + t) {
       double a = col[k + t], bb = col[p];
@@ -444,11 +445,11 @@ neb_status lu_init_device(neb_ctx* c) {
 
 // Launch wrappers of the update kernels: used by lu_factor below and by the distributed factorisation (neb_dist.cu),
 // where A is a rank's local block of columns and the L operand (Lp, ldl) is the broadcast panel.
-void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo,
+void lu_launch_laswp(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, int64_t k, int npiv, int64_t c_lo, int64_t c_hi, int64_t skip_lo,
                      int64_t skip_hi) {
   const int64_t ncols = (c_hi - c_lo) - (skip_hi - skip_lo);
   if (ncols <= 0) return;
-  laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, st>>>(A, ld, k, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
+  laswp_kernel<<<(unsigned)((ncols + 127) / 128), 128, 0, st>>>(A, ld, k, npiv, c->d_ipiv, c_lo, c_hi, skip_lo, skip_hi);
   c->launches++;
 }
 
@@ -520,8 +521,8 @@ neb_status lu_factor(neb_ctx* c) {
     return NEB_OK;
   };
   // row exchanges of panel k on the columns [c_lo, c_hi) \ [skip_lo, skip_hi)
-  auto laswp = [&](cudaStream_t st, int64_t k, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
-    lu_launch_laswp(c, st, c->d_K, ld, k, c_lo, c_hi, skip_lo, skip_hi);
+  auto laswp = [&](cudaStream_t st, int64_t k, int npiv, int64_t c_lo, int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
+    lu_launch_laswp(c, st, c->d_K, ld, k, npiv, c_lo, c_hi, skip_lo, skip_hi);
   };
   // C[r0 .. r0+m, c_first .. c_first+ncols) -= A[r0 .., k .. k+K) * A[k .. k+K, c_first ..) on the tensor cores
   const bool timed = !c->lu_lookahead;
@@ -553,7 +554,7 @@ neb_status lu_factor(neb_ctx* c) {
     for (int64_t k = kb; k < nb; k += NB) {
       NEB_TRY(launch_panel(k, SC));
       const int64_t in_cols = nb - (k + NB);               // columns of this block right of the panel
-      laswp(SC, k, kb, nb, k, k + NB);                     // the block's other columns, left and right of the panel
+      laswp(SC, k, NB, kb, nb, k, k + NB);                 // the block's other columns, left and right of the panel
       trsm(SC, k, k + NB, in_cols);
       gemm(SC, k, NB, k + NB, npad - (k + NB), k + NB, in_cols);
     }
@@ -561,11 +562,19 @@ neb_status lu_factor(neb_ctx* c) {
       NEB_CUDA(c, cudaEventRecord(c->ev_panel, S2));
       NEB_CUDA(c, cudaStreamWaitEvent(S1, c->ev_panel, 0));
     }
+    // the block's pivots are final: its row exchanges on the finished columns to the LEFT go to a stream of their own
+    // (uncoalesced row traffic that nothing needs before the solves; on the main stream it delayed every update)
+    cudaStream_t SL = (c->lu_lookahead && c->left_stream) ? c->left_stream : S1;
+    if (SL != S1 && kb > 0) {
+      NEB_CUDA(c, cudaEventRecord(c->ev_chain, SC));
+      NEB_CUDA(c, cudaStreamWaitEvent(SL, c->ev_chain, 0));
+    }
+    laswp(SL, kb, (int)w, 0, kb, kb, kb);
     const int64_t right = npad - nb;                       // columns (and rows) of the trailing matrix
     // everything the factored block does to the columns [c0, c0 + nc) right of it
     auto wide = [&](int64_t c0, int64_t nc) {
       if (nc <= 0) return;
-      for (int64_t k = kb; k < nb; k += NB) laswp(S1, k, c0, c0 + nc, c0 + nc, c0 + nc);
+      laswp(S1, kb, (int)w, c0, c0 + nc, c0 + nc, c0 + nc);   // the block's w exchanges in one launch
       for (int64_t k = kb; k < nb; k += NB) {
         trsm(S1, k, c0, nc);
         gemm(S1, k, NB, k + NB, nb - (k + NB), c0, nc);    // rows of the block row still below this panel
@@ -582,10 +591,13 @@ neb_status lu_factor(neb_ctx* c) {
     } else {
       wide(nb, right);
     }
-    for (int64_t k = kb; k < nb; k += NB) laswp(S1, k, 0, kb, kb, kb);   // the factors to the left
     chain_on_side = ahead;
     NEB_CUDA(c, cudaGetLastError());
     kb = nb;
+  }
+  if (c->lu_lookahead && c->left_stream) {
+    NEB_CUDA(c, cudaEventRecord(c->ev_left, c->left_stream));
+    NEB_CUDA(c, cudaStreamWaitEvent(S1, c->ev_left, 0));
   }
   // composed permutation for the solves
   NEB_TRY(lu_finish_factors(c));
