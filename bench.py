@@ -41,9 +41,8 @@ sys.path.insert(0, ROOT)
 METRIC = "element-point influence pairs/s (fp64)"
 UNIT = "pairs/s"
 DEFAULT_WORKLOAD = "C2"
-# flop per rectangle pair when every element is evaluated on its own (NEB_OPT_PAIR_STRIPS = 0): the counts of the same
-# ncu table before the strip pairs (profiles/r2_opcounts.md, "Reading")
-ELEMENTWISE_RECT_FLOP = {"eval_rect_uniform": 243.2, "eval_images": 248.7}
+# cases of profiles/r2_opcounts.md that count the same pairs with every element evaluated on its own (NEB_OPT_PAIR_STRIPS = 0)
+ELEMENTWISE_CASE = {"eval_rect_uniform": "eval_rect_single", "eval_images": "eval_images_single"}
 L2_NOTE = "256 MiB buffer written between timed steps; the matrix exceeds L2"
 WORKLOADS = {
     "C1": "C1 cube: N=6144 rect panels, M=100000 points (BASELINE configs[1])",
@@ -371,7 +370,7 @@ class Runner:
             "frac_of_3operand_dfma_peak": ach / self.peaks["dfma3"],
             # the same pairs at the element-by-element operation count (strip pairs share an edge's two corner distances and
             # its logarithm: fewer executed flop for the same closed forms; profiles/r2_opcounts.md)
-            "frac_elementwise": ach / dfma * ELEMENTWISE_RECT_FLOP[rect_key] / ops[rect_key]["flop"],
+            "frac_elementwise": ach / dfma * ops[ELEMENTWISE_CASE[rect_key]]["flop"] / ops[rect_key]["flop"],
             "peak_source": "neb_fp64_peak(0): DFMA-chain microbenchmark run in this process (nominal 148 SM x 64 DFMA/clk x "
                            "2 x 1.965 GHz = 37.2); MEASURED_PEAKS.json has no FP64 entry",
             "constants_source": "profiles/r2_opcounts.md (ncu smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on per pair)"}))

@@ -169,6 +169,7 @@ neb_status neb_dist_factor_block(neb_ctx* c, int64_t g, double* panel, int32_t* 
   NEB_TRY(check_dist_block(c, g, "neb_dist_factor_block"));
   if (!c->dist_scaled) return fail(c, NEB_ESTATE, "neb_dist_factor_block before neb_dist_row_scales(set)");
   if (g % c->dist_world != c->dist_rank) return fail(c, NEB_EINVAL, "neb_dist_factor_block: this rank does not own the block");
+  if (!is_device_pointer(panel) || !is_device_pointer(piv)) return fail(c, NEB_EINVAL, "neb_dist_factor_block: panel and piv must be device pointers");
   NEB_CUDA(c, cudaSetDevice(c->device));
   cudaStream_t st = cuda_stream ? (cudaStream_t)cuda_stream : c->stream;
   const int64_t npad = c->npad, ld = npad, kb = g * DB, lc = (g / c->dist_world) * DB;
@@ -197,6 +198,7 @@ neb_status neb_dist_apply_block(neb_ctx* c, int64_t g, const double* panel, cons
   if (!c->dist_mode) return fail(c, NEB_ESTATE, "neb_dist_apply_block without neb_dist_configure");
   NEB_TRY(check_dist_block(c, g, "neb_dist_apply_block"));
   if (!c->dist_scaled) return fail(c, NEB_ESTATE, "neb_dist_apply_block before neb_dist_row_scales(set)");
+  if (!is_device_pointer(panel) || !is_device_pointer(piv)) return fail(c, NEB_EINVAL, "neb_dist_apply_block: panel and piv must be device pointers");
   NEB_CUDA(c, cudaSetDevice(c->device));
   cudaStream_t st = c->stream;
   const int world = c->dist_world, rank = c->dist_rank;
@@ -243,6 +245,7 @@ neb_status neb_dist_finish_factor(neb_ctx* c, int32_t* singular) {
 neb_status neb_dist_rhs(neb_ctx* c, double* y) {
   if (!c || !y) return NEB_EINVAL;
   if (!c->dist_mode || !c->factored) return fail(c, NEB_ESTATE, "neb_dist_rhs before the distributed factorisation");
+  if (!is_device_pointer(y)) return fail(c, NEB_EINVAL, "neb_dist_rhs: y must be a device pointer");
   NEB_CUDA(c, cudaSetDevice(c->device));
   NEB_TRY(form_rhs(c));
   dist_permute_scale_kernel<<<(unsigned)((c->npad + 255) / 256), 256, 0, c->stream>>>(c->d_b, c->d_rscale, c->d_rowperm, c->npad, y);
@@ -255,6 +258,7 @@ neb_status neb_dist_tri_block(neb_ctx* c, int32_t upper, int64_t g, double* y, d
   if (!c || !y || !acc) return NEB_EINVAL;
   if (!c->dist_mode || !c->factored) return fail(c, NEB_ESTATE, "neb_dist_tri_block before the distributed factorisation");
   NEB_TRY(check_dist_block(c, g, "neb_dist_tri_block"));
+  if (!is_device_pointer(y) || !is_device_pointer(acc)) return fail(c, NEB_EINVAL, "neb_dist_tri_block: y and acc must be device pointers");
   if (g % c->dist_world != c->dist_rank) return NEB_OK;          // not this rank's block: nothing to do
   NEB_CUDA(c, cudaSetDevice(c->device));
   StageTimer tt(c, NEB_STAGE_TRISOLVE);
@@ -282,6 +286,7 @@ neb_status neb_dist_tri_block(neb_ctx* c, int32_t upper, int64_t g, double* y, d
 neb_status neb_dist_set_solution(neb_ctx* c, const double* x, double* sigma_out) {
   if (!c || !x) return NEB_EINVAL;
   if (!c->dist_mode || !c->factored) return fail(c, NEB_ESTATE, "neb_dist_set_solution before the distributed factorisation");
+  if (!is_device_pointer(x)) return fail(c, NEB_EINVAL, "neb_dist_set_solution: x must be a device pointer");
   NEB_CUDA(c, cudaSetDevice(c->device));
   NEB_TRY(finish_sigma(c, x));
   if (sigma_out) {

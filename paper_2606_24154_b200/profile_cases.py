@@ -9,6 +9,8 @@ operation counts follow from ncu's per-launch `smsp__sass_thread_inst_executed_o
 
 Cases (all through the C ABI; inputs from workloads/, seeded):
   eval_rect_uniform   C1 cube (6144 rectangles on uniform-axes windows), 1e5 points            -> eval_kernel
+  eval_rect_single    the same with NEB_OPT_PAIR_STRIPS = 0 (every element on its own)         -> eval_kernel
+  eval_images_single  eval_images with NEB_OPT_PAIR_STRIPS = 0                                 -> eval_kernel
   eval_tri_uniform    4096 equally oriented right triangles (uniform windows), 1e5 points      -> eval_kernel
   eval_rect_general   4096 randomly oriented rectangles (general windows), 1e5 points          -> eval_kernel
   eval_tri_general    4096 randomly oriented right triangles, 1e5 points                       -> eval_kernel
@@ -52,9 +54,10 @@ def run(cases):
         ms, launches = nb.stage_ms()[stage]
         print(f"case {name} kernel {kernel} units {units:d} ms {ms:.4f} launches {launches}", flush=True)
 
-    def eval_case(name, pr, pts, sigma=None):
+    def eval_case(name, pr, pts, sigma=None, pairs=1):
         nb = Neb()
         nb.set_option(B.NEB_OPT_PROFILE, 1)
+        nb.set_option(B.NEB_OPT_PAIR_STRIPS, pairs)
         nb.assemble_problem(pr)
         nb.set_sigma(np.linspace(1e-8, 2e-8, pr.n) if sigma is None else sigma)
         d = torch.from_numpy(np.ascontiguousarray(pts)).cuda()
@@ -66,18 +69,18 @@ def run(cases):
 
     m = 100_000
     for name in cases:
-        if name == "eval_rect_uniform":
+        if name in ("eval_rect_uniform", "eval_rect_single"):
             pr = W.cube()
-            eval_case(name, pr, pr.points)
+            eval_case(name, pr, pr.points, pairs=int(name == "eval_rect_uniform"))
         elif name == "eval_tri_uniform":
             eval_case(name, _sawtooth_triangles(), _points(11, m, 15.0))
         elif name in ("eval_rect_general", "eval_tri_general", "eval_wire"):
             kind = {"eval_rect_general": W.RECT, "eval_tri_general": W.TRI, "eval_wire": W.WIRE}[name]
             pr = W.random_elements(4096, seed=12, kinds=(kind,), size_mm=(0.1, 0.3), box_mm=5.0)
             eval_case(name, pr, _points(13, m, 15.0))
-        elif name == "eval_images":
+        elif name in ("eval_images", "eval_images_single"):
             pr = W.double_thgem(d=20, n_plane=20, m_points=20_000)
-            eval_case(name, pr, pr.points)
+            eval_case(name, pr, pr.points, pairs=int(name == "eval_images"))
         elif name == "eval_near":
             pr = W.cube()
             rs = np.random.RandomState(3)
@@ -128,8 +131,8 @@ def run(cases):
             raise SystemExit(f"unknown case {name}")
 
 
-ALL = ["eval_rect_uniform", "eval_tri_uniform", "eval_rect_general", "eval_tri_general", "eval_wire", "eval_images",
-       "eval_near", "assemble_c2", "assemble_images", "charges", "lines", "lu_c1", "trisolve_c1"]
+ALL = ["eval_rect_uniform", "eval_rect_single", "eval_tri_uniform", "eval_rect_general", "eval_tri_general", "eval_wire", "eval_images",
+       "eval_images_single", "eval_near", "assemble_c2", "assemble_images", "charges", "lines", "lu_c1", "trisolve_c1"]
 
 if __name__ == "__main__":
     run(sys.argv[1:] or ALL)

@@ -1214,3 +1214,66 @@ def test_strip_pairs_equal_single_elements(P):
                         TOL_FAR, "strip pairs far", tuple(s[: pr.points.shape[1]] for s in scale))
             check_field(phi[pr.points.shape[1]:], E[:, pr.points.shape[1]:], phi_o[pr.points.shape[1]:], E_o[:, pr.points.shape[1]:],
                         TOL_NEAR, "strip pairs near", tuple(s[pr.points.shape[1]:] for s in scale))
+
+
+def test_dist_and_svd_call_order_errors(P):
+    """The scale-out and OptSVD calls refuse what include/neb.h says they refuse (status codes, no crash)."""
+    import torch
+    nb = P.Neb()
+    pr = W.plate(n_side=4)
+    f64 = dict(dtype=torch.float64, device="cuda")
+    with pytest.raises(P.NebError) as e:
+        nb.dist_configure(2, 2)                                    # rank outside [0, world)
+    assert e.value.status == 1
+    nb.assemble_problem(pr)
+    with pytest.raises(P.NebError) as e:
+        nb.dist_configure(0, 1)                                    # not on a fresh context
+    assert e.value.status == 3
+    with pytest.raises(P.NebError) as e:
+        nb.dist_row_scales(torch.empty(128, **f64), False)         # context is not distributed
+    assert e.value.status == 3
+    with pytest.raises(P.NebError) as e:
+        nb.get_singular_values(128)                                # no SVD factors
+    assert e.value.status == 3
+    with pytest.raises(P.NebError) as e:
+        nb.set_svd_cutoff(1.5)
+    assert e.value.status == 1
+    nb.close()
+    nd = P.Neb()
+    nd.dist_configure(0, 1)
+    nd.assemble_problem(pr)
+    npad = nd.dist_npad()
+    assert npad == 256
+    panel, piv = torch.empty(npad * 256, **f64), torch.empty(256, dtype=torch.int32, device="cuda")
+    with pytest.raises(P.NebError) as e:
+        nd.dist_factor_block(0, panel, piv)                        # before the row scales were agreed
+    assert e.value.status == 3
+    s = torch.empty(npad, **f64)
+    nd.dist_row_scales(s, False)
+    nd.dist_row_scales(s, True)
+    with pytest.raises(P.NebError) as e:
+        nd.dist_factor_block(1, panel, piv)                        # no such block
+    assert e.value.status == 1
+    with pytest.raises(P.NebError) as e:
+        nd.dist_factor_block(0, np.empty(npad * 256), piv)         # host pointer
+    assert e.value.status == 1
+    with pytest.raises(P.NebError) as e:
+        nd.dist_rhs(s)                                             # before the factorisation
+    assert e.value.status == 3
+    with pytest.raises(P.NebError) as e:
+        nd.get_matrix()                                            # each rank holds only its blocks
+    assert e.value.status == 3
+    nd.dist_factor_block(0, panel, piv)
+    nd.dist_apply_block(0, panel, piv, 0)
+    assert nd.dist_finish_factor() == 0
+    y, acc = torch.empty(npad, **f64), torch.zeros(npad, **f64)
+    nd.dist_rhs(y)
+    nd.dist_tri_block(False, 0, y, acc)
+    acc.zero_()
+    nd.dist_tri_block(True, 0, y, acc)
+    sig = nd.dist_set_solution(y, np.empty(pr.n))
+    one = P.Neb()
+    one.assemble_problem(pr)
+    assert np.max(np.abs(sig - one.solve())) <= TOL_SIGMA * np.max(np.abs(sig))
+    one.close()
+    nd.close()
