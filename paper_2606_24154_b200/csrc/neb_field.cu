@@ -112,9 +112,12 @@ __device__ __forceinline__ void far_copy(double area, double dx, double dy, doub
 // seq = number of tiles this CTA has consumed so far (buffer = seq & 1, mbarrier parity = (seq >> 1) & 1).
 // self0 (compile time: a runtime flag cost 4 % on the hot path): slot 0 of this chunk of copies is the element itself
 // (the first chunk); later chunks hold shifted copies only.
-template <class M, int KIND, bool self0, class Sink>
+// NIMG = 1: the element has no periodic copies — known at compile time, so that the copy loops and the Adaptive-Modelling
+// branch disappear from the tile loop (one straight block per pair of elements); NIMG = 0: n_img, n_near at run time.
+template <class M, int KIND, bool self0, int NIMG, class Sink>
 __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int64_t hi, TileSmem& sm, int n_img, int n_near,
                                              double px, double py, double pz, Sink& sink, unsigned& seq) {
+  if (NIMG == 1) { n_img = 1; n_near = 1; }
   const int64_t tb0 = lo & ~(int64_t)(kTile - 1);
   if (threadIdx.x == 0) tile_issue(sm, g, tb0, seq);
   for (int64_t tb = tb0; tb < hi; tb += kTile) {
@@ -242,18 +245,18 @@ __device__ __forceinline__ void process_kind(const GeoTables& g, int64_t lo, int
   }
 }
 
-template <class M, bool self0, class Sink>
+template <class M, bool self0, int NIMG, class Sink>
 __device__ __forceinline__ void process_range(const GeoTables& g, int64_t j0, int64_t j1, TileSmem& sm, int n_img, int n_near,
                                               double px, double py, double pz, Sink& sink) {
   int64_t r1 = g.n_rect, t1 = r1 + g.n_tri, w1 = t1 + g.n_wire;
   int64_t lo, hi;
   unsigned seq = 0;
   lo = max(j0, (int64_t)0); hi = min(j1, r1);
-  if (lo < hi) process_kind<M, 0, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 0, self0, NIMG>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, r1); hi = min(j1, t1);
-  if (lo < hi) process_kind<M, 1, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 1, self0, NIMG>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
   lo = max(j0, t1); hi = min(j1, w1);
-  if (lo < hi) process_kind<M, 2, self0>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
+  if (lo < hi) process_kind<M, 2, self0, NIMG>(g, lo, hi, sm, n_img, n_near, px, py, pz, sink, seq);
 }
 
 // img: one chunk of the copy table, [3][kMaxImg] (the host packs the sorted shifts in chunks of kMaxImg)
@@ -295,7 +298,7 @@ struct EvalSink {
 #ifndef NEB_EVAL_MINB
 #define NEB_EVAL_MINB 4
 #endif
-template <class M, bool FIRST>
+template <class M, bool FIRST, int NIMG>
 __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables g, const double* __restrict__ img, int n_img, int n_near,
                                                         const double* __restrict__ pts, int64_t m, int64_t per_split,
                                                         double* __restrict__ partial) {
@@ -309,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, NEB_EVAL_MINB) eval_kernel(GeoTables
   int64_t n = (int64_t)g.n_rect + g.n_tri + g.n_wire;
   int64_t j0 = (int64_t)blockIdx.y * per_split, j1 = min(n, j0 + per_split);
   EvalSink sink;
-  process_range<M, FIRST>(g, j0, j1, sm, n_img, n_near, px, py, pz, sink);
+  process_range<M, FIRST, NIMG>(g, j0, j1, sm, n_img, n_near, px, py, pz, sink);
   if (p < m) {
     double* o = partial + (int64_t)blockIdx.y * 4 * m;
     if (FIRST) { o[p] = sink.phi; o[m + p] = sink.ex; o[2 * m + p] = sink.ey; o[3 * m + p] = sink.ez; }
@@ -425,7 +428,7 @@ struct AsmSink {
 #ifndef NEB_ASM_MINB
 #define NEB_ASM_MINB 4
 #endif
-template <class M, bool FIRST>
+template <class M, bool FIRST, int NIMG>
 __global__ void __launch_bounds__(kThreads, NEB_ASM_MINB) assemble_kernel(GeoTables g, const double* __restrict__ img, int n_img,
                                                             const double* __restrict__ colloc, int64_t stride,
                                                             const double* __restrict__ normal,
@@ -452,7 +455,7 @@ __global__ void __launch_bounds__(kThreads, NEB_ASM_MINB) assemble_kernel(GeoTab
   sink.diag = diag[ic];
   double px = colloc[ic], py = colloc[stride + ic], pz = colloc[2 * stride + ic];
   int64_t j0 = gt * kTile, j1 = min(n, j0 + kTile);
-  process_range<M, FIRST>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
+  process_range<M, FIRST, NIMG>(g, j0, j1, sm, n_img, n_img, px, py, pz, sink);   // assembly is always exact
   // the running maximum of a row whose coefficients are still being summed is not the row's maximum: with several
   // chunks of copies only the LAST chunk's values (the finished coefficients) count
   if (i < n && rowmax_bits) atomicMax(rowmax_bits + i, (unsigned long long)__double_as_longlong(sink.rmax));
@@ -577,13 +580,16 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
       const int len = std::min(kMaxImg, c->n_img - ch * kMaxImg);
       const int near_ch = std::max(0, std::min(len, n_near - ch * kMaxImg));
       const double* img = c->d_img + (size_t)ch * 3 * kMaxImg;
+#define NEB_EVAL_ARGS tables(c), img, len, near_ch, d_pts, m, per_e, partial
       if (c->math_fast) {
-        if (ch == 0) eval_kernel<MathFast, true><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
-        else eval_kernel<MathFast, false><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+        if (c->n_img == 1) eval_kernel<MathFast, true, 1><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else if (ch == 0) eval_kernel<MathFast, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else eval_kernel<MathFast, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
       } else {
-        if (ch == 0) eval_kernel<MathLib, true><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
-        else eval_kernel<MathLib, false><<<grid, kThreads, 0, c->stream>>>(tables(c), img, len, near_ch, d_pts, m, per_e, partial);
+        if (ch == 0) eval_kernel<MathLib, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else eval_kernel<MathLib, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
       }
+#undef NEB_EVAL_ARGS
       c->launches++;
     }
     NEB_CUDA(c, cudaGetLastError());
@@ -628,11 +634,12 @@ neb_status assemble_matrix(neb_ctx* c) {
       unsigned long long* rm = (ch == n_chunks - 1) ? rowmax : nullptr;      // row maxima from the finished coefficients
 #define NEB_ASM_ARGS tables(c), img, len, c->d_colloc, c->stride, c->d_normal, c->d_bc_kind, c->d_diag, c->d_K, npad, rm, c->dist_world, c->dist_rank
       if (c->math_fast) {
-        if (ch == 0) assemble_kernel<MathFast, true><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
-        else assemble_kernel<MathFast, false><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        if (c->n_img == 1) assemble_kernel<MathFast, true, 1><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        else if (ch == 0) assemble_kernel<MathFast, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        else assemble_kernel<MathFast, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
       } else {
-        if (ch == 0) assemble_kernel<MathLib, true><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
-        else assemble_kernel<MathLib, false><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        if (ch == 0) assemble_kernel<MathLib, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
+        else assemble_kernel<MathLib, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_ASM_ARGS);
       }
 #undef NEB_ASM_ARGS
       c->launches++;
