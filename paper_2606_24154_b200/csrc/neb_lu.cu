@@ -19,6 +19,7 @@
 namespace neb {
 
 constexpr int NB = 64;           // panel width
+constexpr int kMaxBlockPanels = 16;   // widest outer block of lu_factor: 16 panels = 1024 columns
 constexpr int PANEL_THREADS = 256;
 
 // ------------------------------------------------------------------------------------------------
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(PANEL_THREADS) panel_kernel(double* __restrict
 // others).  One thread per column; a whole 256-column block's exchanges take one launch.
 __global__ void laswp_kernel(double* __restrict__ A, int64_t ld, int64_t k, int npiv, const int32_t* __restrict__ ipiv, int64_t c_lo,
                              int64_t c_hi, int64_t skip_lo, int64_t skip_hi) {
-  __shared__ int s_piv[4 * NB];
+  __shared__ int s_piv[kMaxBlockPanels * NB];
   for (int t = threadIdx.x; t < npiv; t += blockDim.x) s_piv[t] = ipiv[k + t];
   __syncthreads();
   int64_t c = c_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -533,20 +534,24 @@ neb_status lu_factor(neb_ctx* c) {
     lu_launch_trsm(c, st, c->d_K, ld, c->d_K + k * ld, ld, k, c_first, ncols);
   };
 
-  // Two-level right-looking factorisation.  Outer blocks of OB = 256 columns = 4 panels of 64:
+  // Two-level right-looking factorisation.  Outer blocks of w columns = w / 64 panels:
   //   chain   for each panel of the block: factor it, then apply its update (row exchanges, U12 = L11^-1 A12,
   //           rank-64 tensor-core update) to the REST OF THE BLOCK only;
-  //   wide    the block's row exchanges on all other columns, the block row of U (4 x [TRSM + small update]), and
-  //           ONE rank-256 tensor-core update of the whole trailing matrix: C is read and written once per 256
-  //           columns instead of once per 64 (32 flop per byte of C: compute-bound on the DMMA pipe).
-  // Look-ahead: the rank-256 update is applied to the next block's columns first; that block's chain (latency-bound,
+  //   wide    the block's row exchanges on all other columns, the block row of U (w / 64 x [TRSM + small update]), and
+  //           ONE rank-w tensor-core update of the whole trailing matrix: C is read and written once per w columns
+  //           instead of once per 64 (w / 8 flop per byte of C: compute-bound on the DMMA pipe).
+  // Look-ahead: the rank-w update is applied to the next block's columns first; that block's chain (latency-bound,
   // one cluster = 16 SMs per panel) then runs on the side stream while the main stream finishes the update on the
   // other SMs.  Only where the panels run on a cluster (the grid-wide panel kernel needs every SM).
-  // Block width: 256 while the trailing matrix is large (its update dominates and wants the depth); c->lu_nb (64 by
-  // default) once the remaining panels run on a cluster with look-ahead: there the chain of panels is the critical
-  // path and anything added to it (the in-block updates, a wider look-ahead slice) costs more than the deeper
-  // update saves.
-  auto block_width = [&](int64_t remaining) -> int64_t { return remaining > kChainRows ? 4 * NB : (int64_t)c->lu_nb; };
+  // Block width: the deeper the update, the smaller the share of a tile's life spent reading and writing C (the DMMA
+  // pipe idles there unless the SM's other CTA covers it) — 1024 while the trailing matrix exceeds 24576 rows, 512 down to
+  // 8192 rows, where the chain of a wider block still hides behind its update; c->lu_nb (64 by default) below: there
+  // the chain of panels is the critical path and anything added to it (the in-block updates, a wider look-ahead
+  // slice) costs more than the deeper update saves.
+  auto block_width = [&](int64_t remaining) -> int64_t {
+    if (remaining > 24576) return 16 * NB;     // measured on B200 (C3, whole factorisation): updates at 31.7 TFLOP/s; 512 throughout 30.8, 256 29.3
+    return remaining > kChainRows ? 8 * NB : (int64_t)c->lu_nb;
+  };
   bool chain_on_side = false;
   for (int64_t kb = 0; kb < npad;) {
     const int64_t w = min(block_width(npad - kb), npad - kb), nb = kb + w;
