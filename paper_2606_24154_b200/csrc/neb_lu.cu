@@ -281,12 +281,26 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+#ifndef NEB_GEMM_BAND
+#define NEB_GEMM_BAND 32
+#endif
+constexpr int kBandTiles = NEB_GEMM_BAND;   // row tiles (of 128 rows) per L2 band of the update
 __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restrict__ A, int64_t ld, const double* __restrict__ Lp, int64_t ldl,
-                                                               int64_t k, int K, int64_t r0, int64_t m, int64_t c_first) {
+                                                               int64_t k, int K, int64_t r0, int64_t m, int64_t c_first, int64_t tiles_n) {
   extern __shared__ __align__(16) double smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t i0 = r0 + (int64_t)blockIdx.x * GM;       // first row of the tile
-  const int64_t j0 = c_first + (int64_t)blockIdx.y * GN;  // first column
+  // Tile order (1-D grid): bands of kBandTiles row tiles; inside a band column by column, the band's row tiles
+  // innermost.  A band's slice of L (kBandTiles x 128 rows x K: 16 MB at K = 512) then stays in L2 while U streams past
+  // once per band; with the plain (row tiles fastest, all of them) order L (78 MB at C2, 400 MB at C3 for K = 1024) and U
+  // together overflow the 126 MB L2 and every CTA re-reads its operands from HBM (measured: 15.3 GB read by one
+  // rank-512 update of C2 whose C is 2.8 GB).
+  const unsigned tiles_m = (unsigned)((m + GM - 1) / GM), per_band = kBandTiles * (unsigned)tiles_n;
+  const unsigned band = blockIdx.x / per_band, within = blockIdx.x - band * per_band;
+  // (the last band may be shorter: its tiles are numbered after all full bands, so the division above is exact for it too)
+  const unsigned band_rows = min((unsigned)kBandTiles, tiles_m - band * kBandTiles);
+  const unsigned tile_n = within / band_rows, tile_m = band * kBandTiles + (within - tile_n * band_rows);
+  const int64_t i0 = r0 + (int64_t)tile_m * GM;           // first row of the tile
+  const int64_t j0 = c_first + (int64_t)tile_n * GN;      // first column
   const int rows_here = (int)min((int64_t)GM, r0 + m - i0);   // 64 or 128
   const int nchunks = K / GKC;
   // stage st <- chunk ch: sL[kk * LDL + i] = L[i][ch*32 + kk], sU[j * LDU + kk] = U[ch*32 + kk][j]
@@ -465,12 +479,13 @@ void lu_launch_gemm(neb_ctx* c, cudaStream_t st, double* A, int64_t ld, const do
                     int64_t m, int64_t c_first, int64_t ncols, bool timed) {
   if (m <= 0 || ncols <= 0) return;
   c->counter[NEB_COUNTER_GEMM_FLOP] += 2.0 * (double)m * (double)ncols * (double)K;
-  dim3 grid((unsigned)((m + GM - 1) / GM), (unsigned)(ncols / GN));
+  const int64_t tiles_n = ncols / GN;
+  const unsigned grid = (unsigned)(((m + GM - 1) / GM) * tiles_n);
   if (timed) {
     StageTimer tg(c, NEB_STAGE_LU_GEMM);
-    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first);
+    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first, tiles_n);
   } else {
-    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first);
+    gemm_kernel<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(A, ld, Lp, ldl, k, K, r0, m, c_first, tiles_n);
   }
   c->launches++;
 }
@@ -497,7 +512,13 @@ neb_status lu_factor(neb_ctx* c) {
   // panels run on one cluster (neb_lu_panel.cu) whatever their height; NEB_OPT_LU_PANEL = 1 selects the grid-wide
   // cooperative kernel of round 1 instead (all SMs, no look-ahead, n <= 148 x 384 - 128): kept as a cross-check
   const int64_t cluster_rows = c->panel_mode == 0 ? panel_cluster_max_rows(c) : 0;
-  constexpr int64_t kChainRows = 8192;     // below this the panel chain, not the update, is the critical path
+#ifndef NEB_LU_CHAIN_ROWS
+#define NEB_LU_CHAIN_ROWS 4096
+#endif
+#ifndef NEB_LU_MID_PANELS
+#define NEB_LU_MID_PANELS 2
+#endif
+  constexpr int64_t kChainRows = NEB_LU_CHAIN_ROWS;     // below this the panel chain, not the update, is the critical path
   cudaStream_t S1 = c->stream, S2 = c->side_stream;
 
   // panel k on stream st: the cluster kernel where the panel fits, else the grid-wide cooperative kernel
@@ -550,7 +571,8 @@ neb_status lu_factor(neb_ctx* c) {
   // slice) costs more than the deeper update saves.
   auto block_width = [&](int64_t remaining) -> int64_t {
     if (remaining > 24576) return 16 * NB;     // measured on B200 (C3, whole factorisation): updates at 31.7 TFLOP/s; 512 throughout 30.8, 256 29.3
-    return remaining > kChainRows ? 8 * NB : (int64_t)c->lu_nb;
+    if (remaining > 8192) return 8 * NB;
+    return remaining > kChainRows ? (int64_t)NEB_LU_MID_PANELS * NB : (int64_t)c->lu_nb;
   };
   bool chain_on_side = false;
   for (int64_t kb = 0; kb < npad;) {
