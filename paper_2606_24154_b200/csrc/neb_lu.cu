@@ -281,6 +281,10 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+#ifndef NEB_GEMM_UNROLL
+#define NEB_GEMM_UNROLL 8
+#endif
+constexpr int kGemmUnroll = NEB_GEMM_UNROLL;   // k4 steps of a chunk unrolled together
 #ifndef NEB_GEMM_BAND
 #define NEB_GEMM_BAND 32
 #endif
@@ -342,7 +346,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 2) gemm_kernel(double* __restric
     const double* sL = smem + (ch & 1) * GEMM_STAGE;
     const double* sU = sL + GKC * LDL;
     if (active) {
-#pragma unroll 2
+#pragma unroll kGemmUnroll
       for (int k4 = 0; k4 < GKC / 4; ++k4) {
         double fa[4], fb[4];
         // mma A operand (row = C column n, col = k): U[k4*4 + t][n = g]
