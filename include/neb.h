@@ -39,7 +39,7 @@ typedef enum {
   NEB_EINVAL = 1,    /* bad argument (NULL, negative size, unknown kind, degenerate element)  */
   NEB_ENOMEM = 2,    /* device or host allocation failed                                     */
   NEB_ESTATE = 3,    /* call out of order                                                    */
-  NEB_ESINGULAR = 4, /* zero or NaN pivot in the LU                                          */
+  NEB_ESINGULAR = 4, /* zero or NaN pivot in the LU; OptSVD sweeps that do not converge          */
   NEB_ECUDA = 5      /* CUDA runtime error; message in neb_last_error                        */
 } neb_status;
 
@@ -207,7 +207,8 @@ neb_status neb_push(neb_ctx* ctx, int64_t q, double* pos, const double* E, doubl
  * sigma = sum over s_j > rcond s_max of v_j (u_j . b) / s_j; neb_solve_weighting* and re-solves use the same factors.
  * neb_set_svd_cutoff: rcond in [0, 1), default 1e-10.  neb_get_singular_values (test hook): the npad singular values
  * in column order (the npad - n padding columns contribute exact ones), host or device, and the number of sweeps
- * the factorisation took (host, may be NULL); NEB_ESTATE without SVD factors. */
+ * the factorisation took (host, may be NULL); NEB_ESTATE without SVD factors.  neb_solve returns NEB_ESINGULAR if the
+ * rotations have not died out after 60 sweeps (a regular mesh takes 15-20). */
 neb_status neb_set_svd_cutoff(neb_ctx* ctx, double rcond);
 neb_status neb_get_singular_values(neb_ctx* ctx, double* s_out, int32_t* sweeps);
 

@@ -162,6 +162,7 @@ neb_status svd_factor(neb_ctx* c) {
   const double tol = 1e-15;
   constexpr int kMaxSweeps = 60;
   c->svd_sweeps = 0;
+  bool converged = false;
   for (int sweep = 0; sweep < kMaxSweeps; ++sweep) {
     NEB_CUDA(c, cudaMemsetAsync(d_rot, 0, sizeof(unsigned int), c->stream));
     for (int r = 0; r < n - 1; ++r) {
@@ -172,9 +173,10 @@ neb_status svd_factor(neb_ctx* c) {
     NEB_CUDA(c, cudaMemcpyAsync(&h_rot, d_rot, sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream));
     NEB_CUDA(c, cudaStreamSynchronize(c->stream));
     c->svd_sweeps = sweep + 1;
-    if (h_rot == 0) break;
+    if (h_rot == 0) { converged = true; break; }
   }
   cudaFreeAsync(d_rot, c->stream);
+  if (!converged) return fail(c, NEB_ESINGULAR, "OptSVD: the Jacobi sweeps did not converge (NaN/inf in the matrix?)");
   svd_norms_kernel<<<n, SV_THREADS, 0, c->stream>>>(c->d_K, npad, n, c->d_s2);
   svd_max_kernel<<<1, 1024, 0, c->stream>>>(c->d_s2, n);
   c->launches += 2;
