@@ -74,3 +74,30 @@ def test_config_shapes():
     c4 = W.space_charge(W.plate(), q_count=1000)
     assert c4.charge_pos.shape == (3, 1000) and np.all(c4.charge_q == W.Q_E)
     assert 0.8e-4 < c4.charge_pos.std() < 1.2e-4
+
+
+def test_bench_reads_its_roofline_constants_from_the_committed_tables():
+    """bench.py takes flop per pair and DRAM bytes per launch from profiles/*.md (ncu tables): every case it looks up must
+    be there and sane, or the driver's bench run would die on the GPU box."""
+    import importlib.util
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    ops = bench.load_opcounts()
+    need = ["eval_rect_uniform", "eval_rect_single", "eval_images", "eval_images_single", "eval_tri_uniform", "eval_wire",
+            "assemble_c2", "assemble_images", "charges"]
+    for case in need:
+        assert case in ops, case
+        o = ops[case]
+        assert 10.0 < o["flop"] < 400.0 and 5.0 < o["fp64_instr"] < 250.0
+        assert abs(o["flop"] - (2 * o["dfma"] + o["dmul"] + o["dadd"])) < 1e-9
+    for pair, single in bench.ELEMENTWISE_CASE.items():
+        assert ops[single]["flop"] > ops[pair]["flop"]                 # sharing an edge saves work, never adds
+    traffic = bench.load_bench_traffic()
+    for kern in ("eval_kernel", "assemble_kernel", "gemm_kernel"):
+        assert traffic[("C2", kern)] > 1e6
+    from workloads import configs as W
+    fl, inst = bench.flop_per_pair(W.thgem(d=10, n_plane=6, n_grid=2), ops)
+    assert ops["eval_tri_uniform"]["flop"] <= fl <= ops["eval_rect_uniform"]["flop"] and inst < fl
