@@ -49,11 +49,11 @@ enum { NEB_BC_DIRICHLET = 0, NEB_BC_DIELECTRIC = 1 };   /* row kinds            
 /* Options for neb_set_option. */
 enum {
   NEB_OPT_MATH = 0,     /* 1 (default): hand-written log/atan2/sqrt/rcp sequences; 0: CUDA libm  */
-  NEB_OPT_LU_BLOCK = 1, /* LU outer block width (64, 128 or 256) once the trailing matrix is <= 8192 rows;
-                           default 64; larger trailing matrices always use 256 (panels are 64 wide) */
+  NEB_OPT_LU_BLOCK = 1, /* LU outer block width (64, 128 or 256) once the trailing matrix is <= 4096 rows;
+                           default 64; above: 128 up to 8192 rows, 512 up to 24576, 1024 beyond (panels are 64 wide) */
   NEB_OPT_PROFILE = 2,  /* 1: record per-stage CUDA-event timings (neb_stage_ms); default 0      */
-  NEB_OPT_LU_PANEL = 3, /* 0 (default): cluster/DSMEM panel kernel where the panel fits (<= 8192 rows),
-                           grid-wide cooperative kernel above; 1: grid-wide kernel only          */
+  NEB_OPT_LU_PANEL = 3, /* 0 (default): panel kernel on one thread-block cluster (any height up to 131072 rows);
+                           1: the grid-wide cooperative kernel of round 1 (cross-check; n <= 56704) */
   NEB_OPT_EVAL_SPLITS = 5, /* 0 (default): neb_eval splits the elements / charges into as many chunks as fill the GPU for
                            the given number of points (few points -> many chunks); k > 0: always k chunks, so that the
                            fixed-order partial sums, hence the result BITS, do not depend on how many points a call
