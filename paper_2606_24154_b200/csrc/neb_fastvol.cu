@@ -49,10 +49,13 @@ __device__ __forceinline__ bool cell_of(double x, double o, double h, int n, int
   return true;
 }
 
-// one node record through the read-only path: two 16-byte loads of one 32-byte sector
+// one node record through the read-only path: ONE 32-byte load of its sector (sm_100: ld.global.nc.v4.f64, SASS LDG.E.256)
+// instead of two 16-byte loads — the lookup is bound by the L1/TEX request rate (every lane gathers its own sectors):
+// 1e7 lookups in C2's map 0.450 -> 0.427 ms
 __device__ __forceinline__ double4 load_node(const double4* p) {
-  const double2 a = __ldg(reinterpret_cast<const double2*>(p)), b = __ldg(reinterpret_cast<const double2*>(p) + 1);
-  return make_double4(a.x, a.y, b.x, b.y);
+  double4 v;
+  asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
 }
 
 __device__ __forceinline__ double4 lerp4(const double4& a, const double4& b, double f) {
