@@ -1086,7 +1086,8 @@ def _dist_rank_worker(rank, world, port, out_q):
         dist.destroy_process_group()
 
 
-def test_dist_lu_two_ranks_real_library():
+@pytest.mark.parametrize("world", [2, 3])
+def test_dist_lu_two_ranks_real_library(world):
     import socket
     import torch.multiprocessing as mp
     with socket.socket() as s:
@@ -1094,23 +1095,23 @@ def test_dist_lu_two_ranks_real_library():
         port = s.getsockname()[1]
     ctx = mp.get_context("spawn")
     out_q = ctx.Queue()
-    procs = [ctx.Process(target=_dist_rank_worker, args=(r, 2, port, out_q)) for r in range(2)]
+    procs = [ctx.Process(target=_dist_rank_worker, args=(r, world, port, out_q)) for r in range(world)]
     for p in procs:
         p.start()
-    got = dict(out_q.get(timeout=600) for _ in range(2))
+    got = dict(out_q.get(timeout=600) for _ in range(world))
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
     for which in ("mixed", "cube"):
         single = got[0][(which, "single")]
         for la in (True, False):
-            a, b = got[0][(which, la)], got[1][(which, la)]
-            assert np.array_equal(a, b), "both ranks must end with the same sigma"
+            a = got[0][(which, la)]
+            assert all(np.array_equal(a, got[r][(which, la)]) for r in range(1, world)), "every rank must end with the same sigma"
             assert np.max(np.abs(a - single)) <= TOL_SIGMA * np.max(np.abs(single)), which
         # with and without look-ahead the same operations run in the same order on every column: same bits
         assert np.array_equal(got[0][(which, True)], got[0][(which, False)])
         phi, phi1 = got[0][(which, "phi")], got[0][(which, "phi1")]
-        assert np.array_equal(phi, got[1][(which, "phi")])
+        assert all(np.array_equal(phi, got[r][(which, "phi")]) for r in range(1, world))
         assert np.max(np.abs(phi - phi1)) <= 1e-8 * np.max(np.abs(phi1))     # sigma differs by <= 1e-9 between the two solves
 
 
