@@ -174,6 +174,19 @@ neb_status neb_fastvol_get(neb_ctx* ctx, int32_t slot, double* values);
  * (reading S11).  Either output may be NULL.  m = 0 is allowed. */
 neb_status neb_eval(neb_ctx* ctx, int64_t m, const double* pts, double* phi, double* E);
 
+/* neb_eval without any allocation (for callers under CUDA graph capture, in tight serving loops, or in harnesses that
+ * forbid cudaMalloc): the same kernels and the same result as neb_eval to rounding (the elements / charges may be cut
+ * into fewer chunks, i.e. a different but equally fixed summation order), with the per-chunk partial sums in a
+ * file-scope device array of 32 MiB that every GPU holds from the moment the library is loaded until the process exits,
+ * instead of a buffer that grows with m.  Limits: m <= NEB_EVAL_STATIC_MAX_POINTS per call (NEB_EINVAL beyond, with
+ * the limit in neb_last_error); pts, phi, E must be DEVICE pointers (NEB_EINVAL otherwise: staging a host buffer would
+ * allocate); either output may be NULL.  The call issues kernels on the context's stream and calls no cudaMalloc,
+ * cudaFree or other allocating routine.  All contexts of a device share the one array: calls that overlap on the GPU
+ * (contexts on different streams) race on it; calls on one stream are ordered and need no clearing in between (every
+ * call overwrites the part it reads). */
+#define NEB_EVAL_STATIC_MAX_POINTS 65536
+neb_status neb_eval_static(neb_ctx* ctx, int64_t m, const double* pts, double* phi, double* E);
+
 /* UpdateSpaceCharge: q point charges, pos 3*q SoA (m), charge in coulomb.
  * replace != 0 discards the charges held so far; q = 0 with replace clears them. */
 neb_status neb_add_space_charge(neb_ctx* ctx, int64_t q, const double* pos, const double* charge, int32_t replace);

@@ -10,6 +10,7 @@ from . import build as _build
 NEB_RECT, NEB_TRI, NEB_WIRE = 0, 1, 2
 NEB_BC_DIRICHLET, NEB_BC_DIELECTRIC = 0, 1
 NEB_DIST_BLOCK = 256
+NEB_EVAL_STATIC_MAX_POINTS = 65536
 NEB_OPT_MATH, NEB_OPT_LU_BLOCK, NEB_OPT_PROFILE, NEB_OPT_LU_PANEL, NEB_OPT_LU_LOOKAHEAD, NEB_OPT_EVAL_SPLITS, NEB_OPT_SOLVER, NEB_OPT_PAIR_STRIPS = 0, 1, 2, 3, 4, 5, 6, 7
 STAGES = ["geometry", "assemble", "equil", "lu", "lu_gemm", "rhs", "trisolve", "eval", "charges", "reduce", "fastvol"]
 _STATUS = {1: "NEB_EINVAL", 2: "NEB_ENOMEM", 3: "NEB_ESTATE", 4: "NEB_ESINGULAR", 5: "NEB_ECUDA"}
@@ -53,6 +54,7 @@ def lib():
         L.neb_solve.argtypes = [vp, vp]
         L.neb_set_sigma.argtypes = [vp, vp]
         L.neb_eval.argtypes = [vp, i64, vp, vp, vp]
+        L.neb_eval_static.argtypes = [vp, i64, vp, vp, vp]
         L.neb_add_space_charge.argtypes = [vp, i64, vp, vp, i32]
         L.neb_solve_weighting.argtypes = [vp, vp, vp]
         L.neb_solve_weighting_multi.argtypes = [vp, i32, vp, vp]
@@ -205,6 +207,12 @@ class Neb:
             if E is None and want_E:
                 E = torch.empty((3, m), dtype=torch.float64, device=pts.device)
         self._ck(self._L.neb_eval(self._h, m, _ptr(pts), _ptr(phi), _ptr(E)))
+        return phi, E
+
+    def eval_static(self, pts, phi, E):
+        """neb_eval_static: pts (3, m), phi (m) and E (3, m) are contiguous float64 CUDA tensors supplied by the caller
+        (either output may be None); m <= NEB_EVAL_STATIC_MAX_POINTS; nothing is allocated, here or in the library."""
+        self._ck(self._L.neb_eval_static(self._h, int(pts.shape[1]), _ptr(pts), _ptr(phi), _ptr(E)))
         return phi, E
 
     def add_space_charge(self, pos, charge, replace=True):

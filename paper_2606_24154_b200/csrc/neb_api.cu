@@ -400,6 +400,7 @@ neb_status neb_create(neb_ctx** out, int device, void* cuda_stream) {
   for (int s = 0; ok && s < NEB_STAGE_COUNT; ++s)
     ok = cudaEventCreate(&c->ev0[s]) == cudaSuccess && cudaEventCreate(&c->ev1[s]) == cudaSuccess;
   ok = ok && lu_init_device(c) == NEB_OK;
+  ok = ok && field_static_init(c) == NEB_OK;   // device address of the fixed scratch of neb_eval_static
   if (!ok) {
     neb_destroy(c);
     return NEB_ECUDA;
@@ -671,6 +672,17 @@ neb_status neb_get_singular_values(neb_ctx* c, double* s_out, int32_t* sweeps) {
   NEB_CUDA(c, cudaMemcpy(s_out, h.data(), sizeof(double) * c->npad, cudaMemcpyDefault));
   if (sweeps) *sweeps = c->svd_sweeps;
   return NEB_OK;
+}
+
+neb_status neb_eval_static(neb_ctx* c, int64_t m, const double* pts, double* phi, double* E) {
+  if (!c || m < 0 || (m > 0 && !pts)) return NEB_EINVAL;
+  if (!c->have_sigma) return fail(c, NEB_ESTATE, "neb_eval_static before neb_solve / neb_set_sigma");
+  if (m == 0) return NEB_OK;
+  NEB_CUDA(c, cudaSetDevice(c->device));
+  // device pointers only: staging a host buffer would need a temporary, and this entry point allocates nothing
+  if (!is_device_ptr(pts) || (phi && !is_device_ptr(phi)) || (E && !is_device_ptr(E)))
+    return fail(c, NEB_EINVAL, "neb_eval_static: pts, phi and E must be device pointers");
+  return field_at_points_static(c, m, pts, phi, E);
 }
 
 neb_status neb_set_adaptive(neb_ctx* c, double far_distance) {

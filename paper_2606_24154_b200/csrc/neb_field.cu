@@ -617,6 +617,113 @@ neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_
   return NEB_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// neb_eval_static: the fused evaluation (a7 + a8) for callers that may not allocate (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  Same kernels as field_at_points; the per-chunk partial sums,
+// which field_at_points keeps in a cudaMalloc'ed buffer that grows with m, live in a file-scope device array of fixed
+// size instead: kStaticScratchDoubles doubles = 32 MiB, held by every GPU that loads the library until the process
+// exits.  In host code the array's NAME is a host-side stand-in, not a device address: its device address is taken once
+// per context (= per device, with that device current) by cudaGetSymbolAddress in field_static_init, from neb_create.
+// Every call on every context of a device shares the array; the kernels overwrite the part they use before they read it
+// (each chunk's first launch stores, nothing accumulates across calls), so nothing has to be cleared between calls —
+// but two calls that overlap on the GPU (different streams, or contexts on different streams) race on it.
+// ------------------------------------------------------------------------------------------------
+constexpr int64_t kStaticScratchDoubles = (int64_t)4 << 20;                   // 32 MiB
+constexpr int64_t kStaticMaxPoints = NEB_EVAL_STATIC_MAX_POINTS;              // 65536: leaves room for >= 16 chunks
+static __device__ __align__(256) double g_static_partial[kStaticScratchDoubles];
+
+neb_status field_static_init(neb_ctx* c) {
+  void* ptr = nullptr;
+  cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_partial);
+  if (e != cudaSuccess || !ptr) {
+    cudaGetLastError();
+    return fail(c, NEB_ECUDA, std::string("cudaGetSymbolAddress(g_static_partial): ") + cudaGetErrorString(e));
+  }
+  c->d_static_partial = (double*)ptr;
+  return NEB_OK;
+}
+
+neb_status field_at_points_static(neb_ctx* c, int64_t m, const double* d_pts, double* d_phi, double* d_E) {
+  if (m <= 0) return NEB_OK;
+  if (m > kStaticMaxPoints)
+    return fail(c, NEB_EINVAL, "neb_eval_static: at most " + std::to_string(kStaticMaxPoints) + " points per call (fixed 32 MiB scratch); got " +
+                                   std::to_string(m) + " - split the points or use neb_eval");
+  if (!c->d_static_partial) return fail(c, NEB_ESTATE, "neb_eval_static: the static scratch was not set up for this context");
+  const bool use_lines = c->n_lines > 0, use_charges = c->q > 0;
+  const int64_t pt_blocks = (m + kThreads - 1) / kThreads;
+  int se = pick_splits(pt_blocks, c->n, kTile, c->num_sms, c->eval_splits);
+  int sq = use_charges ? pick_splits(pt_blocks, c->q, kChargeTile, c->num_sms, c->eval_splits) : 0;
+  int sl = use_lines ? pick_splits(pt_blocks, c->n_lines, 256, c->num_sms, c->eval_splits) : 0;
+  // the chunk counts are cut down until the partial sums fit the fixed array (fewer, longer chunks: same result to
+  // rounding, a little less parallelism for small m)
+  const int64_t budget = kStaticScratchDoubles / (4 * m);
+  while ((int64_t)se + sq + sl > budget) {
+    if (se >= sq && se >= sl && se > 1) --se;
+    else if (sq >= sl && sq > 1) --sq;
+    else if (sl > 1) --sl;
+    else return fail(c, NEB_EINVAL, "neb_eval_static: the partial sums do not fit the static scratch");
+  }
+  int64_t per_e = (c->n + se - 1) / se, per_q = 0, per_l = 0;
+  per_e = (per_e + kTile - 1) / kTile * kTile;
+  se = (int)((c->n + per_e - 1) / per_e);
+  if (sq) {
+    per_q = (c->q + sq - 1) / sq;
+    per_q = (per_q + kChargeTile - 1) / kChargeTile * kChargeTile;
+    sq = (int)((c->q + per_q - 1) / per_q);
+  }
+  if (sl) {
+    per_l = (c->n_lines + sl - 1) / sl;
+    per_l = (per_l + 255) / 256 * 256;
+    sl = (int)((c->n_lines + per_l - 1) / per_l);
+  }
+  double* partial = c->d_static_partial;
+  int n_near = c->n_img;
+  if (c->adaptive_far > 0.0) {
+    n_near = 1;
+    while (n_near < c->n_img && c->h_img_len[(size_t)n_near] < c->adaptive_far) ++n_near;
+  }
+  {
+    StageTimer t(c, NEB_STAGE_EVAL);
+    dim3 grid((unsigned)pt_blocks, (unsigned)se);
+    for (int ch = 0; ch * kMaxImg < c->n_img; ++ch) {
+      const int len = std::min(kMaxImg, c->n_img - ch * kMaxImg);
+      const int near_ch = std::max(0, std::min(len, n_near - ch * kMaxImg));
+      const double* img = c->d_img + (size_t)ch * 3 * kMaxImg;
+#define NEB_EVAL_ARGS tables(c), img, len, near_ch, d_pts, m, per_e, partial
+      if (c->math_fast) {
+        if (c->n_img == 1) eval_kernel<MathFast, true, 1><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else if (ch == 0) eval_kernel<MathFast, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else eval_kernel<MathFast, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+      } else {
+        if (ch == 0) eval_kernel<MathLib, true, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+        else eval_kernel<MathLib, false, 0><<<grid, kThreads, 0, c->stream>>>(NEB_EVAL_ARGS);
+      }
+#undef NEB_EVAL_ARGS
+      c->launches++;
+    }
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  if (sq) {
+    StageTimer t(c, NEB_STAGE_CHARGES);
+    dim3 grid((unsigned)((m + kThreads * kChargePpt - 1) / (kThreads * kChargePpt)), (unsigned)sq);
+    charge_kernel<<<grid, kThreads, 0, c->stream>>>(c->d_charges, c->q, c->q_cap, d_pts, m, per_q, partial + (size_t)se * 4 * m);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  if (sl) {
+    StageTimer t(c, NEB_STAGE_CHARGES);
+    launch_line_kernel(c, m, d_pts, sl, per_l, partial + (size_t)(se + sq) * 4 * m);
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  {
+    StageTimer t(c, NEB_STAGE_REDUCE);
+    reduce_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(partial, se, sq + sl, m, d_phi, d_E);
+    c->launches++;
+    NEB_CUDA(c, cudaGetLastError());
+  }
+  return NEB_OK;
+}
+
 neb_status assemble_matrix(neb_ctx* c) {
   int64_t n = c->n, npad = c->npad;
   c->counter[NEB_COUNTER_MATRIX_BYTES] = 8.0 * (double)n * (double)(c->dist_mode ? std::min(c->ncol_loc, n) : n);

@@ -114,6 +114,8 @@ struct neb_ctx {
 
   neb::FastVol fastvol[NEB_FASTVOL_SLOTS];
 
+  double* d_static_partial = nullptr;   // device address of neb_field.cu's file-scope scratch array (neb_eval_static)
+
   // scratch for partial sums / staging
   double* d_scratch = nullptr;
   size_t scratch_bytes = 0;
@@ -158,6 +160,9 @@ struct StageTimer {   // records device time of a stage when profiling is on
 // Phi/E at m device points (SoA) from the elements (weights in rec field 15) and/or the charges.
 neb_status field_at_points(neb_ctx* c, int64_t m, const double* d_pts, bool use_elements, bool use_charges,
                            double* d_phi, double* d_E);
+// neb_eval_static: the same evaluation with the partial sums in a fixed file-scope device array (no allocation)
+neb_status field_static_init(neb_ctx* c);   // cudaGetSymbolAddress of that array, once per context, from neb_create
+neb_status field_at_points_static(neb_ctx* c, int64_t m, const double* d_pts, double* d_phi, double* d_E);
 neb_status assemble_matrix(neb_ctx* c);   // a3 + S15 row scales (computed, not yet applied)
 neb_status scale_matrix_rows(neb_ctx* c); // applies the row scales in place
 neb_status form_rhs(neb_ctx* c);          // a4 -> d_b (unscaled, sorted order)
