@@ -203,6 +203,10 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        # torchrun sets OMP_NUM_THREADS=1 for its workers; the one rank that runs the oracle gets the box's cores back
+        # (read by the OpenMP runtime when the oracle's library is loaded, below)
+        os.environ["OMP_NUM_THREADS"] = str(len(os.sched_getaffinity(0)))
     pr = load_problem(args.workload, args.m_points)
     copies = max(1, pr.n_img)
     n_rows, n_pts = max(1, 1024 // copies), max(1, 20000 // copies)
@@ -519,9 +523,17 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # NEB_BENCH_BACKEND=gloo: rehearsal of the multi-rank path on a box with fewer GPUs than ranks (the ranks then share
+    # devices and the two collectives of this script, barrier and max, run on the host); never a measurement
+    backend = os.environ.get("NEB_BENCH_BACKEND", "nccl")
+    if backend != "nccl":
+        local = local % max(1, torch.cuda.device_count())
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
     dev = torch.device("cuda", local)
     ops, traffic = load_opcounts(), load_bench_traffic()
     peaks = measure_peaks(P, local)
@@ -561,6 +573,7 @@ def main():
             "metric": METRIC, "value": rn.pairs_step * args.steps * world / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": make_config(name, pr, rn.m, rn.q),
+            **({"rehearsal": f"backend {backend}: ranks may share a GPU; not a measurement"} if backend != "nccl" else {}),
             "e2e": {"value": rn.pairs_step * args.steps * world / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": rn.h2d,
                     "d2h_bytes_per_step": rn.d2h, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": launches, "clocks": _clocks_summary(samples),

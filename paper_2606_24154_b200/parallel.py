@@ -30,6 +30,8 @@ def max_over_ranks(value: float, device="cpu") -> float:
     """Max of a per-rank scalar (a device-measured time); identity without a process group."""
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
         return float(value)
+    if dist.get_backend() == "gloo":
+        device = "cpu"                      # CPU-only backend (tests, rehearsals): reduce on the host
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
