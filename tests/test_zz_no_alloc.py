@@ -91,3 +91,33 @@ def test_eval_static_on_a_second_context_and_without_charges():
         _close(phi, ref_phi, "Phi")
         _close(E, ref_E, "E")
     nb.close()
+
+
+def test_eval_static_with_many_copies_lines_and_adaptive_modelling():
+    """The branches of the launch logic that neb_eval_static repeats from neb_eval: more than 32 periodic copies (several
+    launches per call, later ones ADD to the partial sums the first one stored — on an array that still holds another
+    call's values), line charges from the voxelisation beside point charges, far copies simplified."""
+    import torch
+    import paper_2606_24154_b200 as P
+    pr = W.double_thgem(d=10, n_plane=10, m_points=3000, k_img=3)          # 7 x 7 = 49 copies: two chunks of the copy table
+    assert pr.n_img == 49
+    rs = np.random.RandomState(6)
+    nb = P.Neb()
+    nb.assemble_problem(pr)
+    nb.set_sigma(rs.uniform(1e-8, 3e-8, pr.n))
+    pos = rs.normal(size=(3, 2000)) * 1e-4
+    nb.add_space_charge(pos, np.full(2000, W.Q_E * 1e5))
+    assert nb.voxelize_space_charge(np.full(3, -4e-4), np.full(3, 1e-4), np.full(3, 8, dtype=np.int32)) > 0
+    nb.add_space_charge(rs.normal(size=(3, 500)) * 1e-4, np.full(500, W.Q_E * 1e5), replace=False)   # points beside the lines
+    pts = torch.from_numpy(pr.points).cuda().contiguous()
+    f64 = dict(dtype=torch.float64, device="cuda")
+    junk = torch.from_numpy(pr.points[:, ::-1].copy() * 0.5).cuda().contiguous()
+    for far in (0.0, 2.5e-3):
+        nb.set_adaptive(far)
+        nb.eval_static(junk, torch.empty(3000, **f64), torch.empty((3, 3000), **f64))     # leaves other values in the array
+        phi, E = torch.empty(3000, **f64), torch.empty((3, 3000), **f64)
+        nb.eval_static(pts, phi, E)
+        ref_phi, ref_E = nb.eval(pts)
+        _close(phi, ref_phi, f"Phi, far={far}")
+        _close(E, ref_E, f"E, far={far}")
+    nb.close()
