@@ -298,8 +298,8 @@ __global__ void finish_sigma_kernel(int64_t n, int64_t stride, const int32_t* __
 __global__ void unpermute_matrix_kernel(int64_t n, int64_t ld, const int32_t* __restrict__ perm, const double* __restrict__ K,
                                         double* __restrict__ out) {
   int64_t si = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  int64_t sj = blockIdx.y;
-  if (si < n) out[(int64_t)perm[si] + (int64_t)perm[sj] * n] = K[si + sj * ld];
+  if (si >= n) return;
+  for (int64_t sj = blockIdx.y; sj < n; sj += gridDim.y) out[(int64_t)perm[si] + (int64_t)perm[sj] * n] = K[si + sj * ld];
 }
 
 __global__ void inverse_perm_kernel(int64_t n, const int32_t* __restrict__ perm, int32_t* __restrict__ inv) {
@@ -833,7 +833,7 @@ neb_status neb_get_matrix(neb_ctx* c, double* K_out) {
   Staging sg(c);
   void* dout;
   NEB_TRY(sg.out(K_out, sizeof(double) * (size_t)c->n * (size_t)c->n, &dout));
-  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)c->n);
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)std::min<int64_t>(c->n, 65535));
   unpermute_matrix_kernel<<<grid, 256, 0, c->stream>>>(c->n, c->npad, c->d_perm, c->d_K, (double*)dout);
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());

@@ -463,10 +463,12 @@ __global__ void __launch_bounds__(kThreads, NEB_ASM_MINB) assemble_kernel(GeoTab
 
 // distributed layout: rows n..npad of every local column, and the local columns whose global index is >= n
 __global__ void pad_identity_dist_kernel(double* K, int64_t n, int64_t npad, int64_t ncol_loc, int world, int rank) {
-  const int64_t lc = blockIdx.y, gc = ((lc >> 8) * world + rank) * 256 + (lc & 255);
-  const int64_t i0 = gc >= n ? 0 : n;
-  for (int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < npad; i += (int64_t)gridDim.x * blockDim.x)
-    K[i + lc * npad] = (i == gc) ? 1.0 : 0.0;
+  for (int64_t lc = blockIdx.y; lc < ncol_loc; lc += gridDim.y) {
+    const int64_t gc = ((lc >> 8) * world + rank) * 256 + (lc & 255);
+    const int64_t i0 = gc >= n ? 0 : n;
+    for (int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < npad; i += (int64_t)gridDim.x * blockDim.x)
+      K[i + lc * npad] = (i == gc) ? 1.0 : 0.0;
+  }
 }
 
 // rows/columns >= n of the padded matrix: identity
@@ -494,10 +496,12 @@ __global__ void rscale_kernel(const unsigned long long* rowmax_bits, int64_t n, 
   rscale[i] = (mx > 0.0) ? 1.0 / mx : (dist ? __longlong_as_double(0x7ff0000000000000LL) : 1.0);
 }
 
-__global__ void scale_rows_kernel(double* K, int64_t n, int64_t ld, const double* __restrict__ rscale) {
+// grid.y covers the columns with a stride (a grid's y extent ends at 65535, the matrix at 131072 columns)
+__global__ void scale_rows_kernel(double* K, int64_t n, int64_t ncols, int64_t ld, const double* __restrict__ rscale) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  int64_t j = blockIdx.y;
-  if (i < n) K[i + j * ld] *= rscale[i];
+  if (i >= n) return;
+  const double s = rscale[i];
+  for (int64_t j = blockIdx.y; j < ncols; j += gridDim.y) K[i + j * ld] *= s;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -754,7 +758,7 @@ neb_status assemble_matrix(neb_ctx* c) {
     NEB_CUDA(c, cudaGetLastError());
     int64_t padcells = (npad - n) * npad + n * (npad - n);
     if (dist) {
-      pad_identity_dist_kernel<<<dim3(4, (unsigned)c->ncol_loc), 256, 0, c->stream>>>(c->d_K, n, npad, c->ncol_loc, c->dist_world, c->dist_rank);
+      pad_identity_dist_kernel<<<dim3(4, (unsigned)std::min<int64_t>(c->ncol_loc, 65535)), 256, 0, c->stream>>>(c->d_K, n, npad, c->ncol_loc, c->dist_world, c->dist_rank);
       c->launches++;
       NEB_CUDA(c, cudaGetLastError());
     } else if (padcells > 0) {
@@ -776,8 +780,9 @@ neb_status assemble_matrix(neb_ctx* c) {
 // returns the unscaled matrix without a second copy).
 neb_status scale_matrix_rows(neb_ctx* c) {
   StageTimer t(c, NEB_STAGE_EQUIL);
-  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)(c->dist_mode ? c->ncol_loc : c->n));   // pad columns are zero above row n
-  scale_rows_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, c->n, c->npad, c->d_rscale);
+  const int64_t ncols = c->dist_mode ? c->ncol_loc : c->n;   // pad columns are zero above row n
+  dim3 grid((unsigned)((c->n + 255) / 256), (unsigned)std::min<int64_t>(ncols, 65535));
+  scale_rows_kernel<<<grid, 256, 0, c->stream>>>(c->d_K, c->n, ncols, c->npad, c->d_rscale);
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());
   return NEB_OK;

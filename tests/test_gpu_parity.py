@@ -1278,3 +1278,36 @@ def test_dist_and_svd_call_order_errors(P):
     assert np.max(np.abs(sig - one.solve())) <= TOL_SIGMA * np.max(np.abs(sig))
     one.close()
     nd.close()
+
+
+def test_more_than_65535_elements(P, orc):
+    """N = 66150 (cube, 105 x 105 panels per face; 35 GB matrix): beyond 2^16 - 1 columns (the y extent of a CUDA grid) and,
+    at 17 rows per thread of the panel cluster, on the panel kernel's 32-rows-per-thread variant, which no BASELINE
+    config reaches.  Sampled matrix rows entry by entry against the oracle, the residual of sigma on those oracle rows,
+    the cube's capacitance against the converged value of the C1 sequence, sampled field points."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 45e9:
+        pytest.skip("needs 45 GB of free device memory")
+    pr = W.cube(n_side=105, m_points=64)
+    assert pr.n == 66150 > 65535
+    g = orc.Geometry(pr)
+    rs = np.random.RandomState(13)
+    rows = np.sort(np.concatenate([rs.choice(pr.n, 30, replace=False), [0, 65535, 65536, pr.n - 1]]))
+    R, Cc = np.repeat(rows, pr.n), np.tile(np.arange(pr.n), rows.size)
+    Krows = orc.matrix_entries(g, R, Cc, mode="f64").reshape(rows.size, pr.n)
+    nb = P.Neb()
+    nb.assemble_problem(pr)
+    Kg = nb.get_matrix_rows(rows)
+    assert np.max(np.abs(Kg - Krows) / np.abs(Krows).max(axis=1, keepdims=True)) <= TOL_K
+    s = nb.solve()
+    gs = _rows_geometry(orc, g, rows)
+    res = np.abs(Krows @ s - orc.rhs(gs, mode="f64")) / (np.abs(Krows).sum(axis=1) * np.abs(s).max())
+    assert res.max() <= 1e-12, res.max()
+    side = pr.meta["side"]
+    cap = s.sum() * (side / 105) ** 2 / (4 * np.pi * orc.EPS0 * side)        # C / (4 pi eps0 a) at 1 V
+    assert 0.6595 < cap < 0.6608, cap                                        # unit cube: 0.66078 approached from below
+    phi, E = nb.eval(pr.points)
+    phi_o, E_o, scale = truth(orc, g, s, pr.points)
+    check_field(phi, E, phi_o, E_o, TOL_FAR, "N=66150", scale)
+    nb.close()
