@@ -409,12 +409,23 @@ __global__ void __launch_bounds__(1024) compose_perm_kernel(const int32_t* __res
   for (int i = threadIdx.x; i < npad; i += blockDim.x) rowperm[i] = s_perm[i];
 }
 
-__global__ void compose_perm_global_kernel(const int32_t* __restrict__ ipiv, int32_t* rowperm, int npad) {
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    for (int i = 0; i < npad; ++i) rowperm[i] = i;
-    for (int i = 0; i < npad; ++i) {
-      int p = ipiv[i];
-      if (p != i) { int tmp = rowperm[i]; rowperm[i] = rowperm[p]; rowperm[p] = tmp; }
+// The same for matrices whose permutation does not fit shared memory (npad > ~5e4): one CTA fills the identity in
+// parallel; its first warp then reads 32 pivots at a time (one coalesced load), a ballot finds the positions that really
+// exchange, and lane 0 applies those exchanges in order (the exchanges are sequential by nature, but few).
+__global__ void __launch_bounds__(1024) compose_perm_global_kernel(const int32_t* __restrict__ ipiv, int32_t* rowperm, int npad) {
+  for (int i = threadIdx.x; i < npad; i += blockDim.x) rowperm[i] = i;
+  __syncthreads();
+  if (threadIdx.x >= 32) return;
+  const int lane = threadIdx.x;
+  for (int base = 0; base < npad; base += 32) {
+    const int i = base + lane;
+    const int p = (i < npad) ? ipiv[i] : i;
+    unsigned m = __ballot_sync(0xffffffffu, p != i);
+    while (m) {                                            // warp-uniform
+      const int b = __ffs(m) - 1;
+      m &= m - 1;
+      const int pp = __shfl_sync(0xffffffffu, p, b);
+      if (lane == 0) { const int ii = base + b, tmp = rowperm[ii]; rowperm[ii] = rowperm[pp]; rowperm[pp] = tmp; }
     }
   }
 }
@@ -500,7 +511,7 @@ neb_status lu_finish_factors(neb_ctx* c) {
   if ((size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * 4 <= 200 * 1024) {
     compose_perm_kernel<<<1, 1024, (size_t)npad * sizeof(int) + (size_t)((npad + 31) / 32) * sizeof(unsigned), c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
   } else {
-    compose_perm_global_kernel<<<1, 32, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
+    compose_perm_global_kernel<<<1, 1024, 0, c->stream>>>(c->d_ipiv, c->d_rowperm, (int)npad);
   }
   c->launches++;
   NEB_CUDA(c, cudaGetLastError());
