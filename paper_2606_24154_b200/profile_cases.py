@@ -22,6 +22,8 @@ Cases (all through the C ABI; inputs from workloads/, seeded):
   charges             1e5 points x 2e5 point charges                                           -> charge_kernel
   lines               1e5 points x the line charges of a voxelised 2e5-charge cloud            -> line_kernel
   lu_c1 / trisolve_c1 C1: factorisation and the two triangular solves                          -> panel/gemm/tri_wave
+  max_n               (not in the default list) cube with 6 x 147^2 = 129654 panels, the largest mesh the panel cluster
+                      takes (npad = 129664 of 130944): 134 GB matrix, whole step, stage times
 """
 import sys
 
@@ -126,6 +128,18 @@ def run(cases):
             nb.solve()
             report(name, "panel_stream_kernel+gemm_kernel" if name == "lu_c1" else "tri_wave_kernel", pr.n,
                    "lu" if name == "lu_c1" else "trisolve", nb)
+            nb.close()
+        elif name == "max_n":
+            pr = W.cube(n_side=147, m_points=1000)
+            nb = Neb()
+            nb.set_option(B.NEB_OPT_PROFILE, 1)
+            nb.assemble_problem(pr)
+            sig = nb.solve()
+            nb.eval(torch.from_numpy(pr.points).cuda())
+            st = {k: round(v[0], 2) for k, v in nb.stage_ms().items() if v[0] > 0}
+            cap = float(sig.sum() * (pr.meta["side"] / 147) ** 2 / (4 * np.pi * 8.8541878128e-12 * pr.meta["side"]))
+            print(f"case max_n kernel all units {pr.n} stages_ms {st} lu_tflops {nb.counter(1) / st['lu'] * 1e-9:.2f} "
+                  f"trisolve_gbs {8.0 * pr.n ** 2 / st['trisolve'] * 1e-6:.0f} capacitance/(4 pi eps0 a) {cap:.6f}", flush=True)
             nb.close()
         else:
             raise SystemExit(f"unknown case {name}")
