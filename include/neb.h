@@ -183,7 +183,8 @@ neb_status neb_eval(neb_ctx* ctx, int64_t m, const double* pts, double* phi, dou
  * allocate); either output may be NULL.  The call issues kernels on the context's stream and calls no cudaMalloc,
  * cudaFree or other allocating routine.  All contexts of a device share the one array: calls that overlap on the GPU
  * (contexts on different streams) race on it; calls on one stream are ordered and need no clearing in between (every
- * call overwrites the part it reads). */
+ * call overwrites the part it reads).  With NEB_OPT_PROFILE = 1 the stage timers synchronise on their events after every
+ * stage: leave profiling off (the default) where a synchronisation is not allowed, e.g. under stream capture. */
 #define NEB_EVAL_STATIC_MAX_POINTS 65536
 neb_status neb_eval_static(neb_ctx* ctx, int64_t m, const double* pts, double* phi, double* E);
 
