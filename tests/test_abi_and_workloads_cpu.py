@@ -101,3 +101,13 @@ def test_bench_reads_its_roofline_constants_from_the_committed_tables():
     from workloads import configs as W
     fl, inst = bench.flop_per_pair(W.thgem(d=10, n_plane=6, n_grid=2), ops)
     assert ops["eval_tri_uniform"]["flop"] <= fl <= ops["eval_rect_uniform"]["flop"] and inst < fl
+
+
+def test_no_alloc_test_file_is_collected_last():
+    """tests/test_zz_no_alloc.py must stay the last file pytest collects (alphabetical order): the suite runs with
+    `pytest -x`, and a failure in that file must not hide any other test."""
+    import glob
+    import os
+    here = os.path.dirname(os.path.abspath(__file__))
+    files = sorted(os.path.basename(p) for p in glob.glob(os.path.join(here, "test_*.py")))
+    assert files[-1] == "test_zz_no_alloc.py", files
